@@ -1,0 +1,120 @@
+/*
+ * nfs.h — C ABI of the B200 (sm_100a) hot path of the double-frame differential analysis of
+ * dynamic near-field-scattering / shadowgraph / DDM image stacks (arxiv 1209.3362,
+ * Cerchiari, Croccolo, Cardinaux, Scheffold).  Citations are lines of /root/reference/PAPER.md.
+ *
+ * What the library computes (the paper's method; readings R1-R18 in DESIGN.md §3):
+ *   1. every pushed uint16 frame is normalised by its spatial mean
+ *   2. and Fourier-transformed exactly once, 2-D real-to-complex, unitary      (L25, L31)
+ *   3. the transformed frames live in a ring buffer in HBM — the role of the
+ *      paper's G-RAM FIFO of image FFTs, Fig. 2(a)                             (L33, L37)
+ *   4. for every requested lag tau the structure function
+ *        D2d(k,tau) = < |F_t(k) - F_{t+tau}(k)|^2 >_t   over all N-tau pairs   (L21, L25, L31-33)
+ *      is accumulated in Fourier space (linearity, L31), and the static spectrum
+ *        I2d(k) = < |F_t(k)|^2 >_t                                             (R9)
+ *   5. both are azimuthally averaged into n_qbins uniform |q| bins on [0, q_Nyquist),
+ *      DC pixel excluded, bin index by exact integer arithmetic                (L25; R6, R7)
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback and no cuFFT.
+ * One context = one CUDA stream = not thread-safe; contexts are independent; no global state.
+ * All functions return 0 (NFS_OK) or a negative nfs_status; nothing throws or aborts across
+ * this boundary.  Errors NFS_ERR_CUDA and NFS_ERR_ZERO_MEAN are sticky: once raised every later
+ * call on the context returns them until nfs_reset().
+ */
+#ifndef NFS_H_
+#define NFS_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define NFS_API __attribute__((visibility("default")))
+#else
+#define NFS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nfs_ctx nfs_ctx; /* opaque, owned by the library */
+
+typedef enum nfs_status {
+  NFS_OK = 0,
+  NFS_ERR_INVALID_ARG = -1, /* NULL pointer; W or H not a power of two in [32,4096]; n_lags < 1; lags not
+                               strictly increasing or < 1; n_qbins < 1; n < 1; index out of range   */
+  NFS_ERR_OOM = -2,         /* ring + accumulators do not fit the free device memory (checked at create) */
+  NFS_ERR_CUDA = -3,        /* first failing CUDA call (sticky)                                        */
+  NFS_ERR_ZERO_MEAN = -4,   /* a pushed frame summed to zero: its normalisation (L21) is undefined.
+                               Detected on the device, surfaced by the next synchronising call (sticky) */
+  NFS_ERR_STATE = -5,       /* call not valid in this state (e.g. finalize before any frame)           */
+  NFS_ERR_UNSUPPORTED = -6  /* W != H (all of the paper's sizes, L33, are square)                      */
+} nfs_status;
+
+/*
+ * nfs_create — plan memory and build the tables ("optimize memory allocation prior to
+ * starting the calculations"; here the trivial alpha=1 case of Fig. 2(a): ring = Lmax + batch frames).
+ *   out       HOST  receives the context.
+ *   W,H             frame size in pixels, powers of two in [32,4096], W == H.
+ *   lags      HOST  [n_lags] lags in frames, >= 1, strictly increasing (copied).
+ *   n_qbins         number of |q| bins on [0, pi rad/px).
+ *   cuda_stream     a cudaStream_t cast to void*, or NULL for a library-owned stream.  All device
+ *                   work of this context is enqueued on it.
+ * nfs_create_ex additionally fixes the internal batch size (frames transformed and accumulated per
+ * kernel wave; 0 = default 256).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
+ */
+NFS_API int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream);
+NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                  int batch_frames);
+
+/*
+ * nfs_push_frames — steps 1-4 for n more frames.
+ *   d_frames  DEVICE [n][H][W] uint16, row-major, x fastest, pitch W, no padding.
+ * Stream-ordered and asynchronous to the host: d_frames must stay valid and unmodified until the
+ * work enqueued by this call on the context's stream has run (record an event after the call).
+ * Frames are numbered in push order; results do not depend on how a stack is split across calls
+ * beyond fp32 partial-sum rounding (<= 1e-6 relative).
+ */
+NFS_API int nfs_push_frames(nfs_ctx* ctx, const uint16_t* d_frames, int n);
+
+/*
+ * nfs_finalize — step 5 ("azimuthally averaged power spectra") for the N frames pushed
+ * so far.  Synchronises the stream; non-destructive snapshot: pushing may continue afterwards.
+ *   D_q_tau   HOST [n_lags][n_qbins] double   mean of D2d over bin b; rows with tau >= N are 0.
+ *   I_q       HOST [n_qbins] double           mean of I2d over bin b.
+ *   counts    HOST [n_qbins] int64            full-plane pixel count of each bin (data independent).
+ * Empty bins hold 0.0 / 0.  Any of the three may be NULL to skip it.
+ */
+NFS_API int nfs_finalize(nfs_ctx* ctx, double* D_q_tau, double* I_q, int64_t* counts);
+
+/* n_pairs HOST [n_lags]: N - tau, or 0 when tau >= N (N(N-1)/2 pairs over N-1 lags). */
+NFS_API int nfs_get_pair_counts(nfs_ctx* ctx, int64_t* n_pairs);
+
+/* Averaged 2-D spectra on the half plane, HOST [H][W/2+1] double, FFT order (ky = 0..H/2-1,-H/2..-1;
+ * kx = 0..W/2), unitary scale (|F(0)|^2 = W*H for a normalised frame).  Synchronise the stream. */
+NFS_API int nfs_get_D2d(nfs_ctx* ctx, int lag_index, double* out);
+NFS_API int nfs_get_I2d(nfs_ctx* ctx, double* out);
+
+/* Number of frames pushed so far; ring capacity in frames; bytes of device memory held. */
+NFS_API int64_t nfs_num_frames(const nfs_ctx* ctx);
+NFS_API int nfs_ring_capacity(const nfs_ctx* ctx);
+NFS_API int64_t nfs_device_bytes(const nfs_ctx* ctx);
+
+/* Kernel launches enqueued by this context since create/reset (bench.py's gpu_launches). */
+NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
+
+/* Lag-accumulation kernel variant: 0 = tiled shared-memory kernel (default), 1 = plain per-pixel
+ * kernel reading the ring through L1/L2 (kept as an in-library cross-check; same results up to
+ * fp32 summation order).  Not a backend switch: both are CUDA kernels of this library. */
+NFS_API int nfs_set_lag_kernel(nfs_ctx* ctx, int variant);
+
+/* Forget all frames (accumulators, ring, reference, sticky errors); keeps the plan and the memory. */
+NFS_API int nfs_reset(nfs_ctx* ctx);
+NFS_API void nfs_destroy(nfs_ctx* ctx);
+NFS_API const char* nfs_strerror(int status);
+/* Text of the first CUDA error seen by this context ("" if none). */
+NFS_API const char* nfs_last_cuda_error(const nfs_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NFS_H_ */

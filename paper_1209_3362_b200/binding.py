@@ -1,0 +1,180 @@
+"""Thin Python binding of include/nfs.h (argument marshalling only; every step runs in the CUDA kernels).
+
+Same names as the C ABI: nfs_create / nfs_push_frames / nfs_finalize / getters, plus a small
+`NFS` convenience class.  torch is used only for device memory and streams.  There is no CPU
+fallback: if libnfs_b200.so is missing or does not load, importing this module raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnfs_b200.so")
+
+NFS_OK = 0
+NFS_ERR_INVALID_ARG = -1
+NFS_ERR_OOM = -2
+NFS_ERR_CUDA = -3
+NFS_ERR_ZERO_MEAN = -4
+NFS_ERR_STATE = -5
+NFS_ERR_UNSUPPORTED = -6
+
+# every symbol include/nfs.h declares: (name, restype, argtypes)
+_P = C.c_void_p
+SYMBOLS = [
+    ("nfs_create", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P]),
+    ("nfs_create_ex", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int]),
+    ("nfs_push_frames", C.c_int, [_P, _P, C.c_int]),
+    ("nfs_finalize", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
+    ("nfs_get_pair_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
+    ("nfs_get_D2d", C.c_int, [_P, C.c_int, C.POINTER(C.c_double)]),
+    ("nfs_get_I2d", C.c_int, [_P, C.POINTER(C.c_double)]),
+    ("nfs_num_frames", C.c_int64, [_P]),
+    ("nfs_ring_capacity", C.c_int, [_P]),
+    ("nfs_device_bytes", C.c_int64, [_P]),
+    ("nfs_num_launches", C.c_int64, [_P]),
+    ("nfs_set_lag_kernel", C.c_int, [_P, C.c_int]),
+    ("nfs_reset", C.c_int, [_P]),
+    ("nfs_destroy", None, [_P]),
+    ("nfs_strerror", C.c_char_p, [C.c_int]),
+    ("nfs_last_cuda_error", C.c_char_p, [_P]),
+]
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """Loads the C-ABI library; raises (never falls back) if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(path):
+            raise ImportError(
+                "%s not found: build it with `python -m paper_1209_3362_b200.build` "
+                "(there is no CPU fallback for the hot path)" % path)
+        lib = C.CDLL(path)
+        for name, res, args in SYMBOLS:
+            fn = getattr(lib, name)  # AttributeError if the symbol is not exported
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+class NFSError(RuntimeError):
+    def __init__(self, status, detail=""):
+        self.status = status
+        msg = load_library().nfs_strerror(status).decode()
+        super().__init__("nfs status %d: %s%s" % (status, msg, (" [" + detail + "]") if detail else ""))
+
+
+def _check(rc, handle=None):
+    if rc != NFS_OK:
+        detail = ""
+        if handle and rc == NFS_ERR_CUDA:
+            detail = load_library().nfs_last_cuda_error(handle).decode()
+        raise NFSError(rc, detail)
+
+
+def _dp(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+# ---- functions with the C names -----------------------------------------------------------------------
+def nfs_create(W, H, lags, n_qbins, cuda_stream=None, batch_frames=0):
+    lg = np.ascontiguousarray(lags, dtype=np.int32)
+    h = _P()
+    rc = load_library().nfs_create_ex(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins),
+                                      _P(cuda_stream) if cuda_stream else None, int(batch_frames))
+    _check(rc)
+    return h
+
+
+def nfs_push_frames(handle, d_frames_ptr: int, n: int):
+    _check(load_library().nfs_push_frames(handle, _P(d_frames_ptr), int(n)), handle)
+
+
+def nfs_finalize(handle, n_lags, n_qbins):
+    D = np.zeros((n_lags, n_qbins), dtype=np.float64)
+    I_q = np.zeros(n_qbins, dtype=np.float64)
+    cnt = np.zeros(n_qbins, dtype=np.int64)
+    _check(load_library().nfs_finalize(handle, _dp(D, C.c_double), _dp(I_q, C.c_double), _dp(cnt, C.c_int64)), handle)
+    return D, I_q, cnt
+
+
+def nfs_destroy(handle):
+    load_library().nfs_destroy(handle)
+
+
+# ---- convenience wrapper ----------------------------------------------------------------------------------
+class NFS:
+    """One context.  `push(frames)` takes a CUDA uint16 torch tensor [n][H][W] (contiguous)."""
+
+    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0):
+        self.lib = load_library()
+        self.W, self.H, self.n_qbins = int(W), int(H), int(n_qbins)
+        self.lags = [int(t) for t in lags]
+        self._stream = stream  # torch.cuda.Stream or None (library-owned stream)
+        self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None,
+                                 batch_frames)
+
+    def push(self, frames):
+        import torch
+
+        assert frames.is_cuda and frames.dtype == torch.uint16 and frames.is_contiguous()
+        assert frames.dim() == 3 and frames.shape[1] == self.H and frames.shape[2] == self.W
+        nfs_push_frames(self.handle, frames.data_ptr(), frames.shape[0])
+
+    def push_ptr(self, ptr, n):
+        nfs_push_frames(self.handle, ptr, n)
+
+    def finalize(self):
+        return nfs_finalize(self.handle, len(self.lags), self.n_qbins)
+
+    def pair_counts(self):
+        out = np.zeros(len(self.lags), dtype=np.int64)
+        _check(self.lib.nfs_get_pair_counts(self.handle, _dp(out, C.c_int64)), self.handle)
+        return out
+
+    def D2d(self, lag_index):
+        out = np.zeros((self.H, self.W // 2 + 1), dtype=np.float64)
+        _check(self.lib.nfs_get_D2d(self.handle, int(lag_index), _dp(out, C.c_double)), self.handle)
+        return out
+
+    def I2d(self):
+        out = np.zeros((self.H, self.W // 2 + 1), dtype=np.float64)
+        _check(self.lib.nfs_get_I2d(self.handle, _dp(out, C.c_double)), self.handle)
+        return out
+
+    def set_lag_kernel(self, variant):
+        _check(self.lib.nfs_set_lag_kernel(self.handle, int(variant)), self.handle)
+
+    def reset(self):
+        _check(self.lib.nfs_reset(self.handle), self.handle)
+
+    @property
+    def num_frames(self):
+        return int(self.lib.nfs_num_frames(self.handle))
+
+    @property
+    def num_launches(self):
+        return int(self.lib.nfs_num_launches(self.handle))
+
+    @property
+    def ring_capacity(self):
+        return int(self.lib.nfs_ring_capacity(self.handle))
+
+    @property
+    def device_bytes(self):
+        return int(self.lib.nfs_device_bytes(self.handle))
+
+    def close(self):
+        if self.handle is not None:
+            nfs_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

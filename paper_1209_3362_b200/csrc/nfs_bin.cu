@@ -1,0 +1,100 @@
+// nfs_bin.cu — step S6 of the hot path: averages over pairs and deterministic azimuthal binning
+// ("azimuthally averaged power spectra"; readings R6-R10 in DESIGN.md).
+//
+// The |q|-bin of every half-plane Fourier pixel is precomputed on the host with exact integer
+// arithmetic and the pixels are grouped by bin (perm / bin_start), each entry carrying its Hermitian
+// weight (2 for 0 < kx < W/2, 1 for kx in {0, W/2}).  One CTA reduces one (row, bin) segment in a
+// fixed order: per-thread strided fp64 sums, then a fixed shuffle/shared tree — no float atomics, so
+// results are bit-identical from run to run.
+#include "nfs_common.cuh"
+
+namespace nfs {
+
+// value of the static spectrum at pixel p: I2d = (sum|F'|^2 + 2 Re(sum F' conj F_r)) / N + |F_r|^2
+__device__ __forceinline__ double i2d_value(const double* __restrict__ I2, const double2* __restrict__ I1,
+                                            const float2* __restrict__ Fref, int64_t p, double invN) {
+  const float2 fr = Fref[p];
+  const double2 s1 = I1[p];
+  const double rx = (double)fr.x, ry = (double)fr.y;
+  return (I2[p] + 2.0 * (s1.x * rx + s1.y * ry)) * invN + (rx * rx + ry * ry);
+}
+
+// grid (n_qbins, n_lags + 1), 128 threads.  Row l < n_lags: D(b, tau_l); row n_lags: I(b).
+__global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, const double* __restrict__ I2,
+                                             const double2* __restrict__ I1, const float2* __restrict__ Fref,
+                                             const uint32_t* __restrict__ perm, const int32_t* __restrict__ bin_start,
+                                             const int32_t* __restrict__ lags, int n_lags, int n_qbins, int64_t P,
+                                             int64_t N, double* __restrict__ out) {
+  const int b = blockIdx.x, row = blockIdx.y;
+  const int beg = bin_start[b], end = bin_start[b + 1];
+  double inv;
+  if (row < n_lags) {
+    const int64_t np = N - (int64_t)lags[row];
+    inv = np > 0 ? 1.0 / (double)np : 0.0;
+  } else {
+    inv = 1.0 / (double)N;
+  }
+  double acc = 0.0, wsum = 0.0;
+  for (int i = beg + (int)threadIdx.x; i < end; i += 128) {
+    const uint32_t e = perm[i];
+    const int64_t p = (int64_t)(e & 0x7fffffffu);
+    const double wgt = (e >> 31) ? 2.0 : 1.0;
+    double v;
+    if (row < n_lags)
+      v = totals[(int64_t)row * P + p] * inv;
+    else
+      v = i2d_value(I2, I1, Fref, p, inv);
+    acc += wgt * v;
+    wsum += wgt;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+  }
+  __shared__ double sa[4], sw[4];
+  if ((threadIdx.x & 31) == 0) {
+    sa[threadIdx.x >> 5] = acc;
+    sw[threadIdx.x >> 5] = wsum;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const double a = (sa[0] + sa[1]) + (sa[2] + sa[3]);
+    const double w = (sw[0] + sw[1]) + (sw[2] + sw[3]);
+    out[(int64_t)row * n_qbins + b] = (w > 0.0 && inv > 0.0) ? a / w : 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_I2d(const double* __restrict__ I2, const double2* __restrict__ I1,
+                                             const float2* __restrict__ Fref, int64_t P, int64_t N,
+                                             double* __restrict__ dst) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < P) dst[p] = i2d_value(I2, I1, Fref, p, 1.0 / (double)N);
+}
+
+__global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int64_t P, double inv,
+                                             double* __restrict__ dst) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < P) dst[p] = tot[p] * inv;
+}
+
+int launch_bin(Ctx& c) {
+  dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 1));
+  k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.I2, c.I1, c.Fref, c.perm, c.bin_start, c.d_lags, c.n_lags, c.n_qbins,
+                                    c.P, c.n_frames, c.d_out);
+  return 1;
+}
+
+int launch_I2d(Ctx& c, double* d_dst) {
+  k_I2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, c.n_frames, d_dst);
+  return 1;
+}
+
+int launch_D2d(Ctx& c, int l, double* d_dst) {
+  const int64_t np = c.n_frames - (int64_t)c.lags[l];
+  const double inv = np > 0 ? 1.0 / (double)np : 0.0;
+  k_D2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.totals + (int64_t)l * c.P, c.P, inv, d_dst);
+  return 1;
+}
+
+}  // namespace nfs

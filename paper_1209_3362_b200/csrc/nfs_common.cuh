@@ -1,0 +1,96 @@
+// nfs_common.cuh — shared declarations of the CUDA hot path (product code; shares nothing with oracle/).
+//
+// Data layout in HBM.  n = W/2, P = H*(n+1) Fourier pixels per frame (half plane):
+//   Fourier frame  float2[P]  = main block [H][n]  (kx = 0..n-1, 16-byte aligned rows)
+//                               followed by the Nyquist column [H]  (kx = n), so that every row of
+//                               the main block is 16-byte aligned.
+//   ring           float2[R][P], slot(t) = t mod R, R = Lmax + batch   (PAPER.md:L33 FIFO of image FFTs)
+//   totals         double[n_lags][P]   sum over pairs of |F'_t - F'_{t+tau}|^2   ("differences area", L33)
+//   ref            float[H][W]   first normalised frame r; F'_t = FFT(i_t - r)   (linearity, L31)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/nfs.h"
+
+namespace nfs {
+
+// ---- lag-accumulation plan (built on the host at create) -------------------------------------------
+constexpr int kG = 10;        // lags per warp task (register window depth)
+constexpr int kTilePx = 32;   // Fourier pixels per CTA tile (one warp width)
+constexpr int kMaxTasks = 10; // warp tasks per CTA (lag group)
+constexpr int kChunk = 20;    // time steps per shared-memory pipeline stage (multiple of kG)
+constexpr int kSpanMax = 128; // max (tau_max - tau_min + 1) of a lag group
+
+struct LagTask {
+  int tau0;  // dense: smallest lag of the run; sparse: unused
+  int cnt;   // number of lags handled (<= kG)
+  int l0;    // index of the first lag in the sorted lag list
+  int kind;  // 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt)
+};
+struct LagGroup {
+  int task0, ntasks;
+  int tau_min, tau_max;
+};
+
+struct Ctx {
+  int W = 0, H = 0, n = 0;  // n = W/2
+  int64_t P = 0;
+  int n_lags = 0, n_qbins = 0, Lmax = 0;
+  int B = 0;   // internal batch (frames)
+  int R = 0;   // ring slots
+  int Bf = 0;  // frames per FFT sub-batch
+  std::vector<int32_t> lags;
+  std::vector<int64_t> counts;  // full-plane pixel count per bin
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  int64_t n_frames = 0;
+  int64_t n_launches = 0;
+  int lag_variant = 0;
+  int status = 0;  // sticky
+  std::string cuda_err;
+  int64_t dev_bytes = 0;
+  int max_smem_optin = 0;
+
+  // device memory
+  float2* ring = nullptr;
+  float2* rowbuf = nullptr;      // [Bf][P] output of the row pass
+  float* ref = nullptr;          // [H][W]
+  float2* Fref = nullptr;        // [P] unitary FFT of ref
+  double* totals = nullptr;      // [n_lags][P]
+  double* I2 = nullptr;          // [P]  sum_t |F'_t|^2
+  double2* I1 = nullptr;         // [P]  sum_t F'_t
+  unsigned long long* sums = nullptr;  // [Bf + 1] exact pixel sums of the frames of a sub-batch
+  float2* tw = nullptr;          // [W] exp(-2 pi i k / W)   (W == H)
+  int32_t* d_lags = nullptr;     // [n_lags]
+  uint32_t* perm = nullptr;      // [n_binned] pixel index | (weight-2 flag << 31), grouped by bin
+  int32_t* bin_start = nullptr;  // [n_qbins + 1]
+  double* d_out = nullptr;       // [(n_lags + 1)][n_qbins] binned results
+  double* d_tmp = nullptr;       // [P] scratch for the 2-D getters
+  int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
+  LagTask* d_tasks = nullptr;
+  LagGroup* d_groups = nullptr;
+  std::vector<LagTask> tasks;
+  std::vector<LagGroup> groups;
+};
+
+// ---- kernel launchers (each returns the number of kernel launches it enqueued; sets cudaGetLastError) ----
+// nfs_fft.cu
+int launch_frame_sums(Ctx& c, const uint16_t* frames, int nf);
+int launch_make_ref(Ctx& c, const uint16_t* frame0);
+int launch_fft_ref(Ctx& c);                                       // Fref = FFT(ref)
+int launch_fft_frames(Ctx& c, const uint16_t* frames, int nf, int64_t t_first);  // ring[t_first..] = FFT(i_t - ref)
+// nfs_lag.cu
+int launch_accum_I(Ctx& c, int64_t t0, int b);
+int launch_lag_simple(Ctx& c, int64_t t0, int b);
+int launch_lag_tiled(Ctx& c, int64_t t0, int b);
+size_t lag_tiled_smem_bytes(const LagGroup& g);
+// nfs_bin.cu
+int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)
+int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
+int launch_D2d(Ctx& c, int l, double* d_dst);
+
+}  // namespace nfs
