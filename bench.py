@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the D(q,tau) hot path on synthetic stacks shaped like BASELINE.json's configs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (frame sums, normalise, 2-D R2C FFT, HBM ring, lag
+accumulation, azimuthal binning) over one whole synthetic stack: reset -> nfs_push_frames -> nfs_finalize.
+`value` = frames/s with the uint16 stack already resident in HBM; `e2e` = the same through the C-ABI
+with the stack in pinned HOST memory (chunked H2D copies overlapped with compute, result D2H), both timed
+with CUDA events / synchronised wall clock.  Prints ONE JSON line (rank 0).
+Multi-GPU: replicas only: every rank analyses its own stack, no data-path collective.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+SM_COUNT = 148
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for k, nm in enumerate(names):
+                    if r[3 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def workload_counts(cfg):
+    P = cfg.H * (cfg.W // 2 + 1)
+    pairs = sum(max(0, cfg.N - t) for t in cfg.lags)
+    return P, pairs
+
+
+def oracle_sample(cfg, stack_np_fn):
+    """The oracle, as it stands, on a bounded sample of the workload -> (frames/s, seconds, description, cores)."""
+    from oracle import nfs_oracle as orc
+
+    n_s = min(cfg.N, 128 if cfg.W >= 1024 else (400 if cfg.W >= 512 else cfg.N))
+    fr = stack_np_fn(n_s)
+    t = time.time()
+    orc.structure_function(fr, cfg.lags, cfg.n_qbins)
+    dt = time.time() - t
+    desc = "first %d frames of the %dx%d stack, all %d lags, full-plane fp64 oracle (oracle/nfs_oracle.c)" % (
+        n_s, cfg.W, cfg.H, len(cfg.lags))
+    return n_s / dt, dt, desc, orc.num_threads()
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle on the box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_1209_3362_b200 import synth
+
+    gen = synth.SynthStack(cfg, "cpu")
+    n_s = min(cfg.N, 128 if cfg.W >= 1024 else (400 if cfg.W >= 512 else cfg.N))
+    frames = gen.next_frames(n_s).numpy()
+    times = []
+    desc, cores = "", 0
+    for i in range(args.warmup + args.steps):
+        v, dt, desc, cores = oracle_sample(cfg, lambda n: frames[:n])
+        if i >= args.warmup:
+            times.append(dt)
+    T = sum(times) / len(times)
+    val = n_s / T
+    out = dict(metric="frames_per_s", value=val, unit="frames/s", n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+               ms_per_step=T * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+               impl="reference",
+               config=dict(workload="%s: %dx%d uint16, %d lags, %d |q| bins (bounded sample: %d of %d frames)" % (
+                   cfg.name, cfg.W, cfg.H, len(cfg.lags), cfg.n_qbins, n_s, cfg.N)),
+               cpu_baseline=dict(value=val, unit="frames/s", cores=cores, kind="oracle", sample=desc),
+               e2e=dict(value=val, unit="frames/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: 1024^2 x 2000, 100 lags)")
+    ap.add_argument("--frames", type=int, default=0, help="override the number of frames (debug)")
+    ap.add_argument("--batch", type=int, default=0, help="internal batch size (0 = library default)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    from paper_1209_3362_b200 import synth
+
+    cfg = synth.config(args.config)
+    if args.frames:
+        cfg.N = args.frames
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    run_ours(args, cfg)
+
+
+def run_ours(args, cfg):
+    import torch
+    from paper_1209_3362_b200 import binding, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --impl ours needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    peaks = load_peaks()
+    P, pairs = workload_counts(cfg)
+    updates = pairs * P
+
+    # every rank analyses its own stack (replicas; seed differs per rank)
+    cfg_r = cfg if rank == 0 else synth.StackConfig(**{**cfg.__dict__, "seed": cfg.seed + 100 * rank, "fringes": []})
+    stack = synth.make_stack(cfg_r, dev)
+    stream = torch.cuda.Stream(device=dev)
+    nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch)
+    nfs.set_profiling(True)
+    torch.cuda.synchronize()
+
+    def step():
+        nfs.reset()
+        nfs.push(stack)
+        return nfs.finalize()
+
+    for _ in range(max(args.warmup, 1) if args.warmup else 0):
+        step()
+    nfs.kernel_times()
+    launches0 = 0
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall = time.time()
+    e0.record(stream)
+    n_launch = 0
+    for _ in range(args.steps):
+        step()
+        n_launch += nfs.num_launches
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t_wall = time.time() - t_wall
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    ktimes = nfs.kernel_times()
+    if dist is not None:
+        tt = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    value = world * cfg.N / (ms_step * 1e-3)
+
+    # ---- end to end through the C-ABI with the stack in pinned HOST memory ----
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (lag accumulation) ----
+    lag_ms, lag_n = ktimes["lag_accum"]
+    lag_s_per_step = lag_ms * 1e-3 / args.steps
+    flop_per_update = 6.0          # 2 sub + 2 mul + 2 add
+    inst_per_update = 4.0          # 2 FADD + 2 FFMA lane-instructions
+    peak_tflops = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * (flop_per_update / inst_per_update) / 1e12
+    ach_tflops = updates * flop_per_update / lag_s_per_step / 1e12
+    B = args.batch or 256
+    nb = (cfg.N + B - 1) // B
+    lag_bytes = P * (8.0 * (cfg.N + nb * (cfg.lags[-1])) * (1 + 0) + 16.0 * len(cfg.lags) * nb)
+    fft_ms = ktimes["frame_sum"][0] + ktimes["fft_row"][0] + ktimes["fft_col"][0]
+    fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N
+    roofline = dict(bound="alu", kernel="k_lag_tiled", achieved=ach_tflops, peak=peak_tflops, unit="TFLOP/s",
+                    frac=ach_tflops / peak_tflops, traffic=None,
+                    peak_source="148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) x 1.5 flop/lane-instr "
+                                "(2 FADD + 2 FFMA per pair-update)" % (peaks["sm_max_mhz"], peaks["source"]),
+                    pair_updates_per_s=updates / lag_s_per_step, ms_per_step=lag_s_per_step * 1e3, launches_per_step=lag_n / args.steps,
+                    hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / lag_s_per_step / 1e9,
+                             peak_gbs=peaks["hbm_gbs"], frac=lag_bytes / lag_s_per_step / 1e9 / peaks["hbm_gbs"]))
+    fft = dict(bound="hbm", ms_per_step=fft_ms / args.steps, algorithmic_gb_per_step=fft_bytes / 1e9,
+               achieved_gbs=fft_bytes / (fft_ms / args.steps * 1e-3) / 1e9, peak_gbs=peaks["hbm_gbs"],
+               frac=fft_bytes / (fft_ms / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    kernels = {k: dict(ms_per_step=v[0] / args.steps, launches_per_step=v[1] / args.steps) for k, v in ktimes.items()}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, dt, desc, cores = oracle_sample(cfg, lambda n: stack[:n].cpu().numpy())
+        cpu = dict(value=v, unit="frames/s", cores=cores, kind="oracle", sample=desc, seconds=dt)
+
+    out = dict(metric="frames_per_s", value=value, unit="frames/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
+               ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+               config=dict(workload="%s: %dx%d uint16 x %d frames, %d lags (max %d), %d |q| bins" % (
+                   cfg.name, cfg.W, cfg.H, cfg.N, len(cfg.lags), cfg.lags[-1], cfg.n_qbins),
+                   parallelism="replicas x%d" % world, internal_batch=B,
+                   l2_policy="inputs larger than L2 (%.2f GB stack streamed from HBM every step)" % (stack.numel() * 2 / 1e9)),
+               frame_pairs_per_s=world * pairs / (ms_step * 1e-3), pair_updates_per_s=world * updates / (ms_step * 1e-3),
+               wall_s_per_step=t_wall / args.steps, gpu_launches=n_launch, clocks=clocks, e2e=e2e, roofline=roofline,
+               fft=fft, kernels=kernels, cpu_baseline=cpu)
+    print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
+    """Stack in pinned host memory; chunks of `chunk` frames double-buffered through two device staging
+    buffers on a copy stream, pushed through the C-ABI, result read back by nfs_finalize."""
+    chunk = cfg.chunk or 256
+    chunk = min(chunk, cfg.N)
+    host = torch.empty(stack.shape, dtype=torch.uint16, pin_memory=True)
+    host.copy_(stack)
+    torch.cuda.synchronize()
+    stage = [torch.empty((chunk, cfg.H, cfg.W), dtype=torch.uint16, device=dev) for _ in range(2)]
+    copy_stream = torch.cuda.Stream(device=dev)
+    copied = [torch.cuda.Event() for _ in range(2)]
+    consumed = [torch.cuda.Event() for _ in range(2)]
+
+    def step():
+        nfs.reset()
+        i, k = 0, 0
+        while i < cfg.N:
+            m = min(chunk, cfg.N - i)
+            b = k & 1
+            with torch.cuda.stream(copy_stream):
+                if k >= 2:
+                    copy_stream.wait_event(consumed[b])
+                stage[b][:m].copy_(host[i:i + m], non_blocking=True)
+                copied[b].record(copy_stream)
+            stream.wait_event(copied[b])
+            nfs.push_ptr(stage[b].data_ptr(), m)
+            consumed[b].record(stream)
+            i += m
+            k += 1
+        return nfs.finalize()
+
+    step()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    steps = max(1, min(args.steps, 3))
+    t = time.time()
+    for _ in range(steps):
+        D, I, cnt = step()
+    torch.cuda.synchronize()
+    dt = (time.time() - t) / steps
+    if dist is not None:
+        tt = torch.tensor([dt], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+    del host
+    return dict(value=world * cfg.N / dt, unit="frames/s", h2d_bytes_per_step=int(stack.numel() * 2),
+                d2h_bytes_per_step=int(D.nbytes + I.nbytes + 4), ms_per_step=dt * 1e3, chunk_frames=chunk,
+                note="pinned host stack -> 2 device staging buffers (copy stream) -> nfs_push_frames -> nfs_finalize")
+
+
+if __name__ == "__main__":
+    main()

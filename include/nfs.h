@@ -102,6 +102,15 @@ NFS_API int64_t nfs_device_bytes(const nfs_ctx* ctx);
 /* Kernel launches enqueued by this context since create/reset (bench.py's gpu_launches). */
 NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
 
+/* Per-kernel timing for bench.py: when enabled, every kernel launch is bracketed by a CUDA event pair
+ * on the context's stream.  nfs_get_kernel_times synchronises, returns the accumulated milliseconds
+ * and launch counts per class since the last call — ms/launches are HOST [NFS_NUM_KERNEL_CLASSES], in
+ * the order: 0 frame sums (+reference), 1 FFT row pass, 2 FFT column pass, 3 I accumulation,
+ * 4 lag accumulation, 5 binning — and clears them. */
+#define NFS_NUM_KERNEL_CLASSES 6
+NFS_API int nfs_set_profiling(nfs_ctx* ctx, int enable);
+NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
+
 /* Lag-accumulation kernel variant: 0 = tiled shared-memory kernel (default), 1 = plain per-pixel
  * kernel reading the ring through L1/L2 (kept as an in-library cross-check; same results up to
  * fp32 summation order).  Not a backend switch: both are CUDA kernels of this library. */

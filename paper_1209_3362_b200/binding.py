@@ -35,11 +35,15 @@ SYMBOLS = [
     ("nfs_device_bytes", C.c_int64, [_P]),
     ("nfs_num_launches", C.c_int64, [_P]),
     ("nfs_set_lag_kernel", C.c_int, [_P, C.c_int]),
+    ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
+    ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_reset", C.c_int, [_P]),
     ("nfs_destroy", None, [_P]),
     ("nfs_strerror", C.c_char_p, [C.c_int]),
     ("nfs_last_cuda_error", C.c_char_p, [_P]),
 ]
+
+KERNEL_CLASSES = ["frame_sum", "fft_row", "fft_col", "accum_I", "lag_accum", "bin"]
 
 _lib = None
 
@@ -148,6 +152,16 @@ class NFS:
 
     def set_lag_kernel(self, variant):
         _check(self.lib.nfs_set_lag_kernel(self.handle, int(variant)), self.handle)
+
+    def set_profiling(self, enable):
+        _check(self.lib.nfs_set_profiling(self.handle, int(bool(enable))), self.handle)
+
+    def kernel_times(self):
+        """-> dict class -> (milliseconds, launches) since the last call (synchronises)."""
+        ms = np.zeros(len(KERNEL_CLASSES), dtype=np.float64)
+        n = np.zeros(len(KERNEL_CLASSES), dtype=np.int64)
+        _check(self.lib.nfs_get_kernel_times(self.handle, _dp(ms, C.c_double), _dp(n, C.c_int64)), self.handle)
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     def reset(self):
         _check(self.lib.nfs_reset(self.handle), self.handle)

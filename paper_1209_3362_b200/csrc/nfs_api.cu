@@ -189,6 +189,8 @@ void free_all(Ctx& c) {
                   c.d_lags, c.perm, c.bin_start, c.d_out,  c.d_tmp, c.d_flags, c.d_tasks, c.d_groups};
   for (void* p : ptrs)
     if (p) cudaFree(p);
+  for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
+  c.ev_pool.clear();
   if (c.own_stream && c.stream) cudaStreamDestroy(c.stream);
 }
 
@@ -410,6 +412,35 @@ int64_t nfs_num_launches(const nfs_ctx* h) { return h ? h->c.n_launches : 0; }
 int nfs_set_lag_kernel(nfs_ctx* h, int variant) {
   if (!h || variant < 0 || variant > 1) return NFS_ERR_INVALID_ARG;
   h->c.lag_variant = variant;
+  return NFS_OK;
+}
+
+int nfs_set_profiling(nfs_ctx* h, int enable) {
+  if (!h) return NFS_ERR_INVALID_ARG;
+  h->c.prof = enable != 0;
+  return NFS_OK;
+}
+
+int nfs_get_kernel_times(nfs_ctx* h, double* ms, int64_t* launches) {
+  if (!h) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (c.status != NFS_OK) return c.status;
+  if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
+  for (size_t i = 0; i < c.ev_class.size(); ++i) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, c.ev_pool[2 * i], c.ev_pool[2 * i + 1]) == cudaSuccess) {
+      c.prof_ms[c.ev_class[i]] += (double)t;
+      c.prof_n[c.ev_class[i]] += 1;
+    }
+  }
+  c.ev_class.clear();
+  c.ev_used = 0;
+  for (int k = 0; k < kNumKernelClasses; ++k) {
+    if (ms) ms[k] = c.prof_ms[k];
+    if (launches) launches[k] = c.prof_n[k];
+    c.prof_ms[k] = 0.0;
+    c.prof_n[k] = 0;
+  }
   return NFS_OK;
 }
 

@@ -80,6 +80,7 @@ __global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int
 
 int launch_bin(Ctx& c) {
   dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 1));
+  ProfScope ps(c, kKBin);
   k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.I2, c.I1, c.Fref, c.perm, c.bin_start, c.d_lags, c.n_lags, c.n_qbins,
                                     c.P, c.n_frames, c.d_out);
   return 1;

@@ -36,6 +36,9 @@ struct LagGroup {
   int tau_min, tau_max;
 };
 
+// kernel classes for the optional per-kernel CUDA-event timing (nfs_set_profiling)
+enum KernelClass { kKSum = 0, kKRow = 1, kKCol = 2, kKAccI = 3, kKLag = 4, kKBin = 5, kNumKernelClasses = 6 };
+
 struct Ctx {
   int W = 0, H = 0, n = 0;  // n = W/2
   int64_t P = 0;
@@ -75,6 +78,36 @@ struct Ctx {
   LagGroup* d_groups = nullptr;
   std::vector<LagTask> tasks;
   std::vector<LagGroup> groups;
+
+  // per-kernel timing: pairs of events recorded on the context's stream around each launch
+  bool prof = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  std::vector<int> ev_class;  // class of pair i (events 2i, 2i+1)
+  double prof_ms[kNumKernelClasses] = {0, 0, 0, 0, 0, 0};
+  int64_t prof_n[kNumKernelClasses] = {0, 0, 0, 0, 0, 0};
+};
+
+// RAII: records an event pair around the launches enqueued in its scope when profiling is on
+struct ProfScope {
+  Ctx& c;
+  cudaEvent_t stop = nullptr;
+  ProfScope(Ctx& ctx, int cls) : c(ctx) {
+    if (!c.prof) return;
+    while (c.ev_pool.size() < c.ev_used + 2) {
+      cudaEvent_t e;
+      cudaEventCreate(&e);
+      c.ev_pool.push_back(e);
+    }
+    cudaEvent_t start = c.ev_pool[c.ev_used];
+    stop = c.ev_pool[c.ev_used + 1];
+    c.ev_used += 2;
+    c.ev_class.push_back(cls);
+    cudaEventRecord(start, c.stream);
+  }
+  ~ProfScope() {
+    if (stop) cudaEventRecord(stop, c.stream);
+  }
 };
 
 // ---- kernel launchers (each returns the number of kernel launches it enqueued; sets cudaGetLastError) ----

@@ -345,6 +345,7 @@ int launch_frame_sums(Ctx& c, const uint16_t* frames, int nf) {
   int nblk = (int)((n16 + 256 * 8 - 1) / (256 * 8));
   if (nblk > 64) nblk = 64;
   if (nblk < 1) nblk = 1;
+  ProfScope ps(c, kKSum);
   cudaMemsetAsync(c.sums, 0, sizeof(unsigned long long) * nf, c.stream);
   k_frame_sum<<<dim3(nblk, nf), 256, 0, c.stream>>>(reinterpret_cast<const uint4*>(frames), n16, c.sums);
   return 1;
@@ -354,6 +355,7 @@ int launch_make_ref(Ctx& c, const uint16_t* frame0) {
   const int64_t npx = (int64_t)c.W * c.H;
   int nblk = (int)((npx + 1023) / 1024);
   if (nblk > 1184) nblk = 1184;
+  ProfScope ps(c, kKSum);
   k_make_ref<<<nblk, 256, 0, c.stream>>>(frame0, npx, (float)c.W * (float)c.H, c.sums, c.ref, c.d_flags);
   return 1;
 }
@@ -372,6 +374,7 @@ static int launch_row(Ctx& c, const uint16_t* frames, int nf) {
   int rpc, threads;
   size_t smem;
   row_cfg(c, rpc, threads, smem);
+  ProfScope ps(c, kKRow);
   k_row<MODE><<<dim3(c.H / rpc, nf), threads, smem, c.stream>>>(frames, c.ref, c.sums, c.rowbuf, c.tw, c.W, c.H, rpc,
                                                               c.d_flags);
   return 1;
@@ -385,6 +388,7 @@ static int launch_col(Ctx& c, float2* dst, int64_t t_first, int R, int nf) {
   const size_t smem = sizeof(float2) * (size_t)c.H * Cw;
   const float scale = (float)(1.0 / sqrt((double)c.W * (double)c.H));
   dim3 grid(c.n / Cw + 1, nf);
+  ProfScope ps(c, kKCol);
   if (lf == 1) {
     if (smem > 48 * 1024) cudaFuncSetAttribute(k_col<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_col<1><<<grid, threads, smem, c.stream>>>(c.rowbuf, dst, t_first, R, c.tw, c.W, c.H, Cw, scale);

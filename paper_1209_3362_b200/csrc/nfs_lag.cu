@@ -283,12 +283,14 @@ __global__ void __launch_bounds__(kMaxTasks * 32, 2)
 // launchers
 // ------------------------------------------------------------------------------------------------
 int launch_accum_I(Ctx& c, int64_t t0, int b) {
+  ProfScope ps(c, kKAccI);
   k_accum_I<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.ring, c.R, c.P, t0, b, c.I2, c.I1);
   return 1;
 }
 
 int launch_lag_simple(Ctx& c, int64_t t0, int b) {
   dim3 grid((unsigned)((c.P + 127) / 128), (unsigned)((c.n_lags + 7) / 8));
+  ProfScope ps(c, kKLag);
   k_lag_simple<<<grid, 128, 0, c.stream>>>(c.ring, c.R, c.P, t0, b, c.d_lags, c.n_lags, c.totals);
   return 1;
 }
@@ -302,6 +304,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   static_assert(kChunk % kG == 0, "chunk must hold whole blocks of kG steps");
   cudaFuncSetAttribute(k_lag_tiled<kG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   dim3 grid((unsigned)(c.P / kTilePx), (unsigned)c.groups.size());
+  ProfScope ps(c, kKLag);
   k_lag_tiled<kG><<<grid, kMaxTasks * 32, smem, c.stream>>>(c.ring, c.R, c.P, t0, b, c.d_tasks, c.d_groups, c.d_lags,
                                                           c.totals);
   return 1;
