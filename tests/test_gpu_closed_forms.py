@@ -1,0 +1,191 @@
+"""The CUDA path against what the mathematics fixes directly (the same closed forms that pin the oracle, SURVEY.md
+§8(c) P3-P6, P9), and — at BASELINE.json's full sizes, in the launch configuration bench.py times — against the
+oracle on sampled Fourier pixels plus properties that hold at any size."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1209_3362_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    assert torch.cuda.is_available()
+    from paper_1209_3362_b200 import binding as b
+
+    b.load_library()
+    return b
+
+
+def run(binding, stack_np, lags, n_b, batch=0):
+    st = torch.from_numpy(np.ascontiguousarray(stack_np)).cuda()
+    N, H, W = st.shape
+    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch)
+    nfs.push(st)
+    D, I_q, cnt = nfs.finalize()
+    D2d = np.stack([nfs.D2d(l) for l in range(len(lags))])
+    I2d = nfs.I2d()
+    nfs.close()
+    return D, I_q, cnt, D2d, I2d
+
+
+def test_constant_stack_gives_exact_zero(binding):
+    """P3: identical frames => every difference vanishes (L21); with the reference subtraction exactly."""
+    rng = np.random.default_rng(5)
+    img = rng.integers(100, 4000, size=(64, 64)).astype(np.uint16)
+    D, I_q, cnt, D2d, I2d = run(binding, np.repeat(img[None], 12, 0), [1, 2, 3, 7], 16)
+    assert np.all(D == 0.0) and np.all(D2d == 0.0)
+    assert I2d[0, 0] == pytest.approx(64 * 64, rel=1e-6)       # unitary scale: |F(0)|^2 = W H (reading R1)
+
+
+def test_gain_invariance(binding):
+    """P3: multiplying frame t by an integer gain leaves every output unchanged (normalisation by the mean, L21)."""
+    cfg = synth.config(0)
+    st = synth.make_stack(cfg, "cpu", n=12).numpy().astype(np.int64)
+    gains = np.array([1, 2, 3, 1, 5, 2, 1, 4, 3, 2, 1, 6])[:, None, None]
+    a = run(binding, st.astype(np.uint16), [1, 2, 3], 16)
+    b = run(binding, (st * gains).astype(np.uint16), [1, 2, 3], 16)
+    nz = a[2] > 0
+    assert np.abs(a[0][:, nz] - b[0][:, nz]).max() / a[0][:, nz].max() < 1e-5
+    assert np.abs(a[1][nz] - b[1][nz]).max() / a[1][nz].max() < 1e-5
+
+
+def test_telegraph_stack(binding):
+    """P5: frames alternate between P and Q: even lags give exactly 0, odd lags |F_P - F_Q|^2 for every tau."""
+    rng = np.random.default_rng(7)
+    Pimg = rng.integers(500, 3000, size=(64, 64)).astype(np.uint16)
+    Qimg = rng.integers(500, 3000, size=(64, 64)).astype(np.uint16)
+    st = np.stack([Pimg if t % 2 == 0 else Qimg for t in range(21)])
+    lags = [1, 2, 3, 4, 5, 6, 9, 12]
+    D, I_q, cnt, D2d, I2d = run(binding, st, lags, 16, batch=8)
+    ip = Pimg / Pimg.mean()
+    iq = Qimg / Qimg.mean()
+    ref = np.abs(np.fft.rfft2(ip - iq, norm="ortho")) ** 2
+    for l, tau in enumerate(lags):
+        if tau % 2 == 0:
+            assert np.all(D2d[l] == 0.0)
+        else:
+            m = ref > 1e-6 * ref.max()
+            assert (np.abs(D2d[l] - ref)[m] / ref[m]).max() < 1e-4
+
+
+def test_travelling_fringe_closed_form(binding):
+    """P4/P9: I_t = A + B cos(2 pi k0.x - w t): D2d(k0,tau) = (B/2A)^2 WH (2 - 2 cos w tau), all in one |q| bin."""
+    W = H = 64
+    A, B = 20000.0, 6000.0
+    k0x, k0y, w = 5, 3, 0.37
+    x = np.arange(W)[None, :]
+    y = np.arange(H)[:, None]
+    N = 40
+    st = np.stack([np.round(A + B * np.cos(2 * np.pi * (k0x * x / W + k0y * y / H) - w * t)) for t in range(N)])
+    lags = [1, 2, 3, 5, 8, 13]
+    n_b = 32
+    D, I_q, cnt, D2d, I2d = run(binding, st.astype(np.uint16), lags, n_b)
+    b0 = int(np.floor(n_b * 2 * np.sqrt((k0x / W) ** 2 + (k0y / H) ** 2)))
+    for l, tau in enumerate(lags):
+        expect = (B / (2 * A)) ** 2 * W * H * (2 - 2 * np.cos(w * tau))
+        assert D2d[l, k0y, k0x] == pytest.approx(expect, rel=2e-3)       # uint16 rounding of the fringe
+        # the conjugate mode (-k0) is the other half of the full plane: bin mean = 2 * expect / c_b
+        assert D[l, b0] == pytest.approx(2 * expect / cnt[b0], rel=5e-3)
+        others = np.delete(D[l], b0)
+        assert others.max() < 1e-4 * D[l, b0]
+
+
+def test_ramp(binding):
+    """P6: I_t = I_0 + t G with sum(G) = 0 (constant mean): D2d(k,tau) = tau^2 |F_G(k)|^2 for k != 0."""
+    rng = np.random.default_rng(11)
+    W = H = 64
+    I0 = rng.integers(20000, 30000, size=(H, W))
+    G = rng.integers(-20, 21, size=(H, W))
+    G.flat[0] -= G.sum()
+    st = np.stack([I0 + t * G for t in range(16)]).astype(np.uint16)
+    lags = [1, 2, 3, 6]
+    D, I_q, cnt, D2d, I2d = run(binding, st, lags, 16)
+    FG = np.abs(np.fft.rfft2(G / I0.mean(), norm="ortho")) ** 2
+    m = FG > 1e-6 * FG.max()
+    m[0, 0] = False
+    for l, tau in enumerate(lags):
+        assert (np.abs(D2d[l] - tau * tau * FG)[m] / (tau * tau * FG[m])).max() < 1e-4
+
+
+def test_parseval_and_dc(binding):
+    """P2: sum_k D2d(k,tau) over the full plane = < sum_x (i_t - i_{t+tau})^2 >_t ; D2d(DC) = 0 (P3)."""
+    cfg = synth.config(0)
+    st = synth.make_stack(cfg, "cpu").numpy()
+    lags = [1, 4, 8]
+    D, I_q, cnt, D2d, I2d = run(binding, st, lags, cfg.n_qbins)
+    i = st.astype(np.float64)
+    i /= i.mean(axis=(1, 2), keepdims=True)
+    n = cfg.W // 2
+    wgt = np.full(n + 1, 2.0)
+    wgt[0] = wgt[n] = 1.0
+    for l, tau in enumerate(lags):
+        real = np.mean(((i[:-tau] - i[tau:]) ** 2).sum(axis=(1, 2)))
+        four = (D2d[l] * wgt[None, :]).sum()
+        assert four == pytest.approx(real, rel=1e-5)
+        assert D2d[l, 0, 0] < 1e-9 * D2d[l].max()
+
+
+# --------------------------------------------------------------------------------------------------------------
+# full sizes, bench.py's launch configuration (default internal batch, one push of the whole stack)
+# --------------------------------------------------------------------------------------------------------------
+def _sample_pixels(W, H, n_rand, seed):
+    n = W // 2
+    rng = np.random.default_rng(seed)
+    ky = [0, 1, 0, 1, H // 2, H - 1, 3, H // 4, 0, H // 2, 7]
+    kx = [1, 0, 2, 1, 0, 1, n, n, n - 1, n, 0]
+    # low-|q| region where the signal lives, plus uniform samples of the whole half plane
+    ky += list(rng.integers(0, 24, n_rand)) + list(rng.integers(0, H, n_rand))
+    kx += list(rng.integers(0, 24, n_rand)) + list(rng.integers(0, n + 1, n_rand))
+    return np.array(ky, dtype=np.int32), np.array(kx, dtype=np.int32)
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+def test_full_size_sampled_pixels_and_invariants(binding, oracle, idx):
+    cfg = synth.config(idx)            # 512^2 x 1000 / 1024^2 x 2000, lags 1..100
+    st = synth.make_stack(cfg, "cuda")
+    nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins)
+    nfs.push(st)
+    D, I_q, cnt = nfs.finalize()
+    sel = [0, 1, 9, 10, 49, 98, 99]
+    D2d = {l: nfs.D2d(l) for l in sel}
+    I2d = nfs.I2d()
+    npairs = nfs.pair_counts()
+    nfs.close()
+    assert npairs.tolist() == [cfg.N - t for t in cfg.lags]
+    # exact, data-independent bin counts
+    assert cnt[:8].tolist() == [8, 36, 64, 84, 112, 132, 172, 184]
+    assert int(cnt.sum()) == {1: 205856, 2: 823468}[idx]
+    # sampled pixels against the oracle (full fp64 transform of every frame, explicit pair loop)
+    ky, kx = _sample_pixels(cfg.W, cfg.H, 24, seed=idx)
+    ref = oracle.structure_function_sampled(st.cpu().numpy(), cfg.lags, ky, kx)
+    dmax = max(D2d[l].max() for l in sel)
+    worst = 0.0
+    for l in sel:
+        g = D2d[l][ky, kx]
+        r = ref.D2d[l]
+        m = r > 1e-6 * dmax
+        assert m.sum() >= 8
+        worst = max(worst, float((np.abs(g - r)[m] / r[m]).max()))
+    assert worst < 1e-3, worst
+    gI = I2d[ky, kx]
+    assert (np.abs(gI - ref.I2d) / ref.I2d).max() < 1e-2
+    # invariants that hold at any size: conservation of the azimuthal mean, D2d(DC) = 0, symmetry of the ky axis
+    n = cfg.W // 2
+    wgt = np.full(n + 1, 2.0)
+    wgt[0] = wgt[n] = 1.0
+    kyy = np.arange(cfg.H)
+    sy = np.where(kyy < cfg.H // 2, kyy, kyy - cfg.H)[:, None].astype(np.float64)
+    sx = np.arange(n + 1)[None, :].astype(np.float64)
+    q2 = 4.0 * ((sx / cfg.W) ** 2 + (sy / cfg.H) ** 2)
+    inc = (q2 < 1.0) & ~((sx == 0) & (sy == 0))
+    for l in sel:
+        lhs = float((cnt * D[l]).sum())
+        rhs = float((D2d[l] * wgt[None, :])[inc].sum())
+        assert lhs == pytest.approx(rhs, rel=1e-9)
+        assert D2d[l][0, 0] < 1e-9 * D2d[l].max()
+        # kx = 0 column is Hermitian in ky: D2d(ky, 0) = D2d(-ky, 0)
+        col = D2d[l][:, 0]
+        assert np.abs(col[1:cfg.H // 2] - col[:cfg.H // 2:-1]).max() <= 1e-4 * col.max()

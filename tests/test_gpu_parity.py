@@ -1,0 +1,231 @@
+"""Parity of the CUDA hot path (through the C ABI) with the CPU oracle, element by element, on the same seeded
+uint16 bytes.  Tolerances are BASELINE.json north_star's:
+  binned D(q,tau), I(q): max relative error 1e-4;  per pixel D2d: 1e-3 wherever D2d > 1e-6 * max D2d;
+  q-bin counts and pair counts: exact;  GPU output run-to-run bit-identical.
+Every test here needs a B200 (-m gpu)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1209_3362_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_BINNED = 1e-4
+TOL_PIXEL = 1e-3
+TOL_SPLIT = 1e-6
+
+
+@pytest.fixture(scope="module")
+def binding():
+    assert torch.cuda.is_available(), "GPU parity tests need a CUDA device"
+    from paper_1209_3362_b200 import binding as b
+
+    b.load_library()
+    return b
+
+
+def gpu_run(binding, stack, lags, n_b, batch=0, variant=0, split=None, want_2d=True):
+    N, H, W = stack.shape
+    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch)
+    nfs.set_lag_kernel(variant)
+    if split:
+        i = 0
+        while i < N:
+            nfs.push(stack[i:i + split].contiguous())
+            i += split
+    else:
+        nfs.push(stack)
+    D, I_q, cnt = nfs.finalize()
+    out = dict(D=D, I_q=I_q, counts=cnt, n_pairs=nfs.pair_counts(), launches=nfs.num_launches, N=nfs.num_frames)
+    if want_2d:
+        out["D2d"] = np.stack([nfs.D2d(l) for l in range(len(lags))])
+        out["I2d"] = nfs.I2d()
+    nfs.close()
+    return out
+
+
+def relerr(a, b):
+    return np.abs(a - b) / np.maximum(np.abs(b), 1e-300)
+
+
+def check_against_oracle(g, r, W, per_pixel=True):
+    n = W // 2
+    assert np.array_equal(g["counts"], r.counts), "q-bin counts must match exactly"
+    assert np.array_equal(g["n_pairs"], r.n_pairs), "pair counts must match exactly"
+    nz = r.counts > 0
+    rows = r.n_pairs > 0
+    assert np.all(g["D"][:, ~nz] == 0.0) and np.all(g["I_q"][~nz] == 0.0), "empty bins hold 0.0"
+    assert np.all(g["D"][~rows] == 0.0), "lags >= N give a row of zeros"
+    if rows.any() and nz.any():
+        eD = relerr(g["D"][rows][:, nz], r.D[rows][:, nz]).max()
+        assert eD < TOL_BINNED, "binned D rel err %.3e" % eD
+    eI = relerr(g["I_q"][nz], r.I_q[nz]).max()
+    assert eI < TOL_BINNED, "binned I rel err %.3e" % eI
+    if per_pixel and r.D2d is not None:
+        ref = r.D2d[:, :, :n + 1]
+        thr = 1e-6 * ref.max()
+        m = ref > thr
+        if m.any():
+            eP = relerr(g["D2d"][m], ref[m]).max()
+            assert eP < TOL_PIXEL, "per-pixel D2d rel err %.3e" % eP
+        # below the threshold only an absolute bound is meaningful
+        assert np.abs(g["D2d"][~m] - ref[~m]).max(initial=0.0) <= TOL_PIXEL * thr + 1e-30
+        refI = r.I2d[:, :n + 1]
+        mI = refI > 1e-6 * refI.max()
+        assert relerr(g["I2d"][mI], refI[mI]).max() < TOL_PIXEL
+        # everywhere: I2d within 1 % (fp32 transform of the static reference frame bounds it)
+        assert relerr(g["I2d"], refI).max() < 1e-2
+
+
+# --------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs[0] in full, every launch shape
+# --------------------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def cfg0():
+    cfg = synth.config(0)
+    st = synth.make_stack(cfg, "cuda")
+    from oracle import nfs_oracle as o
+
+    ref = o.structure_function(st.cpu().numpy(), cfg.lags, cfg.n_qbins, want_2d=True)
+    return cfg, st, ref
+
+
+@pytest.mark.parametrize("variant,batch,split", [(0, 0, None), (1, 0, None), (0, 5, None), (0, 0, 3), (0, 7, 5),
+                                                  (1, 0, 1), (0, 0, 1), (0, 32, None), (0, 1, None)])
+def test_config0_full(binding, cfg0, variant, batch, split):
+    cfg, st, ref = cfg0
+    g = gpu_run(binding, st, cfg.lags, cfg.n_qbins, batch=batch, variant=variant, split=split)
+    assert g["N"] == cfg.N and g["launches"] > 0
+    assert g["counts"][0] == 0, "config 0 has an empty first bin (reading R7)"
+    check_against_oracle(g, ref, cfg.W)
+
+
+def test_config0_golden_counts(binding, cfg0):
+    cfg, st, ref = cfg0
+    g = gpu_run(binding, st, cfg.lags, cfg.n_qbins, want_2d=False)
+    assert g["counts"][:8].tolist() == [0, 8, 16, 20, 24, 40, 36, 48]
+    assert int(g["counts"].sum()) == 3204
+
+
+# --------------------------------------------------------------------------------------------------------------
+# scaled-down versions of configs 1-4: several tiles, ragged tails, dense and sparse lags, every frame size
+# --------------------------------------------------------------------------------------------------------------
+SCALED = [
+    # idx, W,   N,   lags,                                                  n_b, batch, per_pixel
+    (1, 32, 60, list(range(1, 31)), 8, 0, True),                           # smallest supported frame
+    (1, 128, 77, list(range(1, 31)), 32, 16, True),                        # ragged: 77 = 4*16 + 13
+    (1, 256, 60, list(range(1, 31)), 64, 0, True),
+    (1, 512, 300, list(range(1, 101)), 128, 0, True),                      # config 1 shape, 100 dense lags
+    (1, 512, 130, list(range(1, 101)), 128, 48, False),                    # warm-up spans several batches
+    (2, 1024, 64, list(range(1, 41)), 256, 0, True),                       # Poisson, 14 bit
+    (3, 256, 120, [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 14, 17, 21, 26, 33, 41, 52, 65, 80, 99, 110], 64, 0, True),
+    (3, 256, 120, [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 14, 17, 21, 26, 33, 41, 52, 65, 80, 99, 110], 64, 32, True),
+    (3, 128, 90, [2, 3, 7, 8, 9, 40, 41, 43, 70], 32, 20, True),           # short runs, isolated lags
+    (3, 2048, 12, [1, 2, 3, 5, 8], 512, 0, False),                         # config 3 frame size
+    (3, 4096, 4, [1, 2], 512, 0, False),                                   # largest supported frame
+    (4, 128, 400, list(range(1, 201)), 32, 64, False),                     # config 4 shape: long dense window
+]
+
+
+@pytest.mark.parametrize("idx,W,N,lags,n_b,batch,per_pixel", SCALED)
+def test_scaled_configs(binding, oracle, idx, W, N, lags, n_b, batch, per_pixel):
+    cfg = synth.config(idx, W=W, N=N, lags=lags, n_qbins=n_b)
+    st = synth.make_stack(cfg, "cuda")
+    ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=per_pixel)
+    for variant in ((0, 1) if W <= 512 else (0,)):
+        g = gpu_run(binding, st, lags, n_b, batch=batch, variant=variant, want_2d=per_pixel)
+        check_against_oracle(g, ref, W, per_pixel=per_pixel)
+
+
+# --------------------------------------------------------------------------------------------------------------
+# edge cases
+# --------------------------------------------------------------------------------------------------------------
+def test_lags_beyond_N_and_single_frame(binding, oracle):
+    cfg = synth.config(0)
+    st = synth.make_stack(cfg, "cuda", n=6)
+    lags = [1, 2, 5, 6, 9, 100]
+    ref = oracle.structure_function(st.cpu().numpy(), lags, 16, want_2d=True)
+    g = gpu_run(binding, st, lags, 16)
+    assert g["n_pairs"].tolist() == [5, 4, 1, 0, 0, 0]
+    check_against_oracle(g, ref, cfg.W)
+    assert np.all(g["D2d"][3:] == 0.0)
+    # N = 1: no pairs at all, I(q) still defined
+    ref1 = oracle.structure_function(st[:1].cpu().numpy(), [1, 2], 16, want_2d=True)
+    g1 = gpu_run(binding, st[:1].contiguous(), [1, 2], 16)
+    assert g1["n_pairs"].tolist() == [0, 0] and np.all(g1["D"] == 0.0)
+    check_against_oracle(g1, ref1, cfg.W)
+
+
+def test_push_split_invariance_and_bit_reproducibility(binding):
+    cfg = synth.config(1, W=128, N=150, lags=list(range(1, 41)), n_qbins=32)
+    st = synth.make_stack(cfg, "cuda")
+    a = gpu_run(binding, st, cfg.lags, cfg.n_qbins)
+    b = gpu_run(binding, st, cfg.lags, cfg.n_qbins)
+    for k in ("D", "I_q", "D2d", "I2d"):
+        assert np.array_equal(a[k], b[k]), "%s is not run-to-run bit-identical" % k
+    for split in (1, 7, 64):
+        c = gpu_run(binding, st, cfg.lags, cfg.n_qbins, split=split)
+        nz = a["counts"] > 0
+        assert relerr(c["D"][:, nz], a["D"][:, nz]).max() < TOL_SPLIT
+        assert relerr(c["I_q"][nz], a["I_q"][nz]).max() < TOL_SPLIT
+
+
+def test_finalize_is_a_snapshot_and_reset_forgets(binding, oracle):
+    cfg = synth.config(0)
+    st = synth.make_stack(cfg, "cuda")
+    nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins)
+    nfs.push(st[:10].contiguous())
+    D10, I10, _ = nfs.finalize()
+    D10b, _, _ = nfs.finalize()
+    assert np.array_equal(D10, D10b)
+    nfs.push(st[10:].contiguous())
+    D, I_q, cnt = nfs.finalize()
+    ref = oracle.structure_function(st.cpu().numpy(), cfg.lags, cfg.n_qbins)
+    ref10 = oracle.structure_function(st[:10].cpu().numpy(), cfg.lags, cfg.n_qbins)
+    nz = ref.counts > 0
+    assert relerr(D[:, nz], ref.D[:, nz]).max() < TOL_BINNED
+    assert relerr(D10[:, nz], ref10.D[:, nz]).max() < TOL_BINNED
+    nfs.reset()
+    assert nfs.num_frames == 0
+    nfs.push(st)
+    D2, _, _ = nfs.finalize()
+    assert np.array_equal(D2, gpu_run(binding, st, cfg.lags, cfg.n_qbins, want_2d=False)["D"])
+    nfs.close()
+
+
+def test_state_and_argument_errors(binding):
+    nfs = binding.NFS(64, 64, [1, 2], 8)
+    with pytest.raises(binding.NFSError) as e:
+        nfs.finalize()                       # nothing pushed yet
+    assert e.value.status == binding.NFS_ERR_STATE
+    buf = torch.zeros((2, 64, 64), dtype=torch.uint16, device="cuda")
+    with pytest.raises(binding.NFSError) as e:
+        binding.nfs_push_frames(nfs.handle, buf.data_ptr(), 0)
+    assert e.value.status == binding.NFS_ERR_INVALID_ARG
+    with pytest.raises(binding.NFSError) as e:
+        binding.nfs_push_frames(nfs.handle, buf.data_ptr() + 2, 1)   # 16-byte alignment is part of the contract
+    assert e.value.status == binding.NFS_ERR_INVALID_ARG
+    nfs.close()
+
+
+def test_zero_mean_frame_is_sticky_until_reset(binding):
+    st = synth.make_stack(synth.config(0), "cuda", n=4)
+    st[2] = 0
+    nfs = binding.NFS(64, 64, [1, 2], 8)
+    nfs.push(st)
+    with pytest.raises(binding.NFSError) as e:
+        nfs.finalize()
+    assert e.value.status == binding.NFS_ERR_ZERO_MEAN
+    with pytest.raises(binding.NFSError):
+        nfs.push(st)
+    nfs.reset()
+    nfs.push(st[:2].contiguous())
+    nfs.finalize()
+    nfs.close()
+
+
+def test_oom_is_reported_at_create(binding):
+    with pytest.raises(binding.NFSError) as e:
+        binding.NFS(4096, 4096, list(range(1, 4001)), 16)   # 4000 x 67 MB ring + 4000 x 67 MB totals > 180 GB
+    assert e.value.status == binding.NFS_ERR_OOM
