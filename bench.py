@@ -235,7 +235,7 @@ def run_ours(args, cfg):
     B = args.batch or 256
     nb = (cfg.N + B - 1) // B
     lag_bytes = P * (8.0 * (cfg.N + nb * (cfg.lags[-1])) * (1 + 0) + 16.0 * len(cfg.lags) * nb)
-    fft_ms = ktimes["frame_sum"][0] + ktimes["fft_row"][0] + ktimes["fft_col"][0]
+    fft_ms = ktimes["fft"][0]
     fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N
     roofline = dict(bound="alu", kernel="k_lag_tiled", achieved=ach_tflops, peak=peak_tflops, unit="TFLOP/s",
                     frac=ach_tflops / peak_tflops, traffic=None,

@@ -105,9 +105,10 @@ NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
 /* Per-kernel timing for bench.py: when enabled, every kernel launch is bracketed by a CUDA event pair
  * on the context's stream.  nfs_get_kernel_times synchronises, returns the accumulated milliseconds
  * and launch counts per class since the last call — ms/launches are HOST [NFS_NUM_KERNEL_CLASSES], in
- * the order: 0 frame sums (+reference), 1 FFT row pass, 2 FFT column pass, 3 I accumulation,
- * 4 lag accumulation, 5 binning — and clears them. */
-#define NFS_NUM_KERNEL_CLASSES 6
+ * the order: 0 reference set-up at the first frame (sum, reference image), 1 FFT (one persistent
+ * kernel per batch: frame sums, row pass, column pass), 2 I accumulation, 3 lag accumulation,
+ * 4 binning — and clears them. */
+#define NFS_NUM_KERNEL_CLASSES 5
 NFS_API int nfs_set_profiling(nfs_ctx* ctx, int enable);
 NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
 

@@ -43,7 +43,7 @@ SYMBOLS = [
     ("nfs_last_cuda_error", C.c_char_p, [_P]),
 ]
 
-KERNEL_CLASSES = ["frame_sum", "fft_row", "fft_col", "accum_I", "lag_accum", "bin"]
+KERNEL_CLASSES = ["ref_setup", "fft", "accum_I", "lag_accum", "bin"]
 
 _lib = None
 

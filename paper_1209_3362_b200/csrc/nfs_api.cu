@@ -67,27 +67,46 @@ int qbin_of(int kx, int ky, int W, int H, int nb) {
 // host tables: twiddles, bin map, lag plan
 bool build_tables(Ctx& c) {
   const int W = c.W, H = c.H, n = c.n, nb = c.n_qbins;
-  // twiddles exp(-2 pi i k / W), evaluated in fp64, rounded once
-  std::vector<float2> tw(W);
-  for (int k = 0; k < W; ++k) {
-    const double ph = -2.0 * M_PI * (double)k / (double)W;
-    tw[k] = make_float2((float)cos(ph), (float)sin(ph));
+  // twiddle tables of the FFT plan (nfs_fft.cu), evaluated in fp64 and rounded once.
+  // L = W = H.  L <= 1024: one level, Li = L, Mi = L/32 lanes.  L > 1024: outer radix-32 pass over
+  // T = L/32 threads, then inner FFTs of length Li = L/32 with Mi = Li/32 lanes.
+  {
+    const int L = W;
+    const bool two = L > 1024;
+    const int Li = two ? L / 32 : L, Mi = Li / 32;
+    auto tw_of = [](int64_t num, int64_t den) {
+      num %= den;
+      // exact values on the axes and diagonals, fp64 elsewhere
+      if (num == 0) return make_float2(1.f, 0.f);
+      if (4 * num == den) return make_float2(0.f, -1.f);
+      if (2 * num == den) return make_float2(-1.f, 0.f);
+      if (4 * num == 3 * den) return make_float2(0.f, 1.f);
+      const double ph = -2.0 * M_PI * (double)num / (double)den;
+      return make_float2((float)cos(ph), (float)sin(ph));
+    };
+    std::vector<float2> tin((size_t)std::max(Li, 32));
+    for (int j2 = 0; j2 < std::max(Mi, 1); ++j2)
+      for (int k1 = 0; k1 < 32; ++k1) tin[(size_t)j2 * 32 + k1] = tw_of((int64_t)j2 * k1, Li);
+    if (!dev_alloc(c, &c.tw, tin.size())) return false;
+    if (!NFS_CUDA(c, cudaMemcpy(c.tw, tin.data(), sizeof(float2) * tin.size(), cudaMemcpyHostToDevice))) return false;
+    if (two) {
+      const int T = L / 32;
+      std::vector<float2> tout((size_t)L);
+      for (int k1 = 0; k1 < 32; ++k1)
+        for (int j2 = 0; j2 < T; ++j2) tout[(size_t)k1 * T + j2] = tw_of((int64_t)j2 * k1, L);
+      if (!dev_alloc(c, &c.tw_out, tout.size())) return false;
+      if (!NFS_CUDA(c, cudaMemcpy(c.tw_out, tout.data(), sizeof(float2) * tout.size(), cudaMemcpyHostToDevice)))
+        return false;
+    }
   }
-  // exact symmetric points
-  tw[0] = make_float2(1.f, 0.f);
-  tw[W / 4] = make_float2(0.f, -1.f);
-  tw[W / 2] = make_float2(-1.f, 0.f);
-  tw[3 * W / 4] = make_float2(0.f, 1.f);
-  if (!dev_alloc(c, &c.tw, (size_t)W)) return false;
-  if (!NFS_CUDA(c, cudaMemcpy(c.tw, tw.data(), sizeof(float2) * W, cudaMemcpyHostToDevice))) return false;
 
-  // bin map in ring layout: p = ky*n + kx (kx < n), p = H*n + ky (kx = n)
+  // bin map in ring layout: p = kx*H + ky
   std::vector<int32_t> start(nb + 1, 0);
   c.counts.assign(nb, 0);
   std::vector<int32_t> binof((size_t)c.P);
   for (int ky = 0; ky < H; ++ky)
     for (int kx = 0; kx <= n; ++kx) {
-      const int64_t p = kx < n ? (int64_t)ky * n + kx : (int64_t)H * n + ky;
+      const int64_t p = (int64_t)kx * H + ky;
       const int b = qbin_of(kx, ky, W, H, nb);
       binof[p] = b;
       if (b >= 0) {
@@ -102,7 +121,7 @@ bool build_tables(Ctx& c) {
     for (int64_t p = 0; p < c.P; ++p) {  // ascending p inside each bin: fixed order, good locality
       const int b = binof[p];
       if (b < 0) continue;
-      const bool interior = p < (int64_t)H * n && (p % n) != 0;
+      const bool interior = p >= (int64_t)H && p < (int64_t)H * n;  // 0 < kx < n: Hermitian weight 2
       perm[fill[b]++] = (uint32_t)p | (interior ? 0x80000000u : 0u);
     }
   }
@@ -185,8 +204,8 @@ bool build_tables(Ctx& c) {
 }
 
 void free_all(Ctx& c) {
-  void* ptrs[] = {c.ring, c.rowbuf, c.ref,  c.Fref,      c.totals, c.I2,    c.I1,      c.sums,    c.tw,
-                  c.d_lags, c.perm, c.bin_start, c.d_out,  c.d_tmp, c.d_flags, c.d_tasks, c.d_groups};
+  void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.I2,      c.I1,      c.sums,     c.tw,     c.tw_out,
+                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags, c.d_tasks, c.d_groups, c.fft_cnt};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
@@ -215,13 +234,11 @@ int sync_and_check(Ctx& c) {
   return c.status;
 }
 
-// ring-layout double[P] -> [H][W/2+1]
+// ring-layout double[P] ([kx][ky]) -> [H][W/2+1]
 void ring_to_plane(const Ctx& c, const double* src, double* out) {
   const int n = c.n, H = c.H;
-  for (int y = 0; y < H; ++y) {
-    memcpy(out + (size_t)y * (n + 1), src + (size_t)y * n, sizeof(double) * n);
-    out[(size_t)y * (n + 1) + n] = src[(size_t)H * n + y];
-  }
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x <= n; ++x) out[(size_t)y * (n + 1) + x] = src[(size_t)x * H + y];
 }
 
 }  // namespace
@@ -253,11 +270,6 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   c.Lmax = lags[n_lags - 1];
   c.B = batch_frames > 0 ? batch_frames : 256;
   c.R = c.Lmax + c.B;
-  {
-    int64_t bf = (32ll << 20) / (c.P * (int64_t)sizeof(float2));
-    c.Bf = (int)std::max<int64_t>(1, std::min<int64_t>(64, bf));
-    c.Bf = std::min(c.Bf, c.B);
-  }
 
   int dev = 0;
   if (!NFS_CUDA(c, cudaGetDevice(&dev))) goto fail;
@@ -272,7 +284,8 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
     // memory plan: everything is sized before the first frame arrives
     size_t free_b = 0, total_b = 0;
     if (!NFS_CUDA(c, cudaMemGetInfo(&free_b, &total_b))) goto fail;
-    const double need = (double)c.P * ((double)c.R * 8 + (double)c.Bf * 8 + 8 + (double)c.n_lags * 8 + 8 + 16 + 8) +
+    const double need = (double)c.P * ((double)c.R * 8 + 8 + (double)c.n_lags * 8 + 8 + 16 + 8) +
+                        (double)fft_rowT_elems(c) * 8 +
                         (double)W * H * 4 + (double)(n_lags + 1) * n_qbins * 8 + (64 << 20);
     if (need > (double)free_b) {
       free_all(c);
@@ -281,13 +294,14 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
     }
   }
   if (!dev_alloc(c, &c.ring, (size_t)c.R * c.P)) goto fail;
-  if (!dev_alloc(c, &c.rowbuf, (size_t)c.Bf * c.P)) goto fail;
+  if (!dev_alloc(c, &c.rowbuf, fft_rowT_elems(c))) goto fail;
   if (!dev_alloc(c, &c.ref, (size_t)W * H)) goto fail;
   if (!dev_alloc(c, &c.Fref, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.totals, (size_t)c.n_lags * c.P)) goto fail;
   if (!dev_alloc(c, &c.I2, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.I1, (size_t)c.P)) goto fail;
-  if (!dev_alloc(c, &c.sums, (size_t)c.Bf + 1)) goto fail;
+  if (!dev_alloc(c, &c.sums, (size_t)c.B + 1)) goto fail;
+  if (!dev_alloc(c, &c.fft_cnt, 1 + 3 * (size_t)c.B)) goto fail;
   if (!dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 1) * c.n_qbins)) goto fail;
   if (!dev_alloc(c, &c.d_tmp, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.d_flags, 1)) goto fail;
@@ -326,17 +340,10 @@ int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) {
   while (done < n) {
     const int b = std::min(c.B, n - done);
     const int64_t t0 = c.n_frames;
-    for (int f0 = 0; f0 < b; f0 += c.Bf) {
-      const int nf = std::min(c.Bf, b - f0);
-      const uint16_t* fr = d_frames + (int64_t)(done + f0) * fpx;
-      c.n_launches += launch_frame_sums(c, fr, nf);
-      if (t0 + f0 == 0) {
-        c.n_launches += launch_make_ref(c, fr);
-        c.n_launches += launch_fft_ref(c);
-      }
-      c.n_launches += launch_fft_frames(c, fr, nf, t0 + f0);
-      if (!check_launch(c, "fft launch")) return c.status;
-    }
+    const uint16_t* fr = d_frames + (int64_t)done * fpx;
+    if (t0 == 0) c.n_launches += launch_make_ref(c, fr);
+    c.n_launches += launch_fft_frames(c, fr, b, t0);
+    if (!check_launch(c, "fft launch")) return c.status;
     c.n_launches += launch_accum_I(c, t0, b);
     c.n_launches += (c.lag_variant == 1) ? launch_lag_simple(c, t0, b) : launch_lag_tiled(c, t0, b);
     if (!check_launch(c, "lag launch")) return c.status;

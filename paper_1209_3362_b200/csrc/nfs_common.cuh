@@ -1,9 +1,9 @@
 // nfs_common.cuh — shared declarations of the CUDA hot path (product code; shares nothing with oracle/).
 //
-// Data layout in HBM.  n = W/2, P = H*(n+1) Fourier pixels per frame (half plane):
-//   Fourier frame  float2[P]  = main block [H][n]  (kx = 0..n-1, 16-byte aligned rows)
-//                               followed by the Nyquist column [H]  (kx = n), so that every row of
-//                               the main block is 16-byte aligned.
+// Data layout in HBM.  n = W/2, P = (n+1)*H Fourier pixels per frame (half plane):
+//   Fourier frame  float2[P]  = [kx = 0..n][ky = 0..H-1]  (transposed: ky fastest, FFT order), so that
+//                               the column pass writes contiguous 8*H-byte rows and every row is
+//                               16-byte aligned, Nyquist column included.
 //   ring           float2[R][P], slot(t) = t mod R, R = Lmax + batch   (PAPER.md:L33 FIFO of image FFTs)
 //   totals         double[n_lags][P]   sum over pairs of |F'_t - F'_{t+tau}|^2   ("differences area", L33)
 //   ref            float[H][W]   first normalised frame r; F'_t = FFT(i_t - r)   (linearity, L31)
@@ -37,7 +37,7 @@ struct LagGroup {
 };
 
 // kernel classes for the optional per-kernel CUDA-event timing (nfs_set_profiling)
-enum KernelClass { kKSum = 0, kKRow = 1, kKCol = 2, kKAccI = 3, kKLag = 4, kKBin = 5, kNumKernelClasses = 6 };
+enum KernelClass { kKSum = 0, kKFft = 1, kKAccI = 2, kKLag = 3, kKBin = 4, kNumKernelClasses = 5 };
 
 struct Ctx {
   int W = 0, H = 0, n = 0;  // n = W/2
@@ -45,7 +45,6 @@ struct Ctx {
   int n_lags = 0, n_qbins = 0, Lmax = 0;
   int B = 0;   // internal batch (frames)
   int R = 0;   // ring slots
-  int Bf = 0;  // frames per FFT sub-batch
   std::vector<int32_t> lags;
   std::vector<int64_t> counts;  // full-plane pixel count per bin
   cudaStream_t stream = nullptr;
@@ -60,14 +59,17 @@ struct Ctx {
 
   // device memory
   float2* ring = nullptr;
-  float2* rowbuf = nullptr;      // [Bf][P] output of the row pass
+  float2* rowbuf = nullptr;      // [slots][P] output of the row pass (transposed, L2 resident)
   float* ref = nullptr;          // [H][W]
   float2* Fref = nullptr;        // [P] unitary FFT of ref
   double* totals = nullptr;      // [n_lags][P]
   double* I2 = nullptr;          // [P]  sum_t |F'_t|^2
   double2* I1 = nullptr;         // [P]  sum_t F'_t
-  unsigned long long* sums = nullptr;  // [Bf + 1] exact pixel sums of the frames of a sub-batch
-  float2* tw = nullptr;          // [W] exp(-2 pi i k / W)   (W == H)
+  unsigned long long* sums = nullptr;  // [B] exact pixel sums of the frames of a batch
+  unsigned int* fft_cnt = nullptr;     // [1 + 3 B] work-queue head and per-frame completion counters
+  int fft_grid = 0;                    // CTAs of the persistent FFT kernel (set at the first launch)
+  float2* tw = nullptr;          // inner twiddle table (nfs_fft.cu)
+  float2* tw_out = nullptr;      // outer twiddle table, W > 1024 only
   int32_t* d_lags = nullptr;     // [n_lags]
   uint32_t* perm = nullptr;      // [n_binned] pixel index | (weight-2 flag << 31), grouped by bin
   int32_t* bin_start = nullptr;  // [n_qbins + 1]
@@ -84,8 +86,8 @@ struct Ctx {
   std::vector<cudaEvent_t> ev_pool;
   size_t ev_used = 0;
   std::vector<int> ev_class;  // class of pair i (events 2i, 2i+1)
-  double prof_ms[kNumKernelClasses] = {0, 0, 0, 0, 0, 0};
-  int64_t prof_n[kNumKernelClasses] = {0, 0, 0, 0, 0, 0};
+  double prof_ms[kNumKernelClasses] = {0, 0, 0, 0, 0};
+  int64_t prof_n[kNumKernelClasses] = {0, 0, 0, 0, 0};
 };
 
 // RAII: records an event pair around the launches enqueued in its scope when profiling is on
@@ -112,10 +114,9 @@ struct ProfScope {
 
 // ---- kernel launchers (each returns the number of kernel launches it enqueued; sets cudaGetLastError) ----
 // nfs_fft.cu
-int launch_frame_sums(Ctx& c, const uint16_t* frames, int nf);
-int launch_make_ref(Ctx& c, const uint16_t* frame0);
-int launch_fft_ref(Ctx& c);                                       // Fref = FFT(ref)
+int launch_make_ref(Ctx& c, const uint16_t* frame0);              // S_0, ref = i_0, Fref = FFT(ref)
 int launch_fft_frames(Ctx& c, const uint16_t* frames, int nf, int64_t t_first);  // ring[t_first..] = FFT(i_t - ref)
+size_t fft_rowT_elems(const Ctx& c);                              // float2 elements of the row-pass buffer
 // nfs_lag.cu
 int launch_accum_I(Ctx& c, int64_t t0, int b);
 int launch_lag_simple(Ctx& c, int64_t t0, int b);
