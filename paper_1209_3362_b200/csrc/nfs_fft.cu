@@ -9,7 +9,7 @@
 //
 // One persistent kernel per push batch (k_fft<L>, L = W = H).  Its CTAs pull work items from a global
 // queue in a fixed order that software-pipelines the three stages through L2:
-//      step s:  [sum items of frame s] [row items of frame s-1] [column items of frame s-1-kDc]
+//      step s:  [sum items of frame s] [row items of frame s-Dr] [column items of frame s-Dr-Dc]
 // An item waits (acquire-spin on a per-frame counter) only for items that precede it in the queue, so
 // every claimed item is held by a running CTA and the smallest unfinished item can always finish: no
 // deadlock, no co-residency requirement.  The row pass writes its result transposed ([kx][y]) into a
@@ -112,9 +112,12 @@ __device__ __forceinline__ void dft(float2* u) {
 // ------------------------------------------------------------------------------------------------
 // plan constants for FFT length L
 // ------------------------------------------------------------------------------------------------
-constexpr int kDr = 1;   // row items of frame f are queued kDr steps after its sum items
-constexpr int kDc = 4;   // column items of frame f are queued kDc steps after its row items
-constexpr int kSlots = 8;  // intermediate frames kept (all of them L2 resident)
+#ifndef NFS_FFT_DR
+#define NFS_FFT_DR 0
+#define NFS_FFT_DC 0
+#define NFS_FFT_SLOTS 0
+#endif
+constexpr int kMaxSlots = 40;
 
 template <int L>
 struct Plan {
@@ -135,12 +138,23 @@ struct Plan {
   static constexpr int NS = L >= 256 ? 8 : 1;            // sum items per frame
   static constexpr int perStep = NS + NR + NC;
   static constexpr size_t smem = sizeof(float2) * ((size_t)Fc * Sf + 2 * Fc);
+  // Queue distances, in steps (one step = the items of one frame).  About 2 * (resident CTAs) items are
+  // claimed at any time (each CTA holds the item it runs and the next one), i.e. `win` steps; an item
+  // should find its dependencies finished, so they are queued more than `win` steps earlier.
+  // The write-after-read dependency on an intermediate slot needs Dc < slots (it must precede in the queue).
+  static constexpr int claimed = (L <= 1024 ? 4 : 2) * 148;
+  static constexpr int win_ = (claimed + perStep - 1) / perStep;
+  static constexpr int win = win_ < 16 ? win_ : 16;
+  static constexpr int Dr = NFS_FFT_DR ? NFS_FFT_DR : win + 1;                   // sum items -> row items
+  static constexpr int Dc = NFS_FFT_DC ? NFS_FFT_DC : (L <= 1024 ? win + 1 : win);  // row items -> column items
+  static constexpr int slots = NFS_FFT_SLOTS ? NFS_FFT_SLOTS : Dc + win + (L <= 1024 ? 1 : 0);  // intermediate frames
+  static_assert(Dc < slots && slots <= kMaxSlots, "queue order must cover the slot reuse dependency");
 };
 
 struct FftJob {
   const uint16_t* frames;     // [nf][H][W]  (mode 0)
   const float* ref;           // [H][W] fp32 reference r
-  float2* rowT;               // [kSlots][(n+1)*H] row-pass output, transposed
+  float2* rowT;               // [slots][(n+1)*H] row-pass output, transposed
   float2* dst;                // ring base (mode 0) or Fref (mode 1)
   unsigned long long* sums;   // [nf] exact frame sums
   unsigned int* cnt;          // [1 + 3 nf]: queue head, sum_done[nf], row_done[nf], col_done[nf]
@@ -227,21 +241,26 @@ __device__ __forceinline__ int out_index(int tau, int r) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// queue helpers
+// queue helpers.  Completion counters only ever grow, so a value read early (prefetched while the
+// previous item was running) that already satisfies the target stays valid.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+__device__ __forceinline__ unsigned ld_relaxed(const unsigned* p) {
   unsigned v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-// all threads call; returns when *p >= target (thread 0 spins)
-__device__ __forceinline__ void wait_count(const unsigned* p, unsigned target) {
-  if (threadIdx.x == 0) {
-    while (ld_acquire(p) < target) __nanosleep(64);
+// thread 0 only: spin until *p >= target, starting from the prefetched value `seen`
+__device__ __forceinline__ void spin_until(const unsigned* p, unsigned target, unsigned seen) {
+  while (seen < target) {
+    __nanosleep(32);
+    seen = ld_relaxed(p);
   }
-  __syncthreads();
 }
-// all threads call after their global writes
+// acquire side: orders this thread's later loads after the counter loads above; the CTA barrier that
+// follows extends that order to the other threads.  Data produced by other CTAs is then read with
+// __ldcg (L2), never through a possibly stale L1 line.
+__device__ __forceinline__ void acquire_fence() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+// all threads call after their global writes (release side)
 __device__ __forceinline__ void signal_count(unsigned* p) {
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -276,13 +295,60 @@ __device__ __forceinline__ int stage_slot(int j) {
   return ((a ^ ((a >> 3) & 3)) << 1) | (j & 1);
 }
 
+// a decoded work item and its dependencies (all on items that precede it in the queue)
+struct Item {
+  int type;  // 0 sum, 1 row, 2 column, 3 nothing to do
+  int f;     // frame within the batch
+  int blk;   // part / row block / column block
+};
+template <int L>
+__device__ __forceinline__ Item decode_item(unsigned item, int nf) {
+  using P = Plan<L>;
+  Item it;
+  const int s = (int)(item / P::perStep), r = (int)(item % P::perStep);
+  if (r < P::NS) {
+    it.type = 0, it.f = s, it.blk = r;
+  } else if (r < P::NS + P::NR) {
+    it.type = 1, it.f = s - P::Dr, it.blk = r - P::NS;
+  } else {
+    it.type = 2, it.f = s - P::Dr - P::Dc, it.blk = r - P::NS - P::NR;
+  }
+  if (it.f < 0 || it.f >= nf) it.type = 3;
+  return it;
+}
+// first dependency: row <- sum_done[f] == NS; column <- row_done[f] == NR
+template <int L>
+__device__ __forceinline__ const unsigned* dep_a(const FftJob& j, const Item& it, unsigned& target) {
+  using P = Plan<L>;
+  if (it.type == 1) {
+    target = (unsigned)P::NS;
+    return &j.cnt[1 + it.f];
+  }
+  if (it.type == 2) {
+    target = (unsigned)P::NR;
+    return &j.cnt[1 + j.nf + it.f];
+  }
+  target = 0;
+  return nullptr;
+}
+// second dependency (write-after-read on the intermediate slot): row(f) <- col_done[f - slots] == NC
+template <int L>
+__device__ __forceinline__ const unsigned* dep_b(const FftJob& j, const Item& it, unsigned& target) {
+  using P = Plan<L>;
+  if (it.type == 1 && it.f >= P::slots) {
+    target = (unsigned)P::NC;
+    return &j.cnt[1 + 2 * j.nf + (it.f - P::slots)];
+  }
+  target = 0;
+  return nullptr;
+}
+
 // ------------------------------------------------------------------------------------------------
 // items
 // ------------------------------------------------------------------------------------------------
 template <int L>
-__device__ __forceinline__ void item_sum(const FftJob& j, int f, int part) {
+__device__ __forceinline__ void item_sum(const FftJob& j, int f, int part, unsigned long long* s_part) {
   using P = Plan<L>;
-  __shared__ unsigned long long s_part[P::NT / 32];
   if (j.mode == 0) {
     const int64_t n16 = (int64_t)L * L / 8;  // uint4 per frame
     const int64_t per = n16 / P::NS;
@@ -314,131 +380,41 @@ __device__ __forceinline__ void item_sum(const FftJob& j, int f, int part) {
   signal_count(&j.cnt[1 + f]);
 }
 
-template <int L>
-__device__ __forceinline__ void item_row(const FftJob& j, int f, int blk, float2* sm) {
-  using P = Plan<L>;
-  constexpr int W = L, H = L, n = P::n;
-  const int tid = threadIdx.x;
-  const int team = tid / P::T, tau = tid % P::T;
-  float2* nyq = sm + (size_t)P::Fc * P::Sf;  // [2 Fc]
-  float2* buf = sm + (size_t)team * P::Sf;
-  const unsigned nf = (unsigned)j.nf;
-
-  // dependencies: this frame's sum; the column pass of the frame that used this slot before
-  wait_count(&j.cnt[1 + f], (unsigned)P::NS);
-  if (f >= kSlots) wait_count(&j.cnt[1 + 2 * nf + (f - kSlots)], (unsigned)P::NC);
-
-  float hi = 0.f, lo = 0.f;
-  if (j.mode == 0) frame_scale(__ldcg(&j.sums[f]), (float)W * (float)H, hi, lo, j.flags);
-
-  int q = blk * P::Fc + team;         // complex FFT index: image rows 2q, 2q+1
-  const bool valid = q < P::rowFfts;
-  if (!valid) q = P::rowFfts - 1;
-  const int64_t ra = (int64_t)(2 * q) * W, rb = ra + W;
-  const uint16_t* fr = j.frames + (int64_t)f * W * H;
-
-  // load + convert + normalise + subtract reference; stage z[j] = d_a[j] + i d_b[j]
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    const int c = tau + P::T * r;  // chunk of 8 pixels
-    const float4 a0 = __ldg(reinterpret_cast<const float4*>(j.ref + ra + c * 8));
-    const float4 a1 = __ldg(reinterpret_cast<const float4*>(j.ref + ra + c * 8 + 4));
-    const float4 b0 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8));
-    const float4 b1 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8 + 4));
-    float da[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-    float db[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-    if (j.mode == 0) {
-      float pa[8], pb[8];
-      unpack8(__ldg(reinterpret_cast<const uint4*>(fr + ra + c * 8)), pa);
-      unpack8(__ldg(reinterpret_cast<const uint4*>(fr + rb + c * 8)), pb);
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        da[i] = fmaf(pa[i], lo, fmaf(pa[i], hi, -da[i]));  // exact product, one rounding at |d|
-        db[i] = fmaf(pb[i], lo, fmaf(pb[i], hi, -db[i]));
-      }
-    }
-#pragma unroll
-    for (int qq = 0; qq < 4; ++qq) {
-      const int a = 4 * c + qq;
-      const int as = a ^ ((a >> 3) & 3);
-      reinterpret_cast<float4*>(buf)[as] = make_float4(da[2 * qq], db[2 * qq], da[2 * qq + 1], db[2 * qq + 1]);
-    }
+// one chunk of 8 pixels of image rows a and b, and of the reference
+struct Chunk {
+  float4 a0, a1, b0, b1;
+  uint4 pa, pb;
+};
+__device__ __forceinline__ void chunk_load(Chunk& ck, const FftJob& j, const uint16_t* fr, int64_t ra, int64_t rb, int c) {
+  ck.a0 = __ldg(reinterpret_cast<const float4*>(j.ref + ra + c * 8));
+  ck.a1 = __ldg(reinterpret_cast<const float4*>(j.ref + ra + c * 8 + 4));
+  ck.b0 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8));
+  ck.b1 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8 + 4));
+  if (j.mode == 0) {
+    ck.pa = __ldg(reinterpret_cast<const uint4*>(fr + ra + c * 8));
+    ck.pb = __ldg(reinterpret_cast<const uint4*>(fr + rb + c * 8));
   }
-  team_sync<P::T>(team);
-  float2 u[32];
-#pragma unroll
-  for (int t = 0; t < 32; ++t) u[t] = buf[stage_slot(t * P::T + tau)];
-  team_sync<P::T>(team);
-  fft_team<L>(u, buf, tau, team, j);
-  team_sync<P::T>(team);
-#pragma unroll
-  for (int r = 0; r < 32; ++r) buf[out_index<L>(tau, r)] = u[r];
-  team_sync<P::T>(team);
-
-  // untangle the two real rows: A[k] = (Z[k] + conj Z[L-k]) / 2,  B[k] = (Z[k] - conj Z[L-k]) / (2i).
-  // In place: slot k <- A[k], slot L-k <- B[k] (1 <= k < n); slot 0 <- A[0], slot n <- B[0]; Nyquist aside.
-#pragma unroll
-  for (int i = 0; i < 16; ++i) {
-    const int k = tau + P::T * i;
-    if (k == 0) {
-      const float2 z0 = buf[0], zh = buf[n];
-      buf[0] = make_float2(z0.x, 0.f);
-      buf[n] = make_float2(z0.y, 0.f);
-      nyq[2 * team] = make_float2(zh.x, 0.f);
-      nyq[2 * team + 1] = make_float2(zh.y, 0.f);
-    } else {
-      const float2 zk = buf[k], zm = buf[L - k];
-      buf[k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-      buf[L - k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-    }
-  }
-  __syncthreads();
-
-  // transposed store: rowT[slot][kx][y], 16 bytes (rows 2q, 2q+1) per thread and kx
-  float2* out = j.rowT + (size_t)(f % kSlots) * ((size_t)(n + 1) * H);
-  const int y0 = blk * P::Fc * 2;
-  constexpr int FcR = P::FcRow;
-  for (int e = tid; e < n * FcR; e += P::NT) {
-    const int kxl = e & 1, ft = (e >> 1) % FcR, kx = 2 * (e / (2 * FcR)) + kxl;
-    const float2* b = sm + (size_t)ft * P::Sf;
-    const float2 A = b[kx], B = b[kx ? L - kx : n];
-    *reinterpret_cast<float4*>(out + (size_t)kx * H + y0 + 2 * ft) = make_float4(A.x, A.y, B.x, B.y);
-  }
-  if (tid < FcR) {
-    *reinterpret_cast<float4*>(out + (size_t)n * H + y0 + 2 * tid) =
-        make_float4(nyq[2 * tid].x, nyq[2 * tid].y, nyq[2 * tid + 1].x, nyq[2 * tid + 1].y);
-  }
-  signal_count(&j.cnt[1 + nf + f]);
 }
-
-template <int L>
-__device__ __forceinline__ void item_col(const FftJob& j, int f, int blk, float2* sm) {
-  using P = Plan<L>;
-  constexpr int H = L, n = P::n;
-  const int tid = threadIdx.x;
-  const int team = tid / P::T, tau = tid % P::T;
-  float2* buf = sm + (size_t)team * P::Sf;
-  const unsigned nf = (unsigned)j.nf;
-
-  wait_count(&j.cnt[1 + nf + f], (unsigned)P::NR);
-
-  int q = blk * P::Fc + team;  // kx row
-  const bool valid = q <= n;
-  if (!valid) q = n;
-  const float2* src = j.rowT + (size_t)(f % kSlots) * ((size_t)(n + 1) * H) + (size_t)q * H;
-  float2 u[32];
+// convert + normalise + subtract the reference, stage z[j] = d_a[j] + i d_b[j]
+__device__ __forceinline__ void chunk_stage(const Chunk& ck, int mode, float hi, float lo, float2* buf, int c) {
+  float da[8] = {ck.a0.x, ck.a0.y, ck.a0.z, ck.a0.w, ck.a1.x, ck.a1.y, ck.a1.z, ck.a1.w};
+  float db[8] = {ck.b0.x, ck.b0.y, ck.b0.z, ck.b0.w, ck.b1.x, ck.b1.y, ck.b1.z, ck.b1.w};
+  if (mode == 0) {
+    float pa[8], pb[8];
+    unpack8(ck.pa, pa);
+    unpack8(ck.pb, pb);
 #pragma unroll
-  for (int t = 0; t < 32; ++t) u[t] = __ldcg(&src[t * P::T + tau]);
-  fft_team<L>(u, buf, tau, team, j);
-  if (valid) {
-    const int64_t Pn = (int64_t)(n + 1) * H;
-    const int slot = (j.R > 0) ? (int)((j.t_first + f) % j.R) : 0;
-    float2* dst = j.dst + (int64_t)slot * Pn + (int64_t)q * H;
-    const float sc = j.scale;
-#pragma unroll
-    for (int r = 0; r < 32; ++r) dst[out_index<L>(tau, r)] = make_float2(u[r].x * sc, u[r].y * sc);
+    for (int i = 0; i < 8; ++i) {
+      da[i] = fmaf(pa[i], lo, fmaf(pa[i], hi, -da[i]));  // exact product, one rounding at |d|
+      db[i] = fmaf(pb[i], lo, fmaf(pb[i], hi, -db[i]));
+    }
   }
-  signal_count(&j.cnt[1 + 2 * nf + f]);
+#pragma unroll
+  for (int qq = 0; qq < 4; ++qq) {
+    const int a = 4 * c + qq;
+    const int as = a ^ ((a >> 3) & 3);
+    reinterpret_cast<float4*>(buf)[as] = make_float4(da[2 * qq], db[2 * qq], da[2 * qq + 1], db[2 * qq + 1]);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -447,37 +423,158 @@ __device__ __forceinline__ void item_col(const FftJob& j, int f, int blk, float2
 template <int L>
 __global__ void __launch_bounds__(Plan<L>::NT, (L <= 1024 ? 2 : 1)) k_fft(const FftJob j) {
   using P = Plan<L>;
+  constexpr int W = L, H = L, n = P::n;
   extern __shared__ __align__(16) float2 sm[];
-  __shared__ unsigned s_item;
-  const unsigned total = (unsigned)(j.nf + kDr + kDc) * P::perStep;
-  unsigned nxt = 0;
-  if (threadIdx.x == 0) nxt = atomicAdd(&j.cnt[0], 1u);
-  for (;;) {
-    if (threadIdx.x == 0) s_item = nxt;
-    __syncthreads();
-    const unsigned item = s_item;
+  __shared__ unsigned s_item[2];
+  __shared__ unsigned long long s_sum;
+  __shared__ unsigned long long s_part[P::NT / 32];
+  const int tid = threadIdx.x;
+  const int team = tid / P::T, tau = tid % P::T;
+  float2* buf = sm + (size_t)team * P::Sf;
+  float2* nyq = sm + (size_t)P::Fc * P::Sf;  // [2 Fc]
+  const unsigned total = (unsigned)(j.nf + P::Dr + P::Dc) * P::perStep;
+  const size_t Pn = (size_t)(n + 1) * H;
+
+  // thread 0 runs the queue two claims ahead: q1 = the next item, whose dependency counters it reads
+  // while the current item is being processed (seenA / seenB)
+  unsigned q1 = 0, seenA = 0, seenB = 0;
+  if (tid == 0) {
+    s_item[0] = atomicAdd(&j.cnt[0], 1u);
+    q1 = atomicAdd(&j.cnt[0], 1u);
+  }
+  __syncthreads();
+
+  for (int iter = 0;; ++iter) {
+    const unsigned item = s_item[iter & 1];
     if (item >= total) break;
-    if (threadIdx.x == 0) nxt = atomicAdd(&j.cnt[0], 1u);  // prefetch the next claim
-    const int s = (int)(item / P::perStep), r = (int)(item % P::perStep);
-    if (r < P::NS) {
-      if (s < j.nf) {
-        item_sum<L>(j, s, r);
-        continue;
-      }
-    } else if (r < P::NS + P::NR) {
-      const int f = s - kDr;
-      if (f >= 0 && f < j.nf) {
-        item_row<L>(j, f, r - P::NS, sm);
-        continue;
-      }
-    } else {
-      const int f = s - kDr - kDc;
-      if (f >= 0 && f < j.nf) {
-        item_col<L>(j, f, r - P::NS - P::NR, sm);
-        continue;
+    const Item it = decode_item<L>(item, j.nf);
+    unsigned tgtA, tgtB;
+    const unsigned* pA = dep_a<L>(j, it, tgtA);
+    const unsigned* pB = dep_b<L>(j, it, tgtB);
+    unsigned curA = seenA, curB = seenB;  // prefetched for this item during the previous one
+    if (tid == 0) {
+      s_item[(iter + 1) & 1] = q1;
+      unsigned tA, tB;
+      const Item nx = q1 < total ? decode_item<L>(q1, j.nf) : Item{3, 0, 0};
+      const unsigned* nA = dep_a<L>(j, nx, tA);
+      const unsigned* nB = dep_b<L>(j, nx, tB);
+      seenA = nA ? ld_relaxed(nA) : 0u;
+      seenB = nB ? ld_relaxed(nB) : 0u;
+      q1 = atomicAdd(&j.cnt[0], 1u);
+      if (iter == 0) {  // nothing was prefetched for the very first item
+        curA = pA ? ld_relaxed(pA) : 0u;
+        curB = pB ? ld_relaxed(pB) : 0u;
       }
     }
-    __syncthreads();  // no-op item: keep s_item's reader/writer ordering
+
+    if (it.type == 0) {
+      item_sum<L>(j, it.f, it.blk, s_part);
+      continue;
+    }
+    if (it.type == 3) {
+      __syncthreads();  // keeps the s_item double buffer ordered
+      continue;
+    }
+
+    // ---------------- row or column item: load phase ----------------
+    const int f = it.f;
+    const bool is_row = it.type == 1;
+    float2 u[32];
+    int q = it.blk * P::Fc + team;  // row item: complex FFT index (image rows 2q, 2q+1); column item: kx
+    bool valid;
+    float2* rowT = j.rowT + (size_t)(f % P::slots) * Pn;
+    if (is_row) {
+      valid = q < P::rowFfts;
+      if (!valid) q = P::rowFfts - 1;
+      const int64_t ra = (int64_t)(2 * q) * W, rb = ra + W;
+      const uint16_t* fr = j.frames + (int64_t)f * W * H;
+      Chunk ck[2];
+      chunk_load(ck[0], j, fr, ra, rb, tau);  // in flight while thread 0 checks this frame's sum
+      if (tid == 0) {
+        spin_until(pA, tgtA, curA);
+        acquire_fence();
+        s_sum = __ldcg(&j.sums[f]);
+      }
+      __syncthreads();
+      float hi = 0.f, lo = 0.f;
+      if (j.mode == 0) frame_scale(s_sum, (float)W * (float)H, hi, lo, j.flags);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        if (r < 3) chunk_load(ck[(r + 1) & 1], j, fr, ra, rb, tau + P::T * (r + 1));
+        chunk_stage(ck[r & 1], j.mode, hi, lo, buf, tau + P::T * r);
+      }
+      team_sync<P::T>(team);
+#pragma unroll
+      for (int t = 0; t < 32; ++t) u[t] = buf[stage_slot(t * P::T + tau)];
+      team_sync<P::T>(team);
+    } else {
+      valid = q <= n;
+      if (!valid) q = n;
+      if (tid == 0) {
+        spin_until(pA, tgtA, curA);
+        acquire_fence();
+      }
+      __syncthreads();
+      const float2* src = rowT + (size_t)q * H;
+#pragma unroll
+      for (int t = 0; t < 32; ++t) u[t] = __ldcg(&src[t * P::T + tau]);
+    }
+
+    // ---------------- the FFT itself (one call site: the code is large) ----------------
+    fft_team<L>(u, buf, tau, team, j);
+
+    if (is_row) {
+      team_sync<P::T>(team);
+#pragma unroll
+      for (int r = 0; r < 32; ++r) buf[out_index<L>(tau, r)] = u[r];
+      team_sync<P::T>(team);
+      // untangle the two real rows: A[k] = (Z[k] + conj Z[L-k]) / 2,  B[k] = (Z[k] - conj Z[L-k]) / (2i).
+      // In place: slot k <- A[k], slot L-k <- B[k] (1 <= k < n); slot 0 <- A[0], slot n <- B[0]; Nyquist aside.
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const int k = tau + P::T * i;
+        if (k == 0) {
+          const float2 z0 = buf[0], zh = buf[n];
+          buf[0] = make_float2(z0.x, 0.f);
+          buf[n] = make_float2(z0.y, 0.f);
+          nyq[2 * team] = make_float2(zh.x, 0.f);
+          nyq[2 * team + 1] = make_float2(zh.y, 0.f);
+        } else {
+          const float2 zk = buf[k], zm = buf[L - k];
+          buf[k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+          buf[L - k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+        }
+      }
+      // the intermediate slot must have been drained by the column pass of frame f - slots
+      if (tid == 0 && pB) {
+        spin_until(pB, tgtB, curB);
+        acquire_fence();
+      }
+      __syncthreads();
+      // transposed store: rowT[kx][y], 16 bytes (rows 2q, 2q+1) per thread and kx
+      const int y0 = it.blk * P::Fc * 2;
+      constexpr int FcR = P::FcRow;
+      for (int e = tid; e < n * FcR; e += P::NT) {
+        const int kxl = e & 1, ft = (e >> 1) % FcR, kx = 2 * (e / (2 * FcR)) + kxl;
+        const float2* b = sm + (size_t)ft * P::Sf;
+        const float2 A = b[kx], B = b[kx ? L - kx : n];
+        *reinterpret_cast<float4*>(rowT + (size_t)kx * H + y0 + 2 * ft) = make_float4(A.x, A.y, B.x, B.y);
+      }
+      if (tid < FcR) {
+        *reinterpret_cast<float4*>(rowT + (size_t)n * H + y0 + 2 * tid) =
+            make_float4(nyq[2 * tid].x, nyq[2 * tid].y, nyq[2 * tid + 1].x, nyq[2 * tid + 1].y);
+      }
+      signal_count(&j.cnt[1 + j.nf + f]);
+    } else {
+      if (valid) {
+        const int slot = (j.R > 0) ? (int)((j.t_first + f) % j.R) : 0;
+        float2* dst = j.dst + (size_t)slot * Pn + (size_t)q * H;
+        const float sc = j.scale;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) dst[out_index<L>(tau, r)] = make_float2(u[r].x * sc, u[r].y * sc);
+      }
+      signal_count(&j.cnt[1 + 2 * j.nf + f]);
+    }
   }
 }
 
@@ -530,7 +627,7 @@ static int launch_fft_L(Ctx& c, const FftJob& job, int cls) {
     if (per_sm < 1) per_sm = 1;
     c.fft_grid = per_sm * sms;
   }
-  const long long total = (long long)(job.nf + kDr + kDc) * P::perStep;
+  const long long total = (long long)(job.nf + P::Dr + P::Dc) * P::perStep;
   const int grid = (int)std::min<long long>(c.fft_grid, total);
   ProfScope ps(c, cls);
   cudaMemsetAsync(c.fft_cnt, 0, sizeof(unsigned) * (1 + 3 * (size_t)job.nf) + 0, c.stream);
@@ -553,7 +650,23 @@ static int launch_fft(Ctx& c, const FftJob& job, int cls) {
   }
 }
 
-size_t fft_rowT_elems(const Ctx& c) { return (size_t)kSlots * (size_t)c.P; }
+template <int L>
+static constexpr int slots_of() { return Plan<L>::slots; }
+size_t fft_rowT_elems(const Ctx& c) {
+  int slots = kMaxSlots;
+  switch (c.W) {
+    case 32: slots = slots_of<32>(); break;
+    case 64: slots = slots_of<64>(); break;
+    case 128: slots = slots_of<128>(); break;
+    case 256: slots = slots_of<256>(); break;
+    case 512: slots = slots_of<512>(); break;
+    case 1024: slots = slots_of<1024>(); break;
+    case 2048: slots = slots_of<2048>(); break;
+    case 4096: slots = slots_of<4096>(); break;
+    default: break;
+  }
+  return (size_t)slots * (size_t)c.P;
+}
 
 static FftJob make_job(Ctx& c) {
   FftJob j;
