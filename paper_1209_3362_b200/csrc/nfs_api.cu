@@ -294,6 +294,11 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
     }
   }
   if (!dev_alloc(c, &c.ring, (size_t)c.R * c.P)) goto fail;
+  if (!lag_make_tensor_map(c)) {
+    c.status = NFS_ERR_CUDA;
+    c.cuda_err = "cuTensorMapEncodeTiled failed";
+    goto fail;
+  }
   if (!dev_alloc(c, &c.rowbuf, fft_rowT_elems(c))) goto fail;
   if (!dev_alloc(c, &c.ref, (size_t)W * H)) goto fail;
   if (!dev_alloc(c, &c.Fref, (size_t)c.P)) goto fail;

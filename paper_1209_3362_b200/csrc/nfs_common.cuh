@@ -8,6 +8,7 @@
 //   totals         double[n_lags][P]   sum over pairs of |F'_t - F'_{t+tau}|^2   ("differences area", L33)
 //   ref            float[H][W]   first normalised frame r; F'_t = FFT(i_t - r)   (linearity, L31)
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -19,10 +20,10 @@
 namespace nfs {
 
 // ---- lag-accumulation plan (built on the host at create) -------------------------------------------
-constexpr int kG = 10;        // lags per warp task (register window depth)
+constexpr int kG = 13;        // lags per warp task (register window depth)
 constexpr int kTilePx = 32;   // Fourier pixels per CTA tile (one warp width)
-constexpr int kMaxTasks = 10; // warp tasks per CTA (lag group)
-constexpr int kChunk = 20;    // time steps per shared-memory pipeline stage (multiple of kG)
+constexpr int kMaxTasks = 4;  // consumer warps (lag tasks) per CTA: one per SM sub-partition
+constexpr int kChunk = 26;    // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
 constexpr int kSpanMax = 128; // max (tau_max - tau_min + 1) of a lag group
 
 struct LagTask {
@@ -59,6 +60,7 @@ struct Ctx {
 
   // device memory
   float2* ring = nullptr;
+  CUtensorMap ring_map;          // 2-D TMA descriptor of the ring (nfs_lag.cu)
   float2* rowbuf = nullptr;      // [slots][P] output of the row pass (transposed, L2 resident)
   float* ref = nullptr;          // [H][W]
   float2* Fref = nullptr;        // [P] unitary FFT of ref
@@ -122,6 +124,7 @@ int launch_accum_I(Ctx& c, int64_t t0, int b);
 int launch_lag_simple(Ctx& c, int64_t t0, int b);
 int launch_lag_tiled(Ctx& c, int64_t t0, int b);
 size_t lag_tiled_smem_bytes(const LagGroup& g);
+bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout

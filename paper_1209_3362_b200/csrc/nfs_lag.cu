@@ -3,7 +3,7 @@
 // moduli of FFT differences are evaluated N(N-1)/2 times"; L25 average over the measurement time).
 //
 // k_lag_tiled (default): a CTA owns 32 consecutive Fourier pixels and one group of lags; a producer
-// warp streams the batch through shared memory with bulk copies (cp.async.bulk + mbarrier, 3 stages):
+// warp streams the batch through shared memory with TMA tensor copies (cp.async.bulk.tensor + mbarrier):
 // a NEW stream (frames s) and an OLD stream delayed by the group's lags.  A consumer warp owns up to
 // kG lags: for a run of contiguous lags it keeps a rotating register window of the kG most recent OLD
 // frames, so one step costs two LDS.64 and kG pair-updates (packed sub.f32x2 + fma.rn.f32x2: two issue
@@ -84,23 +84,28 @@ __global__ void __launch_bounds__(128) k_lag_simple(const float2* __restrict__ r
 }
 
 // ------------------------------------------------------------------------------------------------
-// tiled kernel: warp-specialised.  Warp 0 = producer (bulk copies global -> shared, completion on
-// mbarriers), warps 1..ntasks = consumers (one lag task each).  Shared memory:
-//   OLD ring  [DEPTH + G - 1][32] float2   frames s - tau for the group's lags; row e holds global
-//             frame f_old0 + e at row e % DEPTH (rows 0..G-2 duplicated behind the end so that a
-//             block of G consecutive rows never wraps)
-//   NEW       [kStages][kChunk][32] float2 the batch's own frames
-// Chunk c (kChunk time steps) lives in stage c % kStages; full[stage] counts the producer lanes'
-// arrivals + the bytes of their copies, empty[stage] counts the consumer warps that are done with it.
+// tiled kernel: warp-specialised.  Warps 0..ntasks-1 = consumers (one lag task each), the last warp =
+// producer (highest warp id: first in the issue arbiter, so loads are never starved by the math warps).
+// Time is cut into chunks of kChunk = kBPC*kG steps.  Shared memory, in rows of 32 pixels (256 B):
+//   OLD  [(NSLOT + 1) * kChunk]  ring of NSLOT = LEAD + kStages chunk slots; OLD row e holds frame
+//                                E0 + e, E0 = t0 - tau_min - LEAD*kChunk, at row e % (NSLOT*kChunk); the
+//                                last kChunk rows duplicate slot 0 so kG consecutive rows never wrap
+//   NEW  [kStages * kChunk]      the batch's own frames, chunk c in stage c % kStages
+// full[stage]: the producer's arrival + the bytes of its copies for consumer chunk c (NEW chunk c, OLD
+// chunk c + LEAD; chunk 0 also brings OLD chunks 0..LEAD-1).  empty[stage]: the consumer warps.
+// A chunk of frames that is contiguous in the HBM ring is one 2-D TMA box (cp.async.bulk.tensor,
+// 32 pixels x kChunk ring slots); a chunk that straddles the ring's wrap-around or starts before the
+// first frame falls back to one 256-byte bulk copy per row.
 // ------------------------------------------------------------------------------------------------
 constexpr int kRowF2 = kTilePx;                 // float2 per shared-memory row (one frame, 32 pixels = 256 B)
 constexpr unsigned kRowBytes = kRowF2 * 8u;
-constexpr int kStages = 3;
+constexpr int kStages = 2;
 
-__host__ __device__ inline int lag_depth(int tau_min, int tau_max) { return (tau_max - tau_min) + kStages * kChunk; }
+__host__ __device__ inline int lag_lead(int tau_min, int tau_max) { return (tau_max - tau_min + kChunk - 1) / kChunk; }
 
 size_t lag_tiled_smem_bytes(const LagGroup& g) {
-  return 64 + sizeof(float2) * kRowF2 * (size_t)(lag_depth(g.tau_min, g.tau_max) + kG - 1 + kStages * kChunk);
+  const int nslot = lag_lead(g.tau_min, g.tau_max) + kStages;
+  return 128 + sizeof(float2) * kRowF2 * (size_t)((nslot + 1) * kChunk + kStages * kChunk);
 }
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -133,6 +138,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+// 2-D tensor copy global -> shared (SASS UTMALDG): box = 32 pixels (64 floats) x kChunk ring slots
+__device__ __forceinline__ void tma_box_g2s(void* dst, const CUtensorMap* tmap, int c0, int c1, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(
+          smem_u32(dst)),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+      : "memory");
+}
 
 // packed fp32x2 arithmetic (SASS FADD2 / FFMA2): one issue slot for both components of a complex number
 typedef unsigned long long f2x;
@@ -154,115 +167,129 @@ __device__ __forceinline__ float f2x_sum(f2x v) {
   return __uint_as_float((unsigned)(v & 0xffffffffull)) + __uint_as_float((unsigned)(v >> 32));
 }
 
+// producer: bring frames f0 .. f0+kChunk-1 of this pixel tile into shared rows dst (and dup, if given).
+// Returns the bytes this lane's copies will complete on the barrier.
+__device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const float2* __restrict__ ring, int R, int64_t P,
+                                               int64_t p0, int64_t f0, f2x* dst, f2x* dup, uint64_t* bar, int lane) {
+  const int s0 = (int)(((f0 % R) + R) % R);
+  if (f0 >= 0 && s0 + kChunk <= R) {
+    if (lane != 0) return 0u;
+    tma_box_g2s(dst, tmap, (int)(2 * p0), s0, bar);
+    if (dup) tma_box_g2s(dup, tmap, (int)(2 * p0), s0, bar);
+    return (dup ? 2u : 1u) * kChunk * kRowBytes;
+  }
+  unsigned bytes = 0;
+  if (lane < kChunk) {
+    const int64_t f = f0 + lane;
+    if (f >= 0) {  // rows before the first frame are never used
+      const float2* src = ring + (f % R) * P + p0;
+      bulk_g2s(dst + (size_t)lane * kRowF2, src, kRowBytes, bar);
+      bytes = kRowBytes;
+      if (dup) {
+        bulk_g2s(dup + (size_t)lane * kRowF2, src, kRowBytes, bar);
+        bytes += kRowBytes;
+      }
+    }
+  }
+  return bytes;
+}
+
 template <int G>
-__global__ void __launch_bounds__((kMaxTasks + 1) * 32, 2)
-    k_lag_tiled(const float2* __restrict__ ring, int R, int64_t P, int64_t t0, int b, const LagTask* __restrict__ tasks,
-                const LagGroup* __restrict__ groups, const int32_t* __restrict__ lags, double* __restrict__ totals) {
+__global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
+    k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
+                int b, int ngroups, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
+                const int32_t* __restrict__ lags, double* __restrict__ totals) {
+  static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
   extern __shared__ __align__(128) unsigned char smraw[];
-  const LagGroup grp = groups[blockIdx.y];
+  const int gi = blockIdx.x % ngroups;  // groups of one pixel tile run side by side (they share L2 lines)
+  const LagGroup grp = groups[gi];
   if ((int64_t)grp.tau_min > t0 + b - 1) return;  // no frame pair of this group exists yet
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t p0 = (int64_t)blockIdx.x * kTilePx;
-  const int DEPTH = lag_depth(grp.tau_min, grp.tau_max);
+  const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
+  const int LEAD = lag_lead(grp.tau_min, grp.tau_max);
+  const int NSLOT = LEAD + kStages;
+  const int DEPTH = NSLOT * kChunk;
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw);      // [kStages]
   uint64_t* empty = full + kStages;                         // [kStages]
-  f2x* OLD = reinterpret_cast<f2x*>(smraw + 64);            // [DEPTH + G - 1][32]
-  f2x* NEW = OLD + (size_t)(DEPTH + G - 1) * kRowF2;        // [kStages][kChunk][32]
-  const int span1 = grp.tau_max - grp.tau_min;              // OLD rows needed before the first step
+  f2x* OLD = reinterpret_cast<f2x*>(smraw + 128);           // [(NSLOT + 1) * kChunk][32]
+  f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * kRowF2;   // [kStages][kChunk][32]
   const int nchunks = (b + kChunk - 1) / kChunk;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(&full[s], 32);
+      mbar_init(&full[s], 1);
       mbar_init(&empty[s], (unsigned)grp.ntasks);
     }
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
 
-  if (warp == 0) {
+  if (warp == kMaxTasks) {
     // ------------------------------- producer -------------------------------
-    const int64_t f_old0 = t0 - grp.tau_max;  // global frame of OLD coordinate e = 0
-    const float2* tile = ring + p0;
+    const int64_t E0 = t0 - grp.tau_min - (int64_t)LEAD * kChunk;  // frame held by OLD row 0
     for (int c = 0; c < nchunks; ++c) {
       const int st = c % kStages;
       if (c >= kStages) mbar_wait(&empty[st], ((c / kStages) - 1) & 1);
-      // OLD rows of this chunk: the first chunk also brings the span1 rows preceding the first step
-      const int e_first = c == 0 ? 0 : span1 + c * kChunk;
-      const int count = c == 0 ? span1 + kChunk : kChunk;
-      unsigned bytes = 0;
-      for (int i = lane; i < count; i += 32) {
-        const int e = e_first + i;
-        const int64_t f = f_old0 + e;
-        if (f < 0 || f >= t0 + b) continue;  // before the first frame / beyond this batch: never used
-        const int row = e % DEPTH;
-        const float2* src = tile + (f % R) * P;
-        bulk_g2s(OLD + (size_t)row * kRowF2, src, kRowBytes, &full[st]);
-        bytes += kRowBytes;
-        if (row < G - 1) {
-          bulk_g2s(OLD + (size_t)(row + DEPTH) * kRowF2, src, kRowBytes, &full[st]);
-          bytes += kRowBytes;
-        }
+      unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
+                                  nullptr, &full[st], lane);
+      for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
+        const int slot = m % NSLOT;
+        f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
+        f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
+        bytes += load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)m * kChunk, dst, dup, &full[st], lane);
       }
-      if (lane < kChunk) {
-        const int j = c * kChunk + lane;
-        if (j < b) {
-          bulk_g2s(NEW + ((size_t)st * kChunk + lane) * kRowF2, tile + ((t0 + j) % R) * P, kRowBytes, &full[st]);
-          bytes += kRowBytes;
-        }
-      }
-      mbar_arrive_expect_tx(&full[st], bytes);
+      bytes = __reduce_add_sync(0xffffffffu, bytes);
+      if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
     }
     return;
   }
 
   // ------------------------------- consumers -------------------------------
-  if (warp > grp.ntasks) return;
-  const LagTask tk = tasks[grp.task0 + warp - 1];
-  // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  w: dense task = rotating window of OLD
-  // frames; sparse task = low word of w[i] holds the OLD row of lag i at the current block start.
+  if (warp >= grp.ntasks) return;
+  const LagTask tk = tasks[grp.task0 + warp];
+  // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  Dense task: w = rotating window of the G most
+  // recent OLD frames.  Sparse task: the low word of w[i] holds the OLD row of lag i at the block start.
   f2x acc[G], w[G];
 #pragma unroll
   for (int g = 0; g < G; ++g) acc[g] = 0ull, w[g] = 0ull;
-  // validity in batch-relative steps: pair (j, lag) exists iff j >= lag - t0
-  const int64_t dt = (int64_t)tk.tau0 - t0;
-  int jfirst, jlast, o0 = 0;
+  // OLD row (before the ring modulo) of the frame that lag tau pairs with step j:  j + off(tau)
+  const int offbase = LEAD * kChunk + grp.tau_min;  // off(tau) = offbase - tau  >= 0
+  int o0 = 0;           // dense: ring row of frame (t0 + jb - tau0) at the current block start
+  int64_t tau_hi;       // largest lag of the task: all pairs of step j exist iff t0 + j >= tau_hi
+  bool wvalid = false;  // dense: the register window matches the current block start
   if (tk.kind == 0) {
-    jfirst = (int)max(dt, (int64_t)-(1 << 24));
-    jlast = jfirst + tk.cnt - 1;
-    o0 = (grp.tau_max - tk.tau0) % DEPTH;
+    o0 = (offbase - tk.tau0) % DEPTH;
+    tau_hi = tk.tau0 + tk.cnt - 1;
   } else {
-    jfirst = (int)max((int64_t)lags[tk.l0] - t0, (int64_t)-(1 << 24));
-    jlast = (int)max((int64_t)lags[tk.l0 + tk.cnt - 1] - t0, (int64_t)-(1 << 24));
+    tau_hi = lags[tk.l0 + tk.cnt - 1];
 #pragma unroll
     for (int i = 0; i < G; ++i)
-      if (i < tk.cnt) w[i] = (f2x)(unsigned)((grp.tau_max - lags[tk.l0 + i]) % DEPTH);
+      if (i < tk.cnt) w[i] = (f2x)(unsigned)((offbase - lags[tk.l0 + i]) % DEPTH);
   }
 
   for (int c = 0; c < nchunks; ++c) {
     const int st = c % kStages;
     mbar_wait(&full[st], (c / kStages) & 1);
-
-    if (c == 0 && tk.kind == 0) {
-      // preload the register window with the G-1 OLD frames preceding the first step
-#pragma unroll
-      for (int q = 1; q < G; ++q) {
-        int e = grp.tau_max - tk.tau0 - q;
-        if (e < 0) e = 0;
-        w[G - q] = OLD[(size_t)(e % DEPTH) * kRowF2 + lane];
-      }
-    }
     const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
 #pragma unroll 1
     for (int blk = 0; blk < kChunk / G; ++blk) {
       const int jb = c * kChunk + blk * G;  // batch-relative index of the block's first step
       if (jb >= b) break;
       const f2x* nb = newc + (size_t)blk * G * kRowF2;
+      const bool fast = (jb + G <= b) && (t0 + jb >= tau_hi);
       if (tk.kind == 0) {
-        const f2x* ob = OLD + (size_t)o0 * kRowF2 + lane;
-        if (jb + 2 * G - 1 < jfirst) {
-          // neither this block nor the next one holds a valid pair: nothing to keep
-        } else if (jb + G <= b && jb >= jlast) {
+        if (fast) {
+          if (!wvalid) {
+            // (re)load the window: the G-1 OLD frames that precede the block's first one
+#pragma unroll
+            for (int q = 1; q < G; ++q) {
+              int r = o0 - q;
+              if (r < 0) r += DEPTH;
+              w[G - q] = OLD[(size_t)r * kRowF2 + lane];
+            }
+            wvalid = true;
+          }
+          const f2x* ob = OLD + (size_t)o0 * kRowF2 + lane;
 #pragma unroll
           for (int u = 0; u < G; ++u) {
             const f2x zn = nb[(size_t)u * kRowF2];
@@ -271,22 +298,27 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 2)
             for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
           }
         } else {
-#pragma unroll
+          // warm-up or last partial block: every pair checked, OLD read directly
+          wvalid = false;
+#pragma unroll 1
           for (int u = 0; u < G; ++u) {
+            const int j = jb + u;
+            if (j >= b) break;
             const f2x zn = nb[(size_t)u * kRowF2];
-            w[u] = ob[(size_t)u * kRowF2];
-            const bool in_batch = jb + u < b;
 #pragma unroll
-            for (int g = 0; g < G; ++g)
-              if (in_batch && g < tk.cnt && jb + u >= jfirst + g) upd2(acc[g], zn, w[(u - g + G) % G]);
+            for (int g = 0; g < G; ++g) {
+              if (g < tk.cnt && t0 + j >= (int64_t)tk.tau0 + g) {
+                int r = o0 + u - g;
+                if (r < 0) r += DEPTH;
+                upd2(acc[g], zn, OLD[(size_t)r * kRowF2 + lane]);
+              }
+            }
           }
         }
         o0 += G;
         if (o0 >= DEPTH) o0 -= DEPTH;
       } else {
-        if (jb + G - 1 < jfirst) {
-          // no valid pair in this block
-        } else if (jb + G <= b && jb >= jlast) {
+        if (fast) {
 #pragma unroll
           for (int u = 0; u < G; ++u) {
             const f2x zn = nb[(size_t)u * kRowF2];
@@ -295,13 +327,14 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 2)
               if (i < tk.cnt) upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
           }
         } else {
-#pragma unroll
+#pragma unroll 1
           for (int u = 0; u < G; ++u) {
+            const int j = jb + u;
+            if (j >= b) break;
             const f2x zn = nb[(size_t)u * kRowF2];
-            const bool in_batch = jb + u < b;
 #pragma unroll
             for (int i = 0; i < G; ++i)
-              if (i < tk.cnt && in_batch && (int64_t)(jb + u) >= (int64_t)__ldg(&lags[tk.l0 + i]) - t0)
+              if (i < tk.cnt && t0 + j >= (int64_t)__ldg(&lags[tk.l0 + i]))
                 upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
           }
         }
@@ -317,13 +350,15 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 2)
     if (lane == 0) mbar_arrive(&empty[st]);
   }
 
+  // fold the batch's fp32 partial sums into the fp64 totals: all loads first, then the stores
   const int64_t p = p0 + lane;
+  double tv[G];
 #pragma unroll
   for (int g = 0; g < G; ++g)
-    if (g < tk.cnt) {
-      double* dst = totals + (int64_t)(tk.l0 + g) * P + p;
-      *dst += (double)f2x_sum(acc[g]);
-    }
+    if (g < tk.cnt) tv[g] = totals[(int64_t)(tk.l0 + g) * P + p];
+#pragma unroll
+  for (int g = 0; g < G; ++g)
+    if (g < tk.cnt) totals[(int64_t)(tk.l0 + g) * P + p] = tv[g] + (double)f2x_sum(acc[g]);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -342,18 +377,38 @@ int launch_lag_simple(Ctx& c, int64_t t0, int b) {
   return 1;
 }
 
+// 2-D tensor map over the ring: dim0 = 2*P floats (32 pixels = 64 floats per box), dim1 = R ring slots
+bool lag_make_tensor_map(Ctx& c) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return false;
+  const cuuint64_t gdim[2] = {(cuuint64_t)(2 * c.P), (cuuint64_t)c.R};
+  const cuuint64_t gstride[1] = {(cuuint64_t)c.P * sizeof(float2)};
+  const cuuint32_t box[2] = {(cuuint32_t)(2 * kTilePx), (cuuint32_t)kChunk};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = reinterpret_cast<EncodeFn>(fn)(&c.ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c.ring, gdim, gstride, box,
+                                                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   size_t smem = 0;
   for (const LagGroup& g : c.groups) {
     size_t s = lag_tiled_smem_bytes(g);
     if (s > smem) smem = s;
   }
-  static_assert(kChunk % kG == 0, "chunk must hold whole blocks of kG steps");
   cudaFuncSetAttribute(k_lag_tiled<kG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  dim3 grid((unsigned)(c.P / kTilePx), (unsigned)c.groups.size());
+  const int ngroups = (int)c.groups.size();
+  const unsigned grid = (unsigned)((c.P / kTilePx) * ngroups);
   ProfScope ps(c, kKLag);
-  k_lag_tiled<kG><<<grid, (kMaxTasks + 1) * 32, smem, c.stream>>>(c.ring, c.R, c.P, t0, b, c.d_tasks, c.d_groups, c.d_lags,
-                                                          c.totals);
+  k_lag_tiled<kG><<<grid, (kMaxTasks + 1) * 32, smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.d_tasks,
+                                                                  c.d_groups, c.d_lags, c.totals);
   return 1;
 }
 
