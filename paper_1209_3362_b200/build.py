@@ -29,19 +29,25 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
+    """Compiles the four .cu files and links `out`.  `defines` (e.g. ["NFS_LAG_STAGES=3"]) overrides the
+    tuning constants of nfs_common.cuh / nfs_fft.cu for experiments; the default build passes none."""
+    if not force and out == LIB and not defines and not needs_build():
         return LIB
     objs = []
+    tag = "" if out == LIB else "." + os.path.basename(out)
     for s in SOURCES:
-        o = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
-        subprocess.check_call(cmd)
+        o = os.path.join(CSRC, s.replace(".cu", tag + ".o"))
+        cmd = [_nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else [])
+        subprocess.check_call(cmd + ["-c", os.path.join(CSRC, s), "-o", o])
         objs.append(o)
-    tmp = LIB + ".tmp.%d" % os.getpid()
+    tmp = out + ".tmp.%d" % os.getpid()
     subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, out)
+    if out != LIB:
+        for o in objs:
+            os.remove(o)
+    return out
 
 
 if __name__ == "__main__":

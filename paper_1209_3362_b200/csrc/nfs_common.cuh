@@ -20,10 +20,20 @@
 namespace nfs {
 
 // ---- lag-accumulation plan (built on the host at create) -------------------------------------------
+#ifndef NFS_LAG_BPC
+#define NFS_LAG_BPC 2
+#endif
+#ifndef NFS_LAG_STAGES
+#define NFS_LAG_STAGES 2
+#endif
+#ifndef NFS_LAG_MINB
+#define NFS_LAG_MINB 4
+#endif
 constexpr int kG = 13;        // lags per warp task (register window depth)
 constexpr int kTilePx = 32;   // Fourier pixels per CTA tile (one warp width)
 constexpr int kMaxTasks = 4;  // consumer warps (lag tasks) per CTA: one per SM sub-partition
-constexpr int kChunk = 26;    // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
+constexpr int kChunk = kG * NFS_LAG_BPC;  // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
+constexpr int kStages = NFS_LAG_STAGES;   // pipeline stages of the lag-accumulation kernel
 constexpr int kSpanMax = 128; // max (tau_max - tau_min + 1) of a lag group
 
 struct LagTask {

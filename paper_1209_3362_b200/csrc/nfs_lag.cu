@@ -99,7 +99,6 @@ __global__ void __launch_bounds__(128) k_lag_simple(const float2* __restrict__ r
 // ------------------------------------------------------------------------------------------------
 constexpr int kRowF2 = kTilePx;                 // float2 per shared-memory row (one frame, 32 pixels = 256 B)
 constexpr unsigned kRowBytes = kRowF2 * 8u;
-constexpr int kStages = 2;
 
 __host__ __device__ inline int lag_lead(int tau_min, int tau_max) { return (tau_max - tau_min + kChunk - 1) / kChunk; }
 
@@ -117,6 +116,20 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// producer side: same wait with a suspend-time hint, so that the idle warp does not burn issue slots
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAITR_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+      "@p bra DONER_%=;\n"
+      "bra WAITR_%=;\n"
+      "DONER_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity), "r"(20000u)
+      : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
   asm volatile(
@@ -195,7 +208,7 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
 }
 
 template <int G>
-__global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
+__global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
                 int b, int ngroups, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
                 const int32_t* __restrict__ lags, double* __restrict__ totals) {
@@ -229,7 +242,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
     const int64_t E0 = t0 - grp.tau_min - (int64_t)LEAD * kChunk;  // frame held by OLD row 0
     for (int c = 0; c < nchunks; ++c) {
       const int st = c % kStages;
-      if (c >= kStages) mbar_wait(&empty[st], ((c / kStages) - 1) & 1);
+      if (c >= kStages) mbar_wait_relaxed(&empty[st], ((c / kStages) - 1) & 1);
       unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
                                   nullptr, &full[st], lane);
       for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
@@ -247,25 +260,33 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
   // ------------------------------- consumers -------------------------------
   if (warp >= grp.ntasks) return;
   const LagTask tk = tasks[grp.task0 + warp];
+  const bool dense = tk.kind == 0;
+  const int cnt = tk.cnt;
   // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  Dense task: w = rotating window of the G most
   // recent OLD frames.  Sparse task: the low word of w[i] holds the OLD row of lag i at the block start.
   f2x acc[G], w[G];
 #pragma unroll
   for (int g = 0; g < G; ++g) acc[g] = 0ull, w[g] = 0ull;
-  // OLD row (before the ring modulo) of the frame that lag tau pairs with step j:  j + off(tau)
-  const int offbase = LEAD * kChunk + grp.tau_min;  // off(tau) = offbase - tau  >= 0
+  // OLD row (before the ring modulo) of the frame that lag tau pairs with step j:  j + offbase - tau
+  const int offbase = LEAD * kChunk + grp.tau_min;
   int o0 = 0;           // dense: ring row of frame (t0 + jb - tau0) at the current block start
-  int64_t tau_hi;       // largest lag of the task: all pairs of step j exist iff t0 + j >= tau_hi
   bool wvalid = false;  // dense: the register window matches the current block start
-  if (tk.kind == 0) {
+  int tau_lo, tau_hi;   // smallest / largest lag of the task
+  if (dense) {
     o0 = (offbase - tk.tau0) % DEPTH;
-    tau_hi = tk.tau0 + tk.cnt - 1;
+    tau_lo = tk.tau0;
+    tau_hi = tk.tau0 + cnt - 1;
   } else {
-    tau_hi = lags[tk.l0 + tk.cnt - 1];
+    tau_lo = lags[tk.l0];
+    tau_hi = lags[tk.l0 + cnt - 1];
 #pragma unroll
     for (int i = 0; i < G; ++i)
-      if (i < tk.cnt) w[i] = (f2x)(unsigned)((offbase - lags[tk.l0 + i]) % DEPTH);
+      if (i < cnt) w[i] = (f2x)(unsigned)((offbase - lags[tk.l0 + i]) % DEPTH);
   }
+  // batch-relative step from which every lag (j_all) / any lag (j_any) of the task has a frame pair
+  const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi - t0));
+  const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo - t0));
+  const int t0c = (int)min((int64_t)1 << 30, t0);  // only compared against lags < 2^30 in the warm-up path
 
   for (int c = 0; c < nchunks; ++c) {
     const int st = c % kStages;
@@ -274,11 +295,12 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
 #pragma unroll 1
     for (int blk = 0; blk < kChunk / G; ++blk) {
       const int jb = c * kChunk + blk * G;  // batch-relative index of the block's first step
-      if (jb >= b) break;
+      const int ns = min(G, b - jb);        // steps of this block inside the batch
+      if (ns <= 0) break;
       const f2x* nb = newc + (size_t)blk * G * kRowF2;
-      const bool fast = (jb + G <= b) && (t0 + jb >= tau_hi);
-      if (tk.kind == 0) {
-        if (fast) {
+      if (jb >= j_all) {
+        // ---- every pair of the block exists ----
+        if (dense) {
           if (!wvalid) {
             // (re)load the window: the G-1 OLD frames that precede the block's first one
 #pragma unroll
@@ -290,54 +312,63 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
             wvalid = true;
           }
           const f2x* ob = OLD + (size_t)o0 * kRowF2 + lane;
+          if (ns == G) {
 #pragma unroll
-          for (int u = 0; u < G; ++u) {
-            const f2x zn = nb[(size_t)u * kRowF2];
-            w[u] = ob[(size_t)u * kRowF2];
+            for (int u = 0; u < G; ++u) {
+              const f2x zn = nb[(size_t)u * kRowF2];
+              w[u] = ob[(size_t)u * kRowF2];
 #pragma unroll
-            for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
+              for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
+            }
+          } else {  // last block of the batch
+#pragma unroll
+            for (int u = 0; u < G; ++u) {
+              if (u < ns) {
+                const f2x zn = nb[(size_t)u * kRowF2];
+                w[u] = ob[(size_t)u * kRowF2];
+#pragma unroll
+                for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
+              }
+            }
           }
         } else {
-          // warm-up or last partial block: every pair checked, OLD read directly
-          wvalid = false;
 #pragma unroll 1
-          for (int u = 0; u < G; ++u) {
-            const int j = jb + u;
-            if (j >= b) break;
+          for (int u = 0; u < ns; ++u) {
             const f2x zn = nb[(size_t)u * kRowF2];
 #pragma unroll
-            for (int g = 0; g < G; ++g) {
-              if (g < tk.cnt && t0 + j >= (int64_t)tk.tau0 + g) {
-                int r = o0 + u - g;
-                if (r < 0) r += DEPTH;
-                upd2(acc[g], zn, OLD[(size_t)r * kRowF2 + lane]);
+            for (int i = 0; i < G; ++i)
+              if (i < cnt) upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
+          }
+        }
+      } else if (jb + ns > j_any) {
+        // ---- warm-up: some lags reach back before the first frame; every pair checked, OLD read directly ----
+        wvalid = false;
+#pragma unroll 1
+        for (int u = 0; u < ns; ++u) {
+          const int tj = t0c + jb + u;
+          const f2x zn = nb[(size_t)u * kRowF2];
+#pragma unroll
+          for (int g = 0; g < G; ++g) {
+            if (g < cnt) {
+              if (dense) {
+                if (tj >= tk.tau0 + g) {
+                  int r = o0 + u - g;
+                  if (r < 0) r += DEPTH;
+                  upd2(acc[g], zn, OLD[(size_t)r * kRowF2 + lane]);
+                }
+              } else if (tj >= __ldg(&lags[tk.l0 + g])) {
+                upd2(acc[g], zn, OLD[(size_t)((unsigned)w[g] + u) * kRowF2 + lane]);
               }
             }
           }
         }
+      } else {
+        wvalid = false;  // no pair yet
+      }
+      if (dense) {
         o0 += G;
         if (o0 >= DEPTH) o0 -= DEPTH;
       } else {
-        if (fast) {
-#pragma unroll
-          for (int u = 0; u < G; ++u) {
-            const f2x zn = nb[(size_t)u * kRowF2];
-#pragma unroll
-            for (int i = 0; i < G; ++i)
-              if (i < tk.cnt) upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
-          }
-        } else {
-#pragma unroll 1
-          for (int u = 0; u < G; ++u) {
-            const int j = jb + u;
-            if (j >= b) break;
-            const f2x zn = nb[(size_t)u * kRowF2];
-#pragma unroll
-            for (int i = 0; i < G; ++i)
-              if (i < tk.cnt && t0 + j >= (int64_t)__ldg(&lags[tk.l0 + i]))
-                upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
-          }
-        }
 #pragma unroll
         for (int i = 0; i < G; ++i) {
           unsigned o = (unsigned)w[i] + G;
@@ -355,10 +386,10 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, 4)
   double tv[G];
 #pragma unroll
   for (int g = 0; g < G; ++g)
-    if (g < tk.cnt) tv[g] = totals[(int64_t)(tk.l0 + g) * P + p];
+    if (g < cnt) tv[g] = totals[(int64_t)(tk.l0 + g) * P + p];
 #pragma unroll
   for (int g = 0; g < G; ++g)
-    if (g < tk.cnt) totals[(int64_t)(tk.l0 + g) * P + p] = tv[g] + (double)f2x_sum(acc[g]);
+    if (g < cnt) totals[(int64_t)(tk.l0 + g) * P + p] = tv[g] + (double)f2x_sum(acc[g]);
 }
 
 // ------------------------------------------------------------------------------------------------
