@@ -232,7 +232,7 @@ def run_ours(args, cfg):
     inst_per_update = 4.0          # 2 FADD + 2 FFMA lane-instructions
     peak_tflops = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * (flop_per_update / inst_per_update) / 1e12
     ach_tflops = updates * flop_per_update / lag_s_per_step / 1e12
-    B = args.batch or 256
+    B = args.batch or 512
     nb = (cfg.N + B - 1) // B
     lag_bytes = P * (8.0 * (cfg.N + nb * (cfg.lags[-1])) * (1 + 0) + 16.0 * len(cfg.lags) * nb)
     fft_ms = ktimes["fft"][0]

@@ -59,8 +59,9 @@ typedef enum nfs_status {
  *   n_qbins         number of |q| bins on [0, pi rad/px).
  *   cuda_stream     a cudaStream_t cast to void*, or NULL for a library-owned stream.  All device
  *                   work of this context is enqueued on it.
- * nfs_create_ex additionally fixes the internal batch size (frames transformed and accumulated per
- * kernel wave; 0 = default 256).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
+ * nfs_create_ex additionally fixes the internal batch size (0 = default 512): pushed frames are
+ * transformed into the ring at once, their frame pairs are accumulated whenever `batch` frames are
+ * pending (and at every finalize/getter).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
  */
 NFS_API int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream);
 NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
@@ -72,7 +73,8 @@ NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int 
  * Stream-ordered and asynchronous to the host: d_frames must stay valid and unmodified until the
  * work enqueued by this call on the context's stream has run (record an event after the call).
  * Frames are numbered in push order; results do not depend on how a stack is split across calls
- * beyond fp32 partial-sum rounding (<= 1e-6 relative).
+ * (batches are cut by frame number, not by call; an interleaved finalize/getter cuts a batch early,
+ * which changes fp32 partial-sum rounding only, <= 1e-6 relative).
  */
 NFS_API int nfs_push_frames(nfs_ctx* ctx, const uint16_t* d_frames, int n);
 

@@ -220,6 +220,7 @@ bool zero_state(Ctx& c) {
   ok &= NFS_CUDA(c, cudaMemsetAsync(c.I1, 0, sizeof(double2) * (size_t)c.P, c.stream));
   ok &= NFS_CUDA(c, cudaMemsetAsync(c.d_flags, 0, sizeof(int), c.stream));
   c.n_frames = 0;
+  c.n_acc = 0;
   c.n_launches = 0;
   return ok;
 }
@@ -239,6 +240,17 @@ void ring_to_plane(const Ctx& c, const double* src, double* out) {
   const int n = c.n, H = c.H;
   for (int y = 0; y < H; ++y)
     for (int x = 0; x <= n; ++x) out[(size_t)y * (n + 1) + x] = src[(size_t)x * H + y];
+}
+
+// steps S5 (+ the I accumulators) for the frames transformed since the last accumulation
+bool flush_pending(Ctx& c) {
+  const int b = (int)(c.n_frames - c.n_acc);
+  if (b <= 0) return true;
+  c.n_launches += launch_accum_I(c, c.n_acc, b);
+  c.n_launches += (c.lag_variant == 1) ? launch_lag_simple(c, c.n_acc, b) : launch_lag_tiled(c, c.n_acc, b);
+  if (!check_launch(c, "lag launch")) return false;
+  c.n_acc = c.n_frames;
+  return true;
 }
 
 }  // namespace
@@ -268,7 +280,7 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   c.n_qbins = n_qbins;
   c.lags.assign(lags, lags + n_lags);
   c.Lmax = lags[n_lags - 1];
-  c.B = batch_frames > 0 ? batch_frames : 256;
+  c.B = batch_frames > 0 ? batch_frames : 512;
   c.R = c.Lmax + c.B;
 
   int dev = 0;
@@ -343,17 +355,16 @@ int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) {
   const int64_t fpx = (int64_t)c.W * c.H;
   int done = 0;
   while (done < n) {
-    const int b = std::min(c.B, n - done);
-    const int64_t t0 = c.n_frames;
+    // transform as many frames as the ring has room for; accumulate whenever a full batch is pending
+    const int pending = (int)(c.n_frames - c.n_acc);
+    const int b = std::min(c.B - pending, n - done);
     const uint16_t* fr = d_frames + (int64_t)done * fpx;
-    if (t0 == 0) c.n_launches += launch_make_ref(c, fr);
-    c.n_launches += launch_fft_frames(c, fr, b, t0);
+    if (c.n_frames == 0) c.n_launches += launch_make_ref(c, fr);
+    c.n_launches += launch_fft_frames(c, fr, b, c.n_frames);
     if (!check_launch(c, "fft launch")) return c.status;
-    c.n_launches += launch_accum_I(c, t0, b);
-    c.n_launches += (c.lag_variant == 1) ? launch_lag_simple(c, t0, b) : launch_lag_tiled(c, t0, b);
-    if (!check_launch(c, "lag launch")) return c.status;
     c.n_frames += b;
     done += b;
+    if (c.n_frames - c.n_acc == c.B && !flush_pending(c)) return c.status;
   }
   return NFS_OK;
 }
@@ -363,6 +374,7 @@ int nfs_finalize(nfs_ctx* h, double* D_q_tau, double* I_q, int64_t* counts) {
   Ctx& c = h->c;
   if (c.status != NFS_OK) return c.status;
   if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_bin(c);
   if (!check_launch(c, "bin launch")) return c.status;
   const size_t nD = (size_t)c.n_lags * c.n_qbins;
@@ -401,6 +413,7 @@ int nfs_get_D2d(nfs_ctx* h, int lag_index, double* out) {
   if (lag_index < 0 || lag_index >= c.n_lags) return NFS_ERR_INVALID_ARG;
   if (c.status != NFS_OK) return c.status;
   if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_D2d(c, lag_index, c.d_tmp);
   if (!check_launch(c, "D2d launch")) return c.status;
   return get_plane(c, out);
@@ -411,6 +424,7 @@ int nfs_get_I2d(nfs_ctx* h, double* out) {
   Ctx& c = h->c;
   if (c.status != NFS_OK) return c.status;
   if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_I2d(c, c.d_tmp);
   if (!check_launch(c, "I2d launch")) return c.status;
   return get_plane(c, out);

@@ -60,7 +60,8 @@ struct Ctx {
   std::vector<int64_t> counts;  // full-plane pixel count per bin
   cudaStream_t stream = nullptr;
   bool own_stream = false;
-  int64_t n_frames = 0;
+  int64_t n_frames = 0;  // frames pushed (all transformed into the ring)
+  int64_t n_acc = 0;     // of those, frames whose pairs are already in the totals
   int64_t n_launches = 0;
   int lag_variant = 0;
   int status = 0;  // sticky

@@ -381,15 +381,13 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
     if (lane == 0) mbar_arrive(&empty[st]);
   }
 
-  // fold the batch's fp32 partial sums into the fp64 totals: all loads first, then the stores
+  // fold the batch's fp32 partial sums into the fp64 totals.  One reduction (RED.ADD.F64 in L2, nothing
+  // returns to the SM) per (lag, pixel) and launch, launches are stream ordered: the order of the
+  // additions is fixed and the result deterministic.
   const int64_t p = p0 + lane;
-  double tv[G];
 #pragma unroll
   for (int g = 0; g < G; ++g)
-    if (g < cnt) tv[g] = totals[(int64_t)(tk.l0 + g) * P + p];
-#pragma unroll
-  for (int g = 0; g < G; ++g)
-    if (g < cnt) totals[(int64_t)(tk.l0 + g) * P + p] = tv[g] + (double)f2x_sum(acc[g]);
+    if (g < cnt) atomicAdd(&totals[(int64_t)(tk.l0 + g) * P + p], (double)f2x_sum(acc[g]));
 }
 
 // ------------------------------------------------------------------------------------------------
