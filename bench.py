@@ -26,6 +26,9 @@ import numpy as np  # noqa: E402
 
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128
+# DRAM bytes (read + write) of one k_lag_tiled launch from the committed `ncu --set full` capture
+# (profiles/r01_summary.md), keyed by (workload, internal batch, frames); other workloads report null.
+NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {}
 
 
 def load_peaks():
@@ -225,28 +228,40 @@ def run_ours(args, cfg):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (lag accumulation) ----
+    # ---- roofline of the dominant kernel (lag accumulation, k_lag_tiled) ----
+    # Algorithmic work per launch: one pair update = 2 FADD + 2 FFMA on fp32 = 4 lane-instructions
+    # = 6 flops; the kernel's average launch duration comes from CUDA events recorded around every launch on
+    # the library's stream (nfs_set_profiling) over the timed region.
     lag_ms, lag_n = ktimes["lag_accum"]
-    lag_s_per_step = lag_ms * 1e-3 / args.steps
-    flop_per_update = 6.0          # 2 sub + 2 mul + 2 add
-    inst_per_update = 4.0          # 2 FADD + 2 FFMA lane-instructions
+    lag_s_per_launch = lag_ms * 1e-3 / max(lag_n, 1)
+    upd_per_launch = updates * args.steps / max(lag_n, 1)
+    flop_per_update = 6.0
+    inst_per_update = 4.0
     peak_tflops = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * (flop_per_update / inst_per_update) / 1e12
-    ach_tflops = updates * flop_per_update / lag_s_per_step / 1e12
+    ach_tflops = upd_per_launch * flop_per_update / lag_s_per_launch / 1e12
     B = args.batch or 512
     nb = (cfg.N + B - 1) // B
-    lag_bytes = P * (8.0 * (cfg.N + nb * (cfg.lags[-1])) * (1 + 0) + 16.0 * len(cfg.lags) * nb)
-    fft_ms = ktimes["fft"][0]
-    fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N
+    # algorithmic HBM bytes of the accumulation: 8*U/B + 16*n_l/B per pixel and new frame
+    lag_bytes = P * (8.0 * (cfg.N + nb * cfg.lags[-1]) + 16.0 * len(cfg.lags) * nb)
+    traffic = NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH.get((cfg.name, B, cfg.N))
     roofline = dict(bound="alu", kernel="k_lag_tiled", achieved=ach_tflops, peak=peak_tflops, unit="TFLOP/s",
-                    frac=ach_tflops / peak_tflops, traffic=None,
-                    peak_source="148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) x 1.5 flop/lane-instr "
-                                "(2 FADD + 2 FFMA per pair-update)" % (peaks["sm_max_mhz"], peaks["source"]),
-                    pair_updates_per_s=updates / lag_s_per_step, ms_per_step=lag_s_per_step * 1e3, launches_per_step=lag_n / args.steps,
-                    hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / lag_s_per_step / 1e9,
-                             peak_gbs=peaks["hbm_gbs"], frac=lag_bytes / lag_s_per_step / 1e9 / peaks["hbm_gbs"]))
-    fft = dict(bound="hbm", ms_per_step=fft_ms / args.steps, algorithmic_gb_per_step=fft_bytes / 1e9,
-               achieved_gbs=fft_bytes / (fft_ms / args.steps * 1e-3) / 1e9, peak_gbs=peaks["hbm_gbs"],
-               frac=fft_bytes / (fft_ms / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"])
+                    frac=ach_tflops / peak_tflops, traffic=traffic,
+                    peak_source="derived (DESIGN.md §7.2): 148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) x 1.5 flop "
+                                "per lane-instruction (2 FADD + 2 FFMA = 6 flops per pair update)" % (peaks["sm_max_mhz"], peaks["source"]),
+                    traffic_source="ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_summary.md",
+                    pair_updates_per_s=upd_per_launch / lag_s_per_launch, ms_per_launch=lag_s_per_launch * 1e3,
+                    ms_per_step=lag_ms / args.steps, launches_per_step=lag_n / args.steps,
+                    hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9,
+                             peak_gbs=peaks["hbm_gbs"], frac=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9 / peaks["hbm_gbs"],
+                             note="of measured copy peak; HBM is not the binding roofline for dense lags (DESIGN.md §7.2)"))
+    fft_ms = ktimes["fft"][0]
+    fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N      # one round trip between the passes
+    fft_bytes_min = (2.0 * cfg.W * cfg.H + 8.0 * P) * cfg.N   # intermediate kept in L2 (what k_fft does)
+    fft_s = fft_ms / args.steps * 1e-3
+    fft = dict(bound="hbm", kernel="k_fft", ms_per_step=fft_ms / args.steps, algorithmic_gb_per_step=fft_bytes / 1e9,
+               achieved_gbs=fft_bytes / fft_s / 1e9, peak_gbs=peaks["hbm_gbs"], frac=fft_bytes / fft_s / 1e9 / peaks["hbm_gbs"],
+               l2_resident_gb_per_step=fft_bytes_min / 1e9, l2_resident_frac=fft_bytes_min / fft_s / 1e9 / peaks["hbm_gbs"],
+               us_per_frame=fft_s / cfg.N * 1e6)
     kernels = {k: dict(ms_per_step=v[0] / args.steps, launches_per_step=v[1] / args.steps) for k, v in ktimes.items()}
 
     cpu = None
