@@ -131,66 +131,11 @@ bool build_tables(Ctx& c) {
   if (!NFS_CUDA(c, cudaMemcpy(c.bin_start, start.data(), sizeof(int32_t) * (nb + 1), cudaMemcpyHostToDevice)))
     return false;
 
-  // lag plan: contiguous runs of >= 4 lags -> dense tasks of kG; everything else -> sparse tasks
-  c.tasks.clear();
-  c.groups.clear();
+  // lag plan (nfs_lag.cu): tasks per consumer warp, groups per CTA, pipeline depth
   const std::vector<int32_t>& L = c.lags;
-  int i = 0;
-  std::vector<int> sparse_pending;  // indices, contiguous in index space
-  auto flush_sparse = [&]() {
-    size_t k = 0;
-    while (k < sparse_pending.size()) {
-      LagTask t;
-      t.kind = 1;
-      t.l0 = sparse_pending[k];
-      t.tau0 = L[t.l0];
-      t.cnt = 0;
-      while (k < sparse_pending.size() && t.cnt < kG && sparse_pending[k] == t.l0 + t.cnt &&
-             L[sparse_pending[k]] - t.tau0 + 1 <= kSpanMax) {
-        ++t.cnt;
-        ++k;
-      }
-      c.tasks.push_back(t);
-    }
-    sparse_pending.clear();
-  };
-  while (i < c.n_lags) {
-    int j = i;
-    while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1) ++j;
-    const int len = j - i + 1;
-    if (len >= 4) {
-      flush_sparse();
-      for (int k = i; k <= j; k += kG) {
-        LagTask t;
-        t.kind = 0;
-        t.l0 = k;
-        t.tau0 = L[k];
-        t.cnt = std::min(kG, j - k + 1);
-        c.tasks.push_back(t);
-      }
-    } else {
-      for (int k = i; k <= j; ++k) sparse_pending.push_back(k);
-    }
-    i = j + 1;
-  }
-  flush_sparse();
-  // groups: consecutive tasks, at most kMaxTasks, lag span at most kSpanMax
-  size_t t = 0;
-  while (t < c.tasks.size()) {
-    LagGroup g;
-    g.task0 = (int)t;
-    g.ntasks = 0;
-    g.tau_min = c.tasks[t].tau0;
-    g.tau_max = g.tau_min;
-    while (t < c.tasks.size() && g.ntasks < kMaxTasks) {
-      const LagTask& tk = c.tasks[t];
-      const int hi = L[tk.l0 + tk.cnt - 1];
-      if (g.ntasks > 0 && hi - g.tau_min + 1 > kSpanMax) break;
-      g.tau_max = std::max(g.tau_max, hi);
-      ++g.ntasks;
-      ++t;
-    }
-    c.groups.push_back(g);
+  if (!lag_plan(c)) {
+    c.status = NFS_ERR_INVALID_ARG;
+    return false;
   }
   if (!dev_alloc(c, &c.d_tasks, c.tasks.size())) return false;
   if (!dev_alloc(c, &c.d_groups, c.groups.size())) return false;
@@ -323,11 +268,6 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   if (!dev_alloc(c, &c.d_tmp, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.d_flags, 1)) goto fail;
   if (!build_tables(c)) goto fail;
-  for (const LagGroup& g : c.groups)
-    if ((int)lag_tiled_smem_bytes(g) > c.max_smem_optin) {
-      c.status = NFS_ERR_INVALID_ARG;
-      goto fail;
-    }
   if (!NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)c.R * c.P, c.stream))) goto fail;
   if (!zero_state(c)) goto fail;
   if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) goto fail;

@@ -19,25 +19,30 @@
 
 namespace nfs {
 
-// ---- lag-accumulation plan (built on the host at create) -------------------------------------------
+// ---- lag-accumulation plan (built on the host at create, nfs_lag.cu: lag_plan) ---------------------
 #ifndef NFS_LAG_BPC
 #define NFS_LAG_BPC 2
 #endif
-#ifndef NFS_LAG_STAGES
-#define NFS_LAG_STAGES 2
+#ifndef NFS_LAG_MAXT
+#define NFS_LAG_MAXT 8
 #endif
 #ifndef NFS_LAG_MINB
-#define NFS_LAG_MINB 4
+#define NFS_LAG_MINB 2
+#endif
+#ifndef NFS_LAG_MAXSTAGES
+#define NFS_LAG_MAXSTAGES 6
 #endif
 constexpr int kG = 13;        // lags per warp task (register window depth)
 constexpr int kTilePx = 32;   // Fourier pixels per CTA tile (one warp width)
-constexpr int kMaxTasks = 4;  // consumer warps (lag tasks) per CTA: one per SM sub-partition
+constexpr int kMaxTasks = NFS_LAG_MAXT;   // consumer warps (lag tasks) per CTA: kMaxTasks / 4 per SM sub-partition
+constexpr int kLagMinBlocks = NFS_LAG_MINB;  // CTAs per SM the kernel is compiled for
 constexpr int kChunk = kG * NFS_LAG_BPC;  // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
-constexpr int kStages = NFS_LAG_STAGES;   // pipeline stages of the lag-accumulation kernel
-constexpr int kSpanMax = 128; // max (tau_max - tau_min + 1) of a lag group
+constexpr int kMinStages = 2;
+constexpr int kMaxStages = NFS_LAG_MAXSTAGES;  // pipeline depth is chosen at create from the shared memory left
+constexpr int kDenseMin = 7;  // contiguous runs of >= kDenseMin lags use the register-window path
 
 struct LagTask {
-  int tau0;  // dense: smallest lag of the run; sparse: unused
+  int tau0;  // smallest lag of the task
   int cnt;   // number of lags handled (<= kG)
   int l0;    // index of the first lag in the sorted lag list
   int kind;  // 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt)
@@ -45,6 +50,8 @@ struct LagTask {
 struct LagGroup {
   int task0, ntasks;
   int tau_min, tau_max;
+  signed char warp_task[16];  // task (relative to task0) run by consumer warp w, or -1: placed so that the
+                              // four SM sub-partitions (warp id mod 4) carry equal work
 };
 
 // kernel classes for the optional per-kernel CUDA-event timing (nfs_set_profiling)
@@ -91,6 +98,8 @@ struct Ctx {
   int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
   LagTask* d_tasks = nullptr;
   LagGroup* d_groups = nullptr;
+  int lag_stages = kMinStages;   // pipeline stages of k_lag_tiled (chosen by lag_plan)
+  size_t lag_smem = 0;           // dynamic shared memory of k_lag_tiled
   std::vector<LagTask> tasks;
   std::vector<LagGroup> groups;
 
@@ -134,7 +143,7 @@ size_t fft_rowT_elems(const Ctx& c);                              // float2 elem
 int launch_accum_I(Ctx& c, int64_t t0, int b);
 int launch_lag_simple(Ctx& c, int64_t t0, int b);
 int launch_lag_tiled(Ctx& c, int64_t t0, int b);
-size_t lag_tiled_smem_bytes(const LagGroup& g);
+bool lag_plan(Ctx& c);             // host: tasks, groups, pipeline depth; false if a lag group cannot fit shared memory
 bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)

@@ -10,6 +10,8 @@
 // slots per update); isolated lags take one LDS.64 per update.  fp32 partial sums per batch are
 // folded into the fp64 totals once per batch (BASELINE.json north_star (4)).
 // k_lag_simple: plain per-pixel kernel through L1/L2, kept as an in-library cross-check.
+#include <algorithm>
+
 #include "nfs_common.cuh"
 
 namespace nfs {
@@ -84,15 +86,18 @@ __global__ void __launch_bounds__(128) k_lag_simple(const float2* __restrict__ r
 }
 
 // ------------------------------------------------------------------------------------------------
-// tiled kernel: warp-specialised.  Warps 0..ntasks-1 = consumers (one lag task each), the last warp =
-// producer (highest warp id: first in the issue arbiter, so loads are never starved by the math warps).
-// Time is cut into chunks of kChunk = kBPC*kG steps.  Shared memory, in rows of 32 pixels (256 B):
-//   OLD  [(NSLOT + 1) * kChunk]  ring of NSLOT = LEAD + kStages chunk slots; OLD row e holds frame
+// tiled kernel: warp-specialised.  Warps 0..kMaxTasks-1 = consumers (one lag task each, placed by the
+// plan so that the four SM sub-partitions carry equal work), the last warp = producer (highest warp
+// id: first in the issue arbiter, so loads are never starved by the math warps).
+// Time is cut into chunks of kChunk = 2*kG steps.  Shared memory, in rows of 32 pixels (256 B):
+//   OLD  [(NSLOT + 1) * kChunk]  ring of NSLOT = LEAD + stages chunk slots; OLD row e holds frame
 //                                E0 + e, E0 = t0 - tau_min - LEAD*kChunk, at row e % (NSLOT*kChunk); the
 //                                last kChunk rows duplicate slot 0 so kG consecutive rows never wrap
-//   NEW  [kStages * kChunk]      the batch's own frames, chunk c in stage c % kStages
+//   NEW  [stages * kChunk]       the batch's own frames, chunk c in stage c % stages
 // full[stage]: the producer's arrival + the bytes of its copies for consumer chunk c (NEW chunk c, OLD
 // chunk c + LEAD; chunk 0 also brings OLD chunks 0..LEAD-1).  empty[stage]: the consumer warps.
+// `stages` (2..kMaxStages) is chosen at create from the shared memory the widest lag group leaves, so
+// that the producer runs several chunks (each ~3 us of math) ahead of the HBM/L2 latency.
 // A chunk of frames that is contiguous in the HBM ring is one 2-D TMA box (cp.async.bulk.tensor,
 // 32 pixels x kChunk ring slots); a chunk that straddles the ring's wrap-around or starts before the
 // first frame falls back to one 256-byte bulk copy per row.
@@ -102,9 +107,9 @@ constexpr unsigned kRowBytes = kRowF2 * 8u;
 
 __host__ __device__ inline int lag_lead(int tau_min, int tau_max) { return (tau_max - tau_min + kChunk - 1) / kChunk; }
 
-size_t lag_tiled_smem_bytes(const LagGroup& g) {
-  const int nslot = lag_lead(g.tau_min, g.tau_max) + kStages;
-  return 128 + sizeof(float2) * kRowF2 * (size_t)((nslot + 1) * kChunk + kStages * kChunk);
+static size_t lag_smem_bytes(int tau_min, int tau_max, int stages) {
+  const int nslot = lag_lead(tau_min, tau_max) + stages;
+  return 128 + sizeof(float2) * kRowF2 * (size_t)((nslot + 1) * kChunk + stages * kChunk);
 }
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -207,31 +212,97 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
   return bytes;
 }
 
-template <int G>
-__global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
+// One block of kG steps of a dense task with exactly CNT lags: step u loads the new frame and the one
+// OLD frame entering the rotating window (2 LDS.64), then CNT pair updates out of registers.
+template <int CNT>
+__device__ __forceinline__ void dense_block(f2x (&acc)[kG], f2x (&w)[kG], const f2x* nb, const f2x* ob) {
+#pragma unroll
+  for (int u = 0; u < kG; ++u) {
+    const f2x zn = nb[(size_t)u * kRowF2];
+    w[u] = ob[(size_t)u * kRowF2];
+#pragma unroll
+    for (int g = 0; g < CNT; ++g) upd2(acc[g], zn, w[(u - g + kG) % kG]);
+  }
+}
+__device__ __forceinline__ void dense_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* nb, const f2x* ob) {
+  switch (cnt) {  // warp-uniform; the plan makes dense tasks of kDenseMin..kG lags
+    case 12: dense_block<12>(acc, w, nb, ob); break;
+    case 11: dense_block<11>(acc, w, nb, ob); break;
+    case 10: dense_block<10>(acc, w, nb, ob); break;
+    case 9: dense_block<9>(acc, w, nb, ob); break;
+    case 8: dense_block<8>(acc, w, nb, ob); break;
+    case 7: dense_block<7>(acc, w, nb, ob); break;
+    default: dense_block<kG>(acc, w, nb, ob); break;  // 13 (and any shorter run: surplus lags are discarded)
+  }
+}
+// ns steps of a sparse task with exactly CNT lags: one LDS.64 per pair update (no window to reuse).
+// The low word of w[i] holds the OLD row of lag i at the block start.
+template <int CNT>
+__device__ __forceinline__ void sparse_block(int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb, const f2x* oldl) {
+  if (ns == kG) {
+#pragma unroll
+    for (int u = 0; u < kG; ++u) {
+      const f2x zn = nb[(size_t)u * kRowF2];
+#pragma unroll
+      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
+    }
+  } else {
+#pragma unroll 1
+    for (int u = 0; u < ns; ++u) {
+      const f2x zn = nb[(size_t)u * kRowF2];
+#pragma unroll
+      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
+    }
+  }
+}
+__device__ __forceinline__ void sparse_dispatch(int cnt, int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb,
+                                                const f2x* oldl) {
+  switch (cnt) {
+    case 1: sparse_block<1>(ns, acc, w, nb, oldl); break;
+    case 2: sparse_block<2>(ns, acc, w, nb, oldl); break;
+    case 3: sparse_block<3>(ns, acc, w, nb, oldl); break;
+    case 4: sparse_block<4>(ns, acc, w, nb, oldl); break;
+    case 5: sparse_block<5>(ns, acc, w, nb, oldl); break;
+    case 6: sparse_block<6>(ns, acc, w, nb, oldl); break;
+    case 7: sparse_block<7>(ns, acc, w, nb, oldl); break;
+    case 8: sparse_block<8>(ns, acc, w, nb, oldl); break;
+    case 9: sparse_block<9>(ns, acc, w, nb, oldl); break;
+    case 10: sparse_block<10>(ns, acc, w, nb, oldl); break;
+    case 11: sparse_block<11>(ns, acc, w, nb, oldl); break;
+    case 12: sparse_block<12>(ns, acc, w, nb, oldl); break;
+    default: sparse_block<kG>(ns, acc, w, nb, oldl); break;
+  }
+}
+
+__global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
-                int b, int ngroups, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
+                int b, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
                 const int32_t* __restrict__ lags, double* __restrict__ totals) {
+  constexpr int G = kG;
   static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
+  static_assert(kMaxTasks <= 16 && kMaxTasks % 4 == 0, "warp_task[16], whole sub-partition rounds");
   extern __shared__ __align__(128) unsigned char smraw[];
   const int gi = blockIdx.x % ngroups;  // groups of one pixel tile run side by side (they share L2 lines)
-  const LagGroup grp = groups[gi];
-  if ((int64_t)grp.tau_min > t0 + b - 1) return;  // no frame pair of this group exists yet
+  const LagGroup& grp = groups[gi];
+  const int tau_min = grp.tau_min, tau_max = grp.tau_max;
+  if ((int64_t)tau_min > t0 + b - 1) return;  // no frame pair of this group exists yet
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
-  const int LEAD = lag_lead(grp.tau_min, grp.tau_max);
-  const int NSLOT = LEAD + kStages;
+  const int LEAD = lag_lead(tau_min, tau_max);
+  const int NSLOT = LEAD + stages;
   const int DEPTH = NSLOT * kChunk;
-  uint64_t* full = reinterpret_cast<uint64_t*>(smraw);      // [kStages]
-  uint64_t* empty = full + kStages;                         // [kStages]
+  uint64_t* full = reinterpret_cast<uint64_t*>(smraw);      // [kMaxStages]
+  uint64_t* empty = full + kMaxStages;                      // [kMaxStages]
+  static_assert(2 * kMaxStages * 8 <= 128, "barriers fit the 128-byte header");
   f2x* OLD = reinterpret_cast<f2x*>(smraw + 128);           // [(NSLOT + 1) * kChunk][32]
-  f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * kRowF2;   // [kStages][kChunk][32]
+  f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * kRowF2;   // [stages][kChunk][32]
   const int nchunks = (b + kChunk - 1) / kChunk;
 
   if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) {
+    const unsigned nt = (unsigned)grp.ntasks;
+    for (int s = 0; s < stages; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], (unsigned)grp.ntasks);
+      mbar_init(&empty[s], nt);
     }
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
@@ -239,10 +310,11 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
 
   if (warp == kMaxTasks) {
     // ------------------------------- producer -------------------------------
-    const int64_t E0 = t0 - grp.tau_min - (int64_t)LEAD * kChunk;  // frame held by OLD row 0
+    const int64_t E0 = t0 - tau_min - (int64_t)LEAD * kChunk;  // frame held by OLD row 0
+    int st = 0;
+    unsigned ph = 0;  // parity of this stage's current use
     for (int c = 0; c < nchunks; ++c) {
-      const int st = c % kStages;
-      if (c >= kStages) mbar_wait_relaxed(&empty[st], ((c / kStages) - 1) & 1);
+      if (c >= stages) mbar_wait_relaxed(&empty[st], ph ^ 1u);
       unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
                                   nullptr, &full[st], lane);
       for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
@@ -253,13 +325,15 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
       }
       bytes = __reduce_add_sync(0xffffffffu, bytes);
       if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
+      if (++st == stages) st = 0, ph ^= 1u;
     }
     return;
   }
 
   // ------------------------------- consumers -------------------------------
-  if (warp >= grp.ntasks) return;
-  const LagTask tk = tasks[grp.task0 + warp];
+  const int tix = grp.warp_task[warp];
+  if (tix < 0) return;
+  const LagTask tk = tasks[grp.task0 + tix];
   const bool dense = tk.kind == 0;
   const int cnt = tk.cnt;
   // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  Dense task: w = rotating window of the G most
@@ -268,7 +342,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
 #pragma unroll
   for (int g = 0; g < G; ++g) acc[g] = 0ull, w[g] = 0ull;
   // OLD row (before the ring modulo) of the frame that lag tau pairs with step j:  j + offbase - tau
-  const int offbase = LEAD * kChunk + grp.tau_min;
+  const int offbase = LEAD * kChunk + tau_min;
   int o0 = 0;           // dense: ring row of frame (t0 + jb - tau0) at the current block start
   bool wvalid = false;  // dense: the register window matches the current block start
   int tau_lo, tau_hi;   // smallest / largest lag of the task
@@ -287,10 +361,12 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
   const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi - t0));
   const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo - t0));
   const int t0c = (int)min((int64_t)1 << 30, t0);  // only compared against lags < 2^30 in the warm-up path
+  const f2x* oldl = OLD + lane;
 
+  int st = 0;
+  unsigned ph = 0;
   for (int c = 0; c < nchunks; ++c) {
-    const int st = c % kStages;
-    mbar_wait(&full[st], (c / kStages) & 1);
+    mbar_wait(&full[st], ph);
     const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
 #pragma unroll 1
     for (int blk = 0; blk < kChunk / G; ++blk) {
@@ -307,20 +383,14 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
             for (int q = 1; q < G; ++q) {
               int r = o0 - q;
               if (r < 0) r += DEPTH;
-              w[G - q] = OLD[(size_t)r * kRowF2 + lane];
+              w[G - q] = oldl[(size_t)r * kRowF2];
             }
             wvalid = true;
           }
-          const f2x* ob = OLD + (size_t)o0 * kRowF2 + lane;
+          const f2x* ob = oldl + (size_t)o0 * kRowF2;
           if (ns == G) {
-#pragma unroll
-            for (int u = 0; u < G; ++u) {
-              const f2x zn = nb[(size_t)u * kRowF2];
-              w[u] = ob[(size_t)u * kRowF2];
-#pragma unroll
-              for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
-            }
-          } else {  // last block of the batch
+            dense_dispatch(cnt, acc, w, nb, ob);
+          } else {  // last block of the batch (surplus lags of a short task are discarded at the fold)
 #pragma unroll
             for (int u = 0; u < G; ++u) {
               if (u < ns) {
@@ -332,13 +402,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
             }
           }
         } else {
-#pragma unroll 1
-          for (int u = 0; u < ns; ++u) {
-            const f2x zn = nb[(size_t)u * kRowF2];
-#pragma unroll
-            for (int i = 0; i < G; ++i)
-              if (i < cnt) upd2(acc[i], zn, OLD[(size_t)((unsigned)w[i] + u) * kRowF2 + lane]);
-          }
+          sparse_dispatch(cnt, ns, acc, w, nb, oldl);
         }
       } else if (jb + ns > j_any) {
         // ---- warm-up: some lags reach back before the first frame; every pair checked, OLD read directly ----
@@ -354,10 +418,10 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
                 if (tj >= tk.tau0 + g) {
                   int r = o0 + u - g;
                   if (r < 0) r += DEPTH;
-                  upd2(acc[g], zn, OLD[(size_t)r * kRowF2 + lane]);
+                  upd2(acc[g], zn, oldl[(size_t)r * kRowF2]);
                 }
               } else if (tj >= __ldg(&lags[tk.l0 + g])) {
-                upd2(acc[g], zn, OLD[(size_t)((unsigned)w[g] + u) * kRowF2 + lane]);
+                upd2(acc[g], zn, oldl[(size_t)((unsigned)w[g] + u) * kRowF2]);
               }
             }
           }
@@ -379,6 +443,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[st]);
+    if (++st == stages) st = 0, ph ^= 1u;
   }
 
   // fold the batch's fp32 partial sums into the fp64 totals.  One reduction (RED.ADD.F64 in L2, nothing
@@ -388,6 +453,150 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, NFS_LAG_MINB)
 #pragma unroll
   for (int g = 0; g < G; ++g)
     if (g < cnt) atomicAdd(&totals[(int64_t)(tk.l0 + g) * P + p], (double)f2x_sum(acc[g]));
+}
+
+// ------------------------------------------------------------------------------------------------
+// host: the lag plan.  Lags are cut into tasks (one consumer warp each) and tasks into groups (one CTA
+// per group and pixel tile).  A run of >= kDenseMin consecutive lags becomes dense tasks of equal size
+// <= kG; the other lags become sparse tasks.  A group takes consecutive lags while its consumer warps
+// (<= kMaxTasks) and its shared-memory window (lag span) fit; the sparse lags of a group are then spread
+// over the warps the dense tasks leave free, and tasks are placed on warps so that the four SM
+// sub-partitions (warp id mod 4) carry equal FP32 work (longest-processing-time first).
+// ------------------------------------------------------------------------------------------------
+namespace {
+struct Atom {
+  int l0, cnt, kind;  // dense task, or one sparse lag (cnt = 1)
+};
+
+void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1,
+                 std::vector<LagTask>& tasks, std::vector<LagGroup>& groups) {
+  LagGroup g;
+  g.task0 = (int)tasks.size();
+  g.tau_min = L[atoms[a0].l0];
+  g.tau_max = L[atoms[a1 - 1].l0 + atoms[a1 - 1].cnt - 1];
+  int n_dense = 0, n_sparse = 0;
+  for (size_t a = a0; a < a1; ++a) (atoms[a].kind == 0 ? n_dense : n_sparse) += 1;
+  // sparse task size: small enough to use the free warps (up to 8 warps in all), large enough to fit them
+  int s = 1;
+  if (n_sparse > 0) {
+    const int free_w = kMaxTasks - n_dense;
+    const int want_w = std::max(1, std::min(free_w, 8 - std::min(n_dense, 7)));
+    s = std::min(kG, std::max(1, (n_sparse + want_w - 1) / want_w));
+    for (;; ++s) {  // stretches are cut separately: make sure the warps suffice
+      int need = 0;
+      size_t a = a0;
+      while (a < a1) {
+        if (atoms[a].kind == 0) { ++a; continue; }
+        size_t e = a;
+        while (e < a1 && atoms[e].kind == 1) ++e;
+        need += ((int)(e - a) + s - 1) / s;
+        a = e;
+      }
+      if (need <= free_w || s >= kG) break;
+    }
+  }
+  size_t a = a0;
+  while (a < a1) {
+    if (atoms[a].kind == 0) {
+      tasks.push_back(LagTask{L[atoms[a].l0], atoms[a].cnt, atoms[a].l0, 0});
+      ++a;
+      continue;
+    }
+    size_t e = a;
+    while (e < a1 && atoms[e].kind == 1) ++e;
+    const int n = (int)(e - a), nt = (n + s - 1) / s;
+    int l = atoms[a].l0;
+    for (int k = 0; k < nt; ++k) {  // equal sizes
+      const int cnt = n / nt + (k < n % nt ? 1 : 0);
+      tasks.push_back(LagTask{L[l], cnt, l, 1});
+      l += cnt;
+    }
+    a = e;
+  }
+  g.ntasks = (int)tasks.size() - g.task0;
+  // placement: heaviest task first onto the least loaded sub-partition that still has a free warp
+  for (int w = 0; w < 16; ++w) g.warp_task[w] = -1;
+  std::vector<int> order(g.ntasks);
+  for (int k = 0; k < g.ntasks; ++k) order[k] = k;
+  auto cost = [&](int k) {
+    const LagTask& t = tasks[g.task0 + k];
+    return t.kind == 0 ? 4 * t.cnt + 2 : 5 * t.cnt + 1;
+  };
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost(x) > cost(y); });
+  int load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0};
+  for (int k : order) {
+    int best = -1;
+    for (int q = 0; q < 4; ++q)
+      if (used[q] < kMaxTasks / 4 && (best < 0 || load[q] < load[best])) best = q;
+    g.warp_task[used[best] * 4 + best] = (signed char)k;
+    used[best] += 1;
+    load[best] += cost(k);
+  }
+  groups.push_back(g);
+}
+}  // namespace
+
+bool lag_plan(Ctx& c) {
+  const std::vector<int32_t>& L = c.lags;
+  int dev = 0, smem_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+  // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
+  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024);
+  budget = std::min(budget, (size_t)c.max_smem_optin);
+  // atoms
+  std::vector<Atom> atoms;
+  for (int i = 0; i < c.n_lags;) {
+    int j = i;
+    while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1) ++j;
+    const int len = j - i + 1;
+    if (len >= kDenseMin) {
+      const int nt = (len + kG - 1) / kG;
+      int l = i;
+      for (int k = 0; k < nt; ++k) {
+        const int cnt = len / nt + (k < len % nt ? 1 : 0);
+        atoms.push_back(Atom{l, cnt, 0});
+        l += cnt;
+      }
+    } else {
+      for (int k = i; k <= j; ++k) atoms.push_back(Atom{k, 1, 1});
+    }
+    i = j + 1;
+  }
+  // greedy groups
+  c.tasks.clear();
+  c.groups.clear();
+  auto fits = [&](size_t a0, size_t a1) {  // atoms [a0, a1) as one group
+    const int tmin = L[atoms[a0].l0], tmax = L[atoms[a1 - 1].l0 + atoms[a1 - 1].cnt - 1];
+    if (lag_smem_bytes(tmin, tmax, kMinStages + 1) > budget && a1 - a0 > 1) return false;
+    int need = 0;
+    size_t a = a0;
+    while (a < a1) {
+      if (atoms[a].kind == 0) { ++need; ++a; continue; }
+      size_t e = a;
+      while (e < a1 && atoms[e].kind == 1) ++e;
+      need += ((int)(e - a) + kG - 1) / kG;
+      a = e;
+    }
+    return need <= kMaxTasks;
+  };
+  size_t a0 = 0;
+  while (a0 < atoms.size()) {
+    size_t a1 = a0 + 1;
+    while (a1 < atoms.size() && fits(a0, a1 + 1)) ++a1;
+    close_group(L, atoms, a0, a1, c.tasks, c.groups);
+    a0 = a1;
+  }
+  // pipeline depth: as deep as the widest group's window leaves room for
+  int stages = kMaxStages;
+  for (const LagGroup& g : c.groups)
+    while (stages > kMinStages && lag_smem_bytes(g.tau_min, g.tau_max, stages) > budget) --stages;
+  size_t smem = 0;
+  for (const LagGroup& g : c.groups) smem = std::max(smem, lag_smem_bytes(g.tau_min, g.tau_max, stages));
+  if (smem > (size_t)c.max_smem_optin) return false;  // a single task's own lag span does not fit
+  c.lag_stages = stages;
+  c.lag_smem = smem;
+  return true;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -427,17 +636,12 @@ bool lag_make_tensor_map(Ctx& c) {
 }
 
 int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
-  size_t smem = 0;
-  for (const LagGroup& g : c.groups) {
-    size_t s = lag_tiled_smem_bytes(g);
-    if (s > smem) smem = s;
-  }
-  cudaFuncSetAttribute(k_lag_tiled<kG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_lag_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
   const int ngroups = (int)c.groups.size();
   const unsigned grid = (unsigned)((c.P / kTilePx) * ngroups);
   ProfScope ps(c, kKLag);
-  k_lag_tiled<kG><<<grid, (kMaxTasks + 1) * 32, smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.d_tasks,
-                                                                  c.d_groups, c.d_lags, c.totals);
+  k_lag_tiled<<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.lag_stages,
+                                                                      c.d_tasks, c.d_groups, c.d_lags, c.totals);
   return 1;
 }
 
