@@ -119,6 +119,19 @@ NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
  * fp32 summation order).  Not a backend switch: both are CUDA kernels of this library. */
 NFS_API int nfs_set_lag_kernel(nfs_ctx* ctx, int variant);
 
+/* Host-only introspection of the lag plan of step S5 (which lags are accumulated
+ * together); makes no CUDA call, so the host logic is testable without a GPU.  Builds the plan
+ * nfs_create would build for `lags` (HOST, strictly increasing, >= 1) on a device with `smem_per_sm`
+ * bytes of shared memory per SM and `smem_optin` bytes per CTA, and writes it to out (HOST, cap int32):
+ *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA]
+ *   per group (21 values): first task, number of tasks, tau_min, tau_max, flags (bit 0: one task of the
+ *     group accumulates the I sums), then for consumer warps 0..15 the task (relative) it runs or -1
+ *   per task (4 values): smallest lag, number of lags, index of its first lag in `lags`, kind (bit 0:
+ *     0 = run of consecutive lags on the register-window path, 1 = lag list; bit 1: also accumulates I)
+ * Returns the number of int32 written (> 0), or NFS_ERR_INVALID_ARG (bad list, cap too small, a single
+ * task's lag span exceeding shared memory). */
+NFS_API int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_optin, int32_t* out, int cap);
+
 /* Forget all frames (accumulators, ring, reference, sticky errors); keeps the plan and the memory. */
 NFS_API int nfs_reset(nfs_ctx* ctx);
 NFS_API void nfs_destroy(nfs_ctx* ctx);

@@ -35,6 +35,7 @@ SYMBOLS = [
     ("nfs_device_bytes", C.c_int64, [_P]),
     ("nfs_num_launches", C.c_int64, [_P]),
     ("nfs_set_lag_kernel", C.c_int, [_P, C.c_int]),
+    ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
     ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
     ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_reset", C.c_int, [_P]),
@@ -104,6 +105,29 @@ def nfs_finalize(handle, n_lags, n_qbins):
     cnt = np.zeros(n_qbins, dtype=np.int64)
     _check(load_library().nfs_finalize(handle, _dp(D, C.c_double), _dp(I_q, C.c_double), _dp(cnt, C.c_int64)), handle)
     return D, I_q, cnt
+
+
+def nfs_plan_lags(lags, smem_per_sm=233472, smem_optin=232448):
+    """Host-only lag plan (no CUDA call): dict(stages, smem, groups=[...], tasks=[...]); see include/nfs.h."""
+    lags = np.ascontiguousarray(lags, dtype=np.int32)
+    cap = 4 + 25 * (len(lags) + 1)
+    out = np.zeros(cap, dtype=np.int32)
+    n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(smem_per_sm), int(smem_optin), _dp(out, C.c_int32), cap)
+    if n < 0:
+        raise NFSError(n)
+    ng, nt, stages, smem = (int(v) for v in out[:4])
+    o = 4
+    groups, tasks = [], []
+    for _ in range(ng):
+        g = out[o:o + 21]
+        groups.append(dict(task0=int(g[0]), ntasks=int(g[1]), tau_min=int(g[2]), tau_max=int(g[3]), flags=int(g[4]),
+                           warp_task=[int(v) for v in g[5:21]]))
+        o += 21
+    for _ in range(nt):
+        t = out[o:o + 4]
+        tasks.append(dict(tau0=int(t[0]), cnt=int(t[1]), l0=int(t[2]), kind=int(t[3])))
+        o += 4
+    return dict(stages=stages, smem=smem, groups=groups, tasks=tasks)
 
 
 def nfs_destroy(handle):

@@ -133,7 +133,10 @@ bool build_tables(Ctx& c) {
 
   // lag plan (nfs_lag.cu): tasks per consumer warp, groups per CTA, pipeline depth
   const std::vector<int32_t>& L = c.lags;
-  if (!lag_plan(c)) {
+  int dev = 0, smem_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+  if (!lag_plan(c, smem_sm)) {
     c.status = NFS_ERR_INVALID_ARG;
     return false;
   }
@@ -191,8 +194,12 @@ void ring_to_plane(const Ctx& c, const double* src, double* out) {
 bool flush_pending(Ctx& c) {
   const int b = (int)(c.n_frames - c.n_acc);
   if (b <= 0) return true;
-  c.n_launches += launch_accum_I(c, c.n_acc, b);
-  c.n_launches += (c.lag_variant == 1) ? launch_lag_simple(c, c.n_acc, b) : launch_lag_tiled(c, c.n_acc, b);
+  if (c.lag_variant == 1) {  // in-library cross-check path: plain kernels
+    c.n_launches += launch_accum_I(c, c.n_acc, b);
+    c.n_launches += launch_lag_simple(c, c.n_acc, b);
+  } else {  // k_lag_tiled also accumulates the I sums of the batch
+    c.n_launches += launch_lag_tiled(c, c.n_acc, b);
+  }
   if (!check_launch(c, "lag launch")) return false;
   c.n_acc = c.n_frames;
   return true;
@@ -379,6 +386,31 @@ int nfs_set_lag_kernel(nfs_ctx* h, int variant) {
   if (!h || variant < 0 || variant > 1) return NFS_ERR_INVALID_ARG;
   h->c.lag_variant = variant;
   return NFS_OK;
+}
+
+int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_optin, int32_t* out, int cap) {
+  if (!lags || n_lags < 1 || !out || cap < 4) return NFS_ERR_INVALID_ARG;
+  for (int l = 0; l < n_lags; ++l)
+    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return NFS_ERR_INVALID_ARG;
+  Ctx c;
+  c.lags.assign(lags, lags + n_lags);
+  c.n_lags = n_lags;
+  c.Lmax = lags[n_lags - 1];
+  c.max_smem_optin = smem_optin;
+  if (!lag_plan(c, smem_per_sm)) return NFS_ERR_INVALID_ARG;
+  const size_t need = 4 + c.groups.size() * 21 + c.tasks.size() * 4;
+  if (need > (size_t)cap) return NFS_ERR_INVALID_ARG;
+  int32_t* o = out;
+  *o++ = (int32_t)c.groups.size();
+  *o++ = (int32_t)c.tasks.size();
+  *o++ = c.lag_stages;
+  *o++ = (int32_t)c.lag_smem;
+  for (const LagGroup& g : c.groups) {
+    *o++ = g.task0, *o++ = g.ntasks, *o++ = g.tau_min, *o++ = g.tau_max, *o++ = g.flags;
+    for (int w = 0; w < 16; ++w) *o++ = g.warp_task[w];
+  }
+  for (const LagTask& t : c.tasks) *o++ = t.tau0, *o++ = t.cnt, *o++ = t.l0, *o++ = t.kind;
+  return (int)need;
 }
 
 int nfs_set_profiling(nfs_ctx* h, int enable) {

@@ -45,11 +45,12 @@ struct LagTask {
   int tau0;  // smallest lag of the task
   int cnt;   // number of lags handled (<= kG)
   int l0;    // index of the first lag in the sorted lag list
-  int kind;  // 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt)
+  int kind;  // bit 0: 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt); bit 1: also accumulates I2, I1
 };
 struct LagGroup {
   int task0, ntasks;
   int tau_min, tau_max;
+  int flags;  // bit 0: one task of this group accumulates the I sums (the group runs for every batch)
   signed char warp_task[16];  // task (relative to task0) run by consumer warp w, or -1: placed so that the
                               // four SM sub-partitions (warp id mod 4) carry equal work
 };
@@ -143,7 +144,9 @@ size_t fft_rowT_elems(const Ctx& c);                              // float2 elem
 int launch_accum_I(Ctx& c, int64_t t0, int b);
 int launch_lag_simple(Ctx& c, int64_t t0, int b);
 int launch_lag_tiled(Ctx& c, int64_t t0, int b);
-bool lag_plan(Ctx& c);             // host: tasks, groups, pipeline depth; false if a lag group cannot fit shared memory
+// host only (no CUDA call): tasks, groups, pipeline depth from the lag list, the shared memory per SM and
+// c.max_smem_optin; false if a lag group cannot fit shared memory
+bool lag_plan(Ctx& c, int smem_per_sm);
 bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)

@@ -122,6 +122,9 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+#ifndef NFS_LAG_PROD_HINT_NS
+#define NFS_LAG_PROD_HINT_NS 20000
+#endif
 // producer side: same wait with a suspend-time hint, so that the idle warp does not burn issue slots
 __device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, unsigned parity) {
   asm volatile(
@@ -133,7 +136,7 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, unsigned parity
       "bra WAITR_%=;\n"
       "DONER_%=:\n"
       "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity), "r"(20000u)
+      "r"(parity), "r"((unsigned)NFS_LAG_PROD_HINT_NS)
       : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
@@ -175,6 +178,11 @@ __device__ __forceinline__ f2x sub2(f2x a, f2x b) {
 __device__ __forceinline__ f2x fma2(f2x a, f2x b, f2x c) {
   f2x r;
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f2x add2(f2x a, f2x b) {
+  f2x r;
+  asm("add.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
   return r;
 }
 __device__ __forceinline__ void upd2(f2x& acc, f2x zn, f2x zo) {
@@ -224,40 +232,21 @@ __device__ __forceinline__ void dense_block(f2x (&acc)[kG], f2x (&w)[kG], const 
     for (int g = 0; g < CNT; ++g) upd2(acc[g], zn, w[(u - g + kG) % kG]);
   }
 }
-__device__ __forceinline__ void dense_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* nb, const f2x* ob) {
-  switch (cnt) {  // warp-uniform; the plan makes dense tasks of kDenseMin..kG lags
-    case 12: dense_block<12>(acc, w, nb, ob); break;
-    case 11: dense_block<11>(acc, w, nb, ob); break;
-    case 10: dense_block<10>(acc, w, nb, ob); break;
-    case 9: dense_block<9>(acc, w, nb, ob); break;
-    case 8: dense_block<8>(acc, w, nb, ob); break;
-    case 7: dense_block<7>(acc, w, nb, ob); break;
-    default: dense_block<kG>(acc, w, nb, ob); break;  // 13 (and any shorter run: surplus lags are discarded)
-  }
-}
-// ns steps of a sparse task with exactly CNT lags: one LDS.64 per pair update (no window to reuse).
+// ns steps of a sparse task with exactly CNT lags (checked path): one LDS.64 per pair update (no window to reuse).
 // The low word of w[i] holds the OLD row of lag i at the block start.
 template <int CNT>
 __device__ __forceinline__ void sparse_block(int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb, const f2x* oldl) {
-  if (ns == kG) {
-#pragma unroll
-    for (int u = 0; u < kG; ++u) {
-      const f2x zn = nb[(size_t)u * kRowF2];
-#pragma unroll
-      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
-    }
-  } else {
 #pragma unroll 1
-    for (int u = 0; u < ns; ++u) {
-      const f2x zn = nb[(size_t)u * kRowF2];
+  for (int u = 0; u < ns; ++u) {
+    const f2x zn = nb[(size_t)u * kRowF2];
 #pragma unroll
-      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
-    }
+    for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
   }
 }
 __device__ __forceinline__ void sparse_dispatch(int cnt, int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb,
                                                 const f2x* oldl) {
   switch (cnt) {
+    case 0: break;  // a task that only accumulates the I sums
     case 1: sparse_block<1>(ns, acc, w, nb, oldl); break;
     case 2: sparse_block<2>(ns, acc, w, nb, oldl); break;
     case 3: sparse_block<3>(ns, acc, w, nb, oldl); break;
@@ -274,18 +263,83 @@ __device__ __forceinline__ void sparse_dispatch(int cnt, int ns, f2x (&acc)[kG],
   }
 }
 
+// ---- whole chunks (kChunk = kChunk/kG blocks) in which every pair of every step exists: the common case ----
+template <int CNT>
+__device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int& o0,
+                                            int DEPTH) {
+#pragma unroll 1
+  for (int blk = 0; blk < kChunk / kG; ++blk) {
+    dense_block<CNT>(acc, w, newc + (size_t)blk * kG * kRowF2, oldl + (size_t)o0 * kRowF2);
+    o0 += kG;
+    if (o0 >= DEPTH) o0 -= DEPTH;
+  }
+}
+__device__ __forceinline__ void dense_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
+                                                     int& o0, int DEPTH) {
+  switch (cnt) {  // warp-uniform; the plan makes dense tasks of kDenseMin..kG lags
+    case 12: dense_chunk<12>(acc, w, newc, oldl, o0, DEPTH); break;
+    case 11: dense_chunk<11>(acc, w, newc, oldl, o0, DEPTH); break;
+    case 10: dense_chunk<10>(acc, w, newc, oldl, o0, DEPTH); break;
+    case 9: dense_chunk<9>(acc, w, newc, oldl, o0, DEPTH); break;
+    case 8: dense_chunk<8>(acc, w, newc, oldl, o0, DEPTH); break;
+    case 7: dense_chunk<7>(acc, w, newc, oldl, o0, DEPTH); break;
+    default: dense_chunk<kG>(acc, w, newc, oldl, o0, DEPTH); break;  // 13 (shorter runs: surplus lags are discarded)
+  }
+}
+template <int CNT>
+__device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH) {
+#pragma unroll 1
+  for (int blk = 0; blk < kChunk / kG; ++blk) {
+    const f2x* nb = newc + (size_t)blk * kG * kRowF2;
+#pragma unroll
+    for (int u = 0; u < kG; ++u) {
+      const f2x zn = nb[(size_t)u * kRowF2];
+#pragma unroll
+      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
+    }
+#pragma unroll
+    for (int i = 0; i < CNT; ++i) {
+      unsigned o = (unsigned)w[i] + kG;
+      if (o >= (unsigned)DEPTH) o -= DEPTH;
+      w[i] = (f2x)o;
+    }
+  }
+}
+__device__ __forceinline__ void sparse_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
+                                                      int DEPTH) {
+  switch (cnt) {
+    case 0: break;  // a task that only accumulates the I sums
+    case 1: sparse_chunk<1>(acc, w, newc, oldl, DEPTH); break;
+    case 2: sparse_chunk<2>(acc, w, newc, oldl, DEPTH); break;
+    case 3: sparse_chunk<3>(acc, w, newc, oldl, DEPTH); break;
+    case 4: sparse_chunk<4>(acc, w, newc, oldl, DEPTH); break;
+    case 5: sparse_chunk<5>(acc, w, newc, oldl, DEPTH); break;
+    case 6: sparse_chunk<6>(acc, w, newc, oldl, DEPTH); break;
+    case 7: sparse_chunk<7>(acc, w, newc, oldl, DEPTH); break;
+    case 8: sparse_chunk<8>(acc, w, newc, oldl, DEPTH); break;
+    case 9: sparse_chunk<9>(acc, w, newc, oldl, DEPTH); break;
+    case 10: sparse_chunk<10>(acc, w, newc, oldl, DEPTH); break;
+    case 11: sparse_chunk<11>(acc, w, newc, oldl, DEPTH); break;
+    case 12: sparse_chunk<12>(acc, w, newc, oldl, DEPTH); break;
+    default: sparse_chunk<kG>(acc, w, newc, oldl, DEPTH); break;
+  }
+}
+
 __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
                 int b, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
-                const int32_t* __restrict__ lags, double* __restrict__ totals) {
+                const int32_t* __restrict__ lags, double* __restrict__ totals, double* __restrict__ I2,
+                double2* __restrict__ I1) {
   constexpr int G = kG;
   static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
   static_assert(kMaxTasks <= 16 && kMaxTasks % 4 == 0, "warp_task[16], whole sub-partition rounds");
   extern __shared__ __align__(128) unsigned char smraw[];
+  __shared__ int s_lags[kMaxTasks * kG];  // the lags of each sparse task, for the warm-up path
   const int gi = blockIdx.x % ngroups;  // groups of one pixel tile run side by side (they share L2 lines)
   const LagGroup& grp = groups[gi];
   const int tau_min = grp.tau_min, tau_max = grp.tau_max;
-  if ((int64_t)tau_min > t0 + b - 1) return;  // no frame pair of this group exists yet
+  // no frame pair of this group exists yet (the group that accumulates the I sums always runs)
+  if (grp.flags == 0 && (int64_t)tau_min > t0 + b - 1) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
   const int LEAD = lag_lead(tau_min, tau_max);
@@ -334,8 +388,10 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   const int tix = grp.warp_task[warp];
   if (tix < 0) return;
   const LagTask tk = tasks[grp.task0 + tix];
-  const bool dense = tk.kind == 0;
+  const bool dense = (tk.kind & 1) == 0;
+  const bool doI = (tk.kind & 2) != 0;  // this warp also accumulates I2 += |F'_s|^2, I1 += F'_s (group 0 only)
   const int cnt = tk.cnt;
+  f2x i2 = 0ull, i1 = 0ull;             // fp32 partials of the batch (<= 1024 terms, like acc)
   // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  Dense task: w = rotating window of the G most
   // recent OLD frames.  Sparse task: the low word of w[i] holds the OLD row of lag i at the block start.
   f2x acc[G], w[G];
@@ -350,13 +406,20 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     o0 = (offbase - tk.tau0) % DEPTH;
     tau_lo = tk.tau0;
     tau_hi = tk.tau0 + cnt - 1;
+  } else if (cnt == 0) {  // I sums only
+    tau_lo = tau_hi = 0;
   } else {
     tau_lo = lags[tk.l0];
     tau_hi = lags[tk.l0 + cnt - 1];
 #pragma unroll
     for (int i = 0; i < G; ++i)
-      if (i < cnt) w[i] = (f2x)(unsigned)((offbase - lags[tk.l0 + i]) % DEPTH);
+      if (i < cnt) {
+        const int lg = lags[tk.l0 + i];
+        w[i] = (f2x)(unsigned)((offbase - lg) % DEPTH);
+        if (lane == 0) s_lags[warp * G + i] = lg;  // read back by this warp only (warm-up path)
+      }
   }
+  __syncwarp();
   // batch-relative step from which every lag (j_all) / any lag (j_any) of the task has a frame pair
   const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi - t0));
   const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo - t0));
@@ -368,12 +431,51 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   for (int c = 0; c < nchunks; ++c) {
     mbar_wait(&full[st], ph);
     const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
+    const int j0 = c * kChunk;
+    if (j0 >= j_all && j0 + kChunk <= b) {
+      // ---- fast chunk: every pair of every step exists ----
+      if (doI) {
 #pragma unroll 1
-    for (int blk = 0; blk < kChunk / G; ++blk) {
+        for (int blk = 0; blk < kChunk / G; ++blk) {
+#pragma unroll
+          for (int u = 0; u < G; ++u) {
+            const f2x zn = newc[(size_t)(blk * G + u) * kRowF2];
+            i2 = fma2(zn, zn, i2);
+            i1 = add2(i1, zn);
+          }
+        }
+      }
+      if (dense) {
+        if (!wvalid) {  // (re)load the window: the G-1 OLD frames that precede the chunk's first one
+#pragma unroll
+          for (int q = 1; q < G; ++q) {
+            int r = o0 - q;
+            if (r < 0) r += DEPTH;
+            w[G - q] = oldl[(size_t)r * kRowF2];
+          }
+          wvalid = true;
+        }
+        dense_chunk_dispatch(cnt, acc, w, newc, oldl, o0, DEPTH);
+      } else {
+        sparse_chunk_dispatch(cnt, acc, w, newc, oldl, DEPTH);
+      }
+    } else {
+#pragma unroll 1
+    for (int blk = 0; blk < kChunk / G; ++blk) {  // warm-up and the batch's last, partial chunk: checked per block
       const int jb = c * kChunk + blk * G;  // batch-relative index of the block's first step
       const int ns = min(G, b - jb);        // steps of this block inside the batch
       if (ns <= 0) break;
       const f2x* nb = newc + (size_t)blk * G * kRowF2;
+      if (doI) {
+#pragma unroll
+        for (int u = 0; u < G; ++u) {
+          if (u < ns) {
+            const f2x zn = nb[(size_t)u * kRowF2];
+            i2 = fma2(zn, zn, i2);
+            i1 = add2(i1, zn);
+          }
+        }
+      }
       if (jb >= j_all) {
         // ---- every pair of the block exists ----
         if (dense) {
@@ -388,17 +490,14 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
             wvalid = true;
           }
           const f2x* ob = oldl + (size_t)o0 * kRowF2;
-          if (ns == G) {
-            dense_dispatch(cnt, acc, w, nb, ob);
-          } else {  // last block of the batch (surplus lags of a short task are discarded at the fold)
+          // all G lags of the window are updated; the surplus ones of a short task are discarded at the fold
 #pragma unroll
-            for (int u = 0; u < G; ++u) {
-              if (u < ns) {
-                const f2x zn = nb[(size_t)u * kRowF2];
-                w[u] = ob[(size_t)u * kRowF2];
+          for (int u = 0; u < G; ++u) {
+            if (u < ns) {
+              const f2x zn = nb[(size_t)u * kRowF2];
+              w[u] = ob[(size_t)u * kRowF2];
 #pragma unroll
-                for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
-              }
+              for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
             }
           }
         } else {
@@ -420,7 +519,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
                   if (r < 0) r += DEPTH;
                   upd2(acc[g], zn, oldl[(size_t)r * kRowF2]);
                 }
-              } else if (tj >= __ldg(&lags[tk.l0 + g])) {
+              } else if (tj >= s_lags[warp * G + g]) {
                 upd2(acc[g], zn, oldl[(size_t)((unsigned)w[g] + u) * kRowF2]);
               }
             }
@@ -435,11 +534,14 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
       } else {
 #pragma unroll
         for (int i = 0; i < G; ++i) {
-          unsigned o = (unsigned)w[i] + G;
-          if (o >= (unsigned)DEPTH) o -= DEPTH;
-          w[i] = (f2x)o;
+          if (i < cnt) {
+            unsigned o = (unsigned)w[i] + G;
+            if (o >= (unsigned)DEPTH) o -= DEPTH;
+            w[i] = (f2x)o;
+          }
         }
       }
+    }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[st]);
@@ -453,6 +555,13 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
 #pragma unroll
   for (int g = 0; g < G; ++g)
     if (g < cnt) atomicAdd(&totals[(int64_t)(tk.l0 + g) * P + p], (double)f2x_sum(acc[g]));
+  if (doI) {  // one writer per pixel and launch
+    I2[p] += (double)f2x_sum(i2);
+    double2 v = I1[p];
+    v.x += (double)__uint_as_float((unsigned)(i1 & 0xffffffffull));
+    v.y += (double)__uint_as_float((unsigned)(i1 >> 32));
+    I1[p] = v;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -468,7 +577,7 @@ struct Atom {
   int l0, cnt, kind;  // dense task, or one sparse lag (cnt = 1)
 };
 
-void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1,
+void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1, bool with_I,
                  std::vector<LagTask>& tasks, std::vector<LagGroup>& groups) {
   LagGroup g;
   g.task0 = (int)tasks.size();
@@ -514,14 +623,27 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
     a = e;
   }
   g.ntasks = (int)tasks.size() - g.task0;
+  g.flags = with_I ? 1 : 0;
+  auto cost = [&](int k) {
+    const LagTask& t = tasks[g.task0 + k];
+    return ((t.kind & 1) == 0 ? 4 * t.cnt + 2 : 5 * t.cnt + 1) + ((t.kind & 2) ? 5 : 0);
+  };
+  if (with_I) {  // this group also accumulates the I sums (kind bit 1): on a warp of its own if one is free,
+                 // else on its lightest task
+    if (g.ntasks < kMaxTasks) {
+      tasks.push_back(LagTask{0, 0, 0, 1 | 2});
+      g.ntasks += 1;
+    } else {
+      int best = 0;
+      for (int k = 1; k < g.ntasks; ++k)
+        if (cost(k) < cost(best)) best = k;
+      tasks[g.task0 + best].kind |= 2;
+    }
+  }
   // placement: heaviest task first onto the least loaded sub-partition that still has a free warp
   for (int w = 0; w < 16; ++w) g.warp_task[w] = -1;
   std::vector<int> order(g.ntasks);
   for (int k = 0; k < g.ntasks; ++k) order[k] = k;
-  auto cost = [&](int k) {
-    const LagTask& t = tasks[g.task0 + k];
-    return t.kind == 0 ? 4 * t.cnt + 2 : 5 * t.cnt + 1;
-  };
   std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost(x) > cost(y); });
   int load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0};
   for (int k : order) {
@@ -536,13 +658,10 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 }
 }  // namespace
 
-bool lag_plan(Ctx& c) {
+bool lag_plan(Ctx& c, int smem_sm) {
   const std::vector<int32_t>& L = c.lags;
-  int dev = 0, smem_sm = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
   // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
-  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024);
+  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
   budget = std::min(budget, (size_t)c.max_smem_optin);
   // atoms
   std::vector<Atom> atoms;
@@ -580,13 +699,24 @@ bool lag_plan(Ctx& c) {
     }
     return need <= kMaxTasks;
   };
+  std::vector<std::pair<size_t, size_t>> cuts;
   size_t a0 = 0;
   while (a0 < atoms.size()) {
     size_t a1 = a0 + 1;
     while (a1 < atoms.size() && fits(a0, a1 + 1)) ++a1;
-    close_group(L, atoms, a0, a1, c.tasks, c.groups);
+    cuts.push_back({a0, a1});
     a0 = a1;
   }
+  // the group with the fewest lags also accumulates the I sums of the batch
+  size_t gI = 0;
+  auto nl = [&](const std::pair<size_t, size_t>& r) {
+    int n = 0;
+    for (size_t a = r.first; a < r.second; ++a) n += atoms[a].cnt;
+    return n;
+  };
+  for (size_t k = 1; k < cuts.size(); ++k)
+    if (nl(cuts[k]) < nl(cuts[gI])) gI = k;
+  for (size_t k = 0; k < cuts.size(); ++k) close_group(L, atoms, cuts[k].first, cuts[k].second, k == gI, c.tasks, c.groups);
   // pipeline depth: as deep as the widest group's window leaves room for
   int stages = kMaxStages;
   for (const LagGroup& g : c.groups)
@@ -641,7 +771,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   const unsigned grid = (unsigned)((c.P / kTilePx) * ngroups);
   ProfScope ps(c, kKLag);
   k_lag_tiled<<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.lag_stages,
-                                                                      c.d_tasks, c.d_groups, c.d_lags, c.totals);
+                                                                      c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1);
   return 1;
 }
 
