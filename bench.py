@@ -285,7 +285,7 @@ def run_ours(args, cfg):
     inst_per_update = 4.0
     peak_tflops = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * (flop_per_update / inst_per_update) / 1e12
     ach_tflops = upd_per_launch * flop_per_update / lag_s_per_launch / 1e12
-    B = args.batch or 512
+    B = nfs.ring_capacity - cfg.lags[-1]  # the library's internal batch (frames)
     nb = (cfg.N + B - 1) // B
     # algorithmic HBM bytes of the accumulation: 8*U/B + 16*n_l/B per pixel and new frame
     lag_bytes = P * (8.0 * (cfg.N + nb * cfg.lags[-1]) + 16.0 * len(cfg.lags) * nb)

@@ -59,9 +59,12 @@ typedef enum nfs_status {
  *   n_qbins         number of |q| bins on [0, pi rad/px).
  *   cuda_stream     a cudaStream_t cast to void*, or NULL for a library-owned stream.  All device
  *                   work of this context is enqueued on it.
- * nfs_create_ex additionally fixes the internal batch size (0 = default 512): pushed frames are
+ * nfs_create_ex additionally fixes the internal batch size, 1..8192 (0 = default: 1024, halved down to
+ * 128 while the ring would take more than a third of the free device memory): pushed frames are
  * transformed into the ring at once, their frame pairs are accumulated whenever `batch` frames are
  * pending (and at every finalize/getter).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
+ * Whatever the batch, fp32 partial sums never span more than 520 frames before they are folded into
+ * the fp64 totals.
  */
 NFS_API int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream);
 NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,

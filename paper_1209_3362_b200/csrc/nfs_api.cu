@@ -213,7 +213,7 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
                   int batch_frames) {
   if (!out) return NFS_ERR_INVALID_ARG;
   *out = nullptr;
-  if (!lags || n_lags < 1 || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 1024)
+  if (!lags || n_lags < 1 || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
     return NFS_ERR_INVALID_ARG;
   if (!is_pow2(W) || !is_pow2(H) || W < 32 || H < 32 || W > 4096 || H > 4096) return NFS_ERR_INVALID_ARG;
   if (W != H) return NFS_ERR_UNSUPPORTED;
@@ -232,7 +232,7 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   c.n_qbins = n_qbins;
   c.lags.assign(lags, lags + n_lags);
   c.Lmax = lags[n_lags - 1];
-  c.B = batch_frames > 0 ? batch_frames : 512;
+  c.B = batch_frames > 0 ? batch_frames : 1024;
   c.R = c.Lmax + c.B;
 
   int dev = 0;
@@ -248,6 +248,11 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
     // memory plan: everything is sized before the first frame arrives
     size_t free_b = 0, total_b = 0;
     if (!NFS_CUDA(c, cudaMemGetInfo(&free_b, &total_b))) goto fail;
+    // default batch: 1024 frames, halved (down to 128) while the ring would take more than a third of the free memory
+    while (batch_frames == 0 && c.B > 128 && (double)c.R * (double)c.P * 8.0 > (double)free_b / 3.0) {
+      c.B /= 2;
+      c.R = c.Lmax + c.B;
+    }
     const double need = (double)c.P * ((double)c.R * 8 + 8 + (double)c.n_lags * 8 + 8 + 16 + 8) +
                         (double)fft_rowT_elems(c) * 8 +
                         (double)W * H * 4 + (double)(n_lags + 1) * n_qbins * 8 + (64 << 20);

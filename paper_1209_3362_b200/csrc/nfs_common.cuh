@@ -39,6 +39,8 @@ constexpr int kLagMinBlocks = NFS_LAG_MINB;  // CTAs per SM the kernel is compil
 constexpr int kChunk = kG * NFS_LAG_BPC;  // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
 constexpr int kMinStages = 2;
 constexpr int kMaxStages = NFS_LAG_MAXSTAGES;  // pipeline depth is chosen at create from the shared memory left
+constexpr int kFoldChunks = 20;  // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (520) steps
+constexpr int kSparseMax = 6;  // lags per lag-list task (one LDS.64 per pair update, exact-count code paths)
 constexpr int kDenseMin = 7;  // contiguous runs of >= kDenseMin lags use the register-window path
 
 struct LagTask {

@@ -232,37 +232,6 @@ __device__ __forceinline__ void dense_block(f2x (&acc)[kG], f2x (&w)[kG], const 
     for (int g = 0; g < CNT; ++g) upd2(acc[g], zn, w[(u - g + kG) % kG]);
   }
 }
-// ns steps of a sparse task with exactly CNT lags (checked path): one LDS.64 per pair update (no window to reuse).
-// The low word of w[i] holds the OLD row of lag i at the block start.
-template <int CNT>
-__device__ __forceinline__ void sparse_block(int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb, const f2x* oldl) {
-#pragma unroll 1
-  for (int u = 0; u < ns; ++u) {
-    const f2x zn = nb[(size_t)u * kRowF2];
-#pragma unroll
-    for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
-  }
-}
-__device__ __forceinline__ void sparse_dispatch(int cnt, int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb,
-                                                const f2x* oldl) {
-  switch (cnt) {
-    case 0: break;  // a task that only accumulates the I sums
-    case 1: sparse_block<1>(ns, acc, w, nb, oldl); break;
-    case 2: sparse_block<2>(ns, acc, w, nb, oldl); break;
-    case 3: sparse_block<3>(ns, acc, w, nb, oldl); break;
-    case 4: sparse_block<4>(ns, acc, w, nb, oldl); break;
-    case 5: sparse_block<5>(ns, acc, w, nb, oldl); break;
-    case 6: sparse_block<6>(ns, acc, w, nb, oldl); break;
-    case 7: sparse_block<7>(ns, acc, w, nb, oldl); break;
-    case 8: sparse_block<8>(ns, acc, w, nb, oldl); break;
-    case 9: sparse_block<9>(ns, acc, w, nb, oldl); break;
-    case 10: sparse_block<10>(ns, acc, w, nb, oldl); break;
-    case 11: sparse_block<11>(ns, acc, w, nb, oldl); break;
-    case 12: sparse_block<12>(ns, acc, w, nb, oldl); break;
-    default: sparse_block<kG>(ns, acc, w, nb, oldl); break;
-  }
-}
-
 // ---- whole chunks (kChunk = kChunk/kG blocks) in which every pair of every step exists: the common case ----
 template <int CNT>
 __device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int& o0,
@@ -314,14 +283,39 @@ __device__ __forceinline__ void sparse_chunk_dispatch(int cnt, f2x (&acc)[kG], f
     case 3: sparse_chunk<3>(acc, w, newc, oldl, DEPTH); break;
     case 4: sparse_chunk<4>(acc, w, newc, oldl, DEPTH); break;
     case 5: sparse_chunk<5>(acc, w, newc, oldl, DEPTH); break;
-    case 6: sparse_chunk<6>(acc, w, newc, oldl, DEPTH); break;
-    case 7: sparse_chunk<7>(acc, w, newc, oldl, DEPTH); break;
-    case 8: sparse_chunk<8>(acc, w, newc, oldl, DEPTH); break;
-    case 9: sparse_chunk<9>(acc, w, newc, oldl, DEPTH); break;
-    case 10: sparse_chunk<10>(acc, w, newc, oldl, DEPTH); break;
-    case 11: sparse_chunk<11>(acc, w, newc, oldl, DEPTH); break;
-    case 12: sparse_chunk<12>(acc, w, newc, oldl, DEPTH); break;
-    default: sparse_chunk<kG>(acc, w, newc, oldl, DEPTH); break;
+    default: sparse_chunk<kSparseMax>(acc, w, newc, oldl, DEPTH); break;  // the plan makes lag lists of <= kSparseMax
+  }
+}
+
+// One block of a lag-list task with exactly CNT lags in which some pairs do not exist (warm-up: the OLD
+// frame would precede the first frame; or the batch's ragged tail): pair (step u, lag i) is counted iff
+// u >= u0_i = lag_i - (frame number of step 0), and u < ns.
+template <int CNT>
+__device__ __forceinline__ void sparse_masked(int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb, const f2x* oldl,
+                                              const int* my_lags, int64_t frame0) {
+  int u0[CNT];
+#pragma unroll
+  for (int i = 0; i < CNT; ++i) u0[i] = (int)min((int64_t)99, max((int64_t)0, (int64_t)my_lags[i] - frame0));
+#pragma unroll
+  for (int u = 0; u < kG; ++u) {
+    if (u < ns) {
+      const f2x zn = nb[(size_t)u * kRowF2];
+#pragma unroll
+      for (int i = 0; i < CNT; ++i)
+        if (u >= u0[i]) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
+    }
+  }
+}
+__device__ __forceinline__ void sparse_masked_dispatch(int cnt, int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb,
+                                                       const f2x* oldl, const int* my_lags, int64_t frame0) {
+  switch (cnt) {
+    case 0: break;
+    case 1: sparse_masked<1>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 2: sparse_masked<2>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 3: sparse_masked<3>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 4: sparse_masked<4>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 5: sparse_masked<5>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    default: sparse_masked<kSparseMax>(ns, acc, w, nb, oldl, my_lags, frame0); break;
   }
 }
 
@@ -332,6 +326,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
                 double2* __restrict__ I1) {
   constexpr int G = kG;
   static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
+  static_assert(kSparseMax == 6, "sparse_chunk_dispatch lists cases 0..5 and the default");
   static_assert(kMaxTasks <= 16 && kMaxTasks % 4 == 0, "warp_task[16], whole sub-partition rounds");
   extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ int s_lags[kMaxTasks * kG];  // the lags of each sparse task, for the warm-up path
@@ -426,9 +421,13 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   const int t0c = (int)min((int64_t)1 << 30, t0);  // only compared against lags < 2^30 in the warm-up path
   const f2x* oldl = OLD + lane;
 
+  const int64_t p = p0 + lane;
   int st = 0;
   unsigned ph = 0;
-  for (int c = 0; c < nchunks; ++c) {
+  for (int cseg = 0; cseg < nchunks; cseg += kFoldChunks) {  // fp32 partial sums span one segment of chunks
+  const int cend = min(nchunks, cseg + kFoldChunks);
+#pragma unroll 1
+  for (int c = cseg; c < cend; ++c) {
     mbar_wait(&full[st], ph);
     const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
     const int j0 = c * kChunk;
@@ -476,57 +475,35 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
           }
         }
       }
-      if (jb >= j_all) {
-        // ---- every pair of the block exists ----
-        if (dense) {
-          if (!wvalid) {
-            // (re)load the window: the G-1 OLD frames that precede the block's first one
+      if (jb + ns <= j_any) {
+        wvalid = false;  // no pair of this task yet
+      } else if (dense) {
+        // ---- masked block: pair (step u, lag tau0 + g) exists iff u - g >= vbase, and u < ns.  All G lags of
+        // the window are updated; the surplus ones of a short task are discarded at the fold. ----
+        const int vbase = (int)max((int64_t)-64, (int64_t)tk.tau0 - t0 - jb);
+        if (!wvalid) {  // (re)load the window; rows of frames before the first one are masked below
 #pragma unroll
-            for (int q = 1; q < G; ++q) {
-              int r = o0 - q;
-              if (r < 0) r += DEPTH;
-              w[G - q] = oldl[(size_t)r * kRowF2];
-            }
-            wvalid = true;
+          for (int q = 1; q < G; ++q) {
+            int r = o0 - q;
+            if (r < 0) r += DEPTH;
+            w[G - q] = oldl[(size_t)r * kRowF2];
           }
-          const f2x* ob = oldl + (size_t)o0 * kRowF2;
-          // all G lags of the window are updated; the surplus ones of a short task are discarded at the fold
-#pragma unroll
-          for (int u = 0; u < G; ++u) {
-            if (u < ns) {
-              const f2x zn = nb[(size_t)u * kRowF2];
-              w[u] = ob[(size_t)u * kRowF2];
-#pragma unroll
-              for (int g = 0; g < G; ++g) upd2(acc[g], zn, w[(u - g + G) % G]);
-            }
-          }
-        } else {
-          sparse_dispatch(cnt, ns, acc, w, nb, oldl);
         }
-      } else if (jb + ns > j_any) {
-        // ---- warm-up: some lags reach back before the first frame; every pair checked, OLD read directly ----
-        wvalid = false;
-#pragma unroll 1
-        for (int u = 0; u < ns; ++u) {
-          const int tj = t0c + jb + u;
-          const f2x zn = nb[(size_t)u * kRowF2];
+        wvalid = ns == G;
+        const f2x* ob = oldl + (size_t)o0 * kRowF2;
 #pragma unroll
-          for (int g = 0; g < G; ++g) {
-            if (g < cnt) {
-              if (dense) {
-                if (tj >= tk.tau0 + g) {
-                  int r = o0 + u - g;
-                  if (r < 0) r += DEPTH;
-                  upd2(acc[g], zn, oldl[(size_t)r * kRowF2]);
-                }
-              } else if (tj >= s_lags[warp * G + g]) {
-                upd2(acc[g], zn, oldl[(size_t)((unsigned)w[g] + u) * kRowF2]);
-              }
-            }
+        for (int u = 0; u < G; ++u) {
+          if (u < ns) {
+            const f2x zn = nb[(size_t)u * kRowF2];
+            w[u] = ob[(size_t)u * kRowF2];
+#pragma unroll
+            for (int g = 0; g < G; ++g)
+              if (u - g >= vbase) upd2(acc[g], zn, w[(u - g + G) % G]);
           }
         }
       } else {
-        wvalid = false;  // no pair yet
+        // ---- masked block of a lag list: pair (step u, lag i) exists iff u >= u0_i, and u < ns ----
+        sparse_masked_dispatch(cnt, ns, acc, w, nb, oldl, &s_lags[warp * G], t0 + jb);
       }
       if (dense) {
         o0 += G;
@@ -547,21 +524,23 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     if (lane == 0) mbar_arrive(&empty[st]);
     if (++st == stages) st = 0, ph ^= 1u;
   }
-
-  // fold the batch's fp32 partial sums into the fp64 totals.  One reduction (RED.ADD.F64 in L2, nothing
-  // returns to the SM) per (lag, pixel) and launch, launches are stream ordered: the order of the
-  // additions is fixed and the result deterministic.
-  const int64_t p = p0 + lane;
+  // fold the fp32 partial sums (<= kFoldChunks * kChunk terms) into the fp64 totals: one reduction
+  // (RED.ADD.F64 in L2, nothing returns to the SM) per (lag, pixel).  Every address has one writer per
+  // launch, which folds in program order, and launches are stream ordered: the order of the additions
+  // is fixed and the result deterministic.
 #pragma unroll
-  for (int g = 0; g < G; ++g)
+  for (int g = 0; g < G; ++g) {
     if (g < cnt) atomicAdd(&totals[(int64_t)(tk.l0 + g) * P + p], (double)f2x_sum(acc[g]));
-  if (doI) {  // one writer per pixel and launch
-    I2[p] += (double)f2x_sum(i2);
-    double2 v = I1[p];
-    v.x += (double)__uint_as_float((unsigned)(i1 & 0xffffffffull));
-    v.y += (double)__uint_as_float((unsigned)(i1 >> 32));
-    I1[p] = v;
+    acc[g] = 0ull;
   }
+  if (doI) {
+    atomicAdd(&I2[p], (double)f2x_sum(i2));
+    atomicAdd(&I1[p].x, (double)__uint_as_float((unsigned)(i1 & 0xffffffffull)));
+    atomicAdd(&I1[p].y, (double)__uint_as_float((unsigned)(i1 >> 32)));
+    i2 = 0ull, i1 = 0ull;
+  }
+  }
+
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -590,7 +569,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   if (n_sparse > 0) {
     const int free_w = kMaxTasks - n_dense;
     const int want_w = std::max(1, std::min(free_w, 8 - std::min(n_dense, 7)));
-    s = std::min(kG, std::max(1, (n_sparse + want_w - 1) / want_w));
+    s = std::min(kSparseMax, std::max(1, (n_sparse + want_w - 1) / want_w));
     for (;; ++s) {  // stretches are cut separately: make sure the warps suffice
       int need = 0;
       size_t a = a0;
@@ -601,7 +580,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
         need += ((int)(e - a) + s - 1) / s;
         a = e;
       }
-      if (need <= free_w || s >= kG) break;
+      if (need <= free_w || s >= kSparseMax) break;
     }
   }
   size_t a = a0;
@@ -694,7 +673,7 @@ bool lag_plan(Ctx& c, int smem_sm) {
       if (atoms[a].kind == 0) { ++need; ++a; continue; }
       size_t e = a;
       while (e < a1 && atoms[e].kind == 1) ++e;
-      need += ((int)(e - a) + kG - 1) / kG;
+      need += ((int)(e - a) + kSparseMax - 1) / kSparseMax;
       a = e;
     }
     return need <= kMaxTasks;

@@ -125,6 +125,9 @@ SCALED = [
     (3, 2048, 12, [1, 2, 3, 5, 8], 512, 0, False),                         # config 3 frame size
     (3, 4096, 4, [1, 2], 512, 0, False),                                   # largest supported frame
     (4, 128, 400, list(range(1, 201)), 32, 64, False),                     # config 4 shape: long dense window
+    (1, 64, 1300, list(range(1, 21)) + [25, 31, 47, 90, 300, 560], 16, 1200, True),  # one batch of 1200 steps: the
+    # fp32 partial sums are folded into the fp64 totals twice inside the launch (every 520 steps), then a ragged batch
+    (1, 64, 700, list(range(1, 14)), 16, 0, True),                         # default batch (1024) holds the whole stack
 ]
 
 

@@ -11,7 +11,8 @@ import pytest
 
 from paper_1209_3362_b200 import binding, synth
 
-KG = 13          # lags per task (nfs_common.cuh: kG)
+KG = 13          # lags per register-window task (nfs_common.cuh: kG)
+KS = 6           # lags per lag-list task (kSparseMax)
 MAX_TASKS = 8    # consumer warps per CTA (kMaxTasks)
 SMEM_SM = 233472   # B200: shared memory per SM
 SMEM_OPTIN = 232448  # B200: opt-in maximum per CTA
@@ -36,7 +37,7 @@ def check_plan(lags, plan):
             assert ti not in seen_tasks
             seen_tasks.add(ti)
             t = tasks[ti]
-            assert 0 <= t["cnt"] <= KG
+            assert 0 <= t["cnt"] <= (KG if (t["kind"] & 1) == 0 else KS)
             has_I += (t["kind"] >> 1) & 1
             if t["cnt"] == 0:
                 assert t["kind"] == 3, "a task without lags only accumulates I"
