@@ -27,8 +27,8 @@ import numpy as np  # noqa: E402
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128
 # DRAM bytes (read + write) of one k_lag_tiled launch from the committed `ncu --set full` capture
-# (profiles/r01_summary.md), keyed by (workload, internal batch, frames); other workloads report null.
-NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {}
+# (profiles/r01_lag_ncu.md), keyed by (workload, internal batch, frames); other workloads report null.
+NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {("config2", 1024, 2000): 0.5 * (5.268e9 + 5.490e9)}  # profiles/r01_lag_ncu.md
 
 
 def load_peaks():
@@ -133,17 +133,24 @@ def workload_counts(cfg):
     return P, pairs
 
 
+def oracle_sample_frames(cfg):
+    """Frames of the bounded oracle sample: about 10-30 s of CPU work on the box's host cores."""
+    return min(cfg.N, 128 if cfg.W >= 2048 else (400 if cfg.W >= 1024 else (1000 if cfg.W >= 512 else cfg.N)))
+
+
 def oracle_sample(cfg, stack_np_fn):
     """The oracle, as it stands, on a bounded sample of the workload -> (frames/s, seconds, description, cores)."""
     from oracle import nfs_oracle as orc
 
-    n_s = min(cfg.N, 128 if cfg.W >= 1024 else (400 if cfg.W >= 512 else cfg.N))
+    n_s = oracle_sample_frames(cfg)
     fr = stack_np_fn(n_s)
     t = time.time()
     orc.structure_function(fr, cfg.lags, cfg.n_qbins)
     dt = time.time() - t
-    desc = "first %d frames of the %dx%d stack, all %d lags, full-plane fp64 oracle (oracle/nfs_oracle.c)" % (
-        n_s, cfg.W, cfg.H, len(cfg.lags))
+    pairs_s = sum(max(0, n_s - t) for t in cfg.lags)
+    pairs_full = sum(max(0, cfg.N - t) for t in cfg.lags)
+    desc = ("first %d frames of the %dx%d stack, all %d lags, full-plane fp64 oracle (oracle/nfs_oracle.c); the sample has "
+            "%.1f frame pairs per frame, the full stack %.1f" % (n_s, cfg.W, cfg.H, len(cfg.lags), pairs_s / n_s, pairs_full / cfg.N))
     return n_s / dt, dt, desc, orc.num_threads()
 
 
@@ -154,7 +161,7 @@ def run_reference(args, cfg):
     from paper_1209_3362_b200 import synth
 
     gen = synth.SynthStack(cfg, "cpu")
-    n_s = min(cfg.N, 128 if cfg.W >= 1024 else (400 if cfg.W >= 512 else cfg.N))
+    n_s = oracle_sample_frames(cfg)
     frames = gen.next_frames(n_s).numpy()
     times = []
     desc, cores = "", 0
@@ -294,7 +301,7 @@ def run_ours(args, cfg):
                     frac=ach_tflops / peak_tflops, traffic=traffic,
                     peak_source="derived (DESIGN.md §7.2): 148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) x 1.5 flop "
                                 "per lane-instruction (2 FADD + 2 FFMA = 6 flops per pair update)" % (peaks["sm_max_mhz"], peaks["source"]),
-                    traffic_source="ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_summary.md",
+                    traffic_source="ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the two batches), profiles/r01_lag_ncu.md",
                     pair_updates_per_s=upd_per_launch / lag_s_per_launch, ms_per_launch=lag_s_per_launch * 1e3,
                     ms_per_step=lag_ms / args.steps, launches_per_step=lag_n / args.steps,
                     hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9,

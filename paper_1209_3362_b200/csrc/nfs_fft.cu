@@ -112,6 +112,9 @@ __device__ __forceinline__ void dft(float2* u) {
 // ------------------------------------------------------------------------------------------------
 // plan constants for FFT length L
 // ------------------------------------------------------------------------------------------------
+#ifndef NFS_FFT_NT
+#define NFS_FFT_NT 128
+#endif
 #ifndef NFS_FFT_DR
 #define NFS_FFT_DR 0
 #define NFS_FFT_DC 0
@@ -122,7 +125,8 @@ constexpr int kMaxSlots = 40;
 template <int L>
 struct Plan {
   static constexpr int T = L / 32;                       // threads per FFT
-  static constexpr int NT = L <= 1024 ? 256 : 512;       // threads per CTA
+  static constexpr int NT = L <= 1024 ? (L >= 512 ? NFS_FFT_NT : 256) : 512;  // threads per CTA
+  static constexpr int minBlocks = L <= 1024 ? 512 / NT : 1;  // CTAs per SM the kernel is compiled for
   static constexpr int Fc = NT / T;                      // FFTs per CTA item
   static constexpr bool two = L > 1024;                  // two-level plan
   static constexpr int Mi = two ? L / 1024 : T;          // lanes per (inner) FFT
@@ -135,14 +139,14 @@ struct Plan {
   static constexpr int FcRow = Fc < rowFfts ? Fc : rowFfts;
   static constexpr int NR = (rowFfts + Fc - 1) / Fc;     // row items per frame
   static constexpr int NC = (n + 1 + Fc - 1) / Fc;       // column items per frame
-  static constexpr int NS = L >= 256 ? 8 : 1;            // sum items per frame
+  static constexpr int NS = L >= 256 ? 8 * 256 / NT : 1;  // sum items per frame
   static constexpr int perStep = NS + NR + NC;
   static constexpr size_t smem = sizeof(float2) * ((size_t)Fc * Sf + 2 * Fc);
   // Queue distances, in steps (one step = the items of one frame).  About 2 * (resident CTAs) items are
   // claimed at any time (each CTA holds the item it runs and the next one), i.e. `win` steps; an item
   // should find its dependencies finished, so they are queued more than `win` steps earlier.
   // The write-after-read dependency on an intermediate slot needs Dc < slots (it must precede in the queue).
-  static constexpr int claimed = (L <= 1024 ? 4 : 2) * 148;
+  static constexpr int claimed = 2 * minBlocks * 148;
   static constexpr int win_ = (claimed + perStep - 1) / perStep;
   static constexpr int win = win_ < 16 ? win_ : 16;
   static constexpr int Dr = NFS_FFT_DR ? NFS_FFT_DR : win + 1;                   // sum items -> row items
@@ -421,7 +425,7 @@ __device__ __forceinline__ void chunk_stage(const Chunk& ck, int mode, float hi,
 // the persistent kernel
 // ------------------------------------------------------------------------------------------------
 template <int L>
-__global__ void __launch_bounds__(Plan<L>::NT, (L <= 1024 ? 2 : 1)) k_fft(const FftJob j) {
+__global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const FftJob j) {
   using P = Plan<L>;
   constexpr int W = L, H = L, n = P::n;
   extern __shared__ __align__(16) float2 sm[];
