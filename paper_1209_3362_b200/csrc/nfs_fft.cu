@@ -29,8 +29,33 @@ namespace nfs {
 // ------------------------------------------------------------------------------------------------
 // complex helpers and register DFTs
 // ------------------------------------------------------------------------------------------------
+#ifndef NFS_FFT_PACKED
+#define NFS_FFT_PACKED 1
+#endif
+#if NFS_FFT_PACKED
+// complex add / subtract as one packed instruction (SASS FADD2): one issue slot instead of two
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+  unsigned long long ua, ub, ur;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+  asm("add.f32x2 %0, %1, %2;" : "=l"(ur) : "l"(ua), "l"(ub));
+  float2 r;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(ur));
+  return r;
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+  unsigned long long ua, ub, ur;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+  asm("sub.f32x2 %0, %1, %2;" : "=l"(ur) : "l"(ua), "l"(ub));
+  float2 r;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(ur));
+  return r;
+}
+#else
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#endif
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
@@ -107,6 +132,61 @@ __device__ __forceinline__ void dft(float2* u) {
 #pragma unroll
     for (int k = 0; k < N; ++k) u[k] = t[k];
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// L2 eviction hints (NFS_FFT_L2HINTS): the uint16 frame is read by the sum items and again, a few queue
+// steps later, by the row items; the row-pass intermediate is written and re-read through L2; the ring
+// slot is written once and not read again by this kernel.
+// ------------------------------------------------------------------------------------------------
+#ifndef NFS_FFT_L2HINTS
+#define NFS_FFT_L2HINTS 1
+#endif
+__device__ __forceinline__ unsigned long long pol_evict_last() {
+  unsigned long long p;
+  asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ unsigned long long pol_evict_first() {
+  unsigned long long p;
+  asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint4 ld_u4_hint(const uint4* p, unsigned long long pol) {
+#if NFS_FFT_L2HINTS
+  uint4 v;
+  asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+               : "l"(p), "l"(pol));
+  return v;
+#else
+  return __ldg(p);
+#endif
+}
+__device__ __forceinline__ float2 ld_f2_cg_hint(const float2* p, unsigned long long pol) {
+#if NFS_FFT_L2HINTS
+  float2 v;
+  asm volatile("ld.global.cg.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol) : "memory");
+  return v;
+#else
+  return __ldcg(p);
+#endif
+}
+__device__ __forceinline__ void st_f2_hint(float2* p, float2 v, unsigned long long pol) {
+#if NFS_FFT_L2HINTS
+  asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+#else
+  *p = v;
+#endif
+}
+__device__ __forceinline__ void st_f4_hint(float4* p, float4 v, unsigned long long pol) {
+#if NFS_FFT_L2HINTS
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w),
+               "l"(pol)
+               : "memory");
+#else
+  *p = v;
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -364,7 +444,7 @@ __device__ __forceinline__ void item_sum(const FftJob& j, int f, int part, unsig
       for (int q = 0; q < 4; ++q) {
         const int64_t i = i0 + (int64_t)q * P::NT + threadIdx.x;
         if (i < per) {
-          const uint4 v = __ldg(&src[i]);
+          const uint4 v = ld_u4_hint(&src[i], pol_evict_last());
           a32 += (v.x & 0xffffu) + (v.x >> 16) + (v.y & 0xffffu) + (v.y >> 16) + (v.z & 0xffffu) + (v.z >> 16) +
                  (v.w & 0xffffu) + (v.w >> 16);
         }
@@ -395,8 +475,8 @@ __device__ __forceinline__ void chunk_load(Chunk& ck, const FftJob& j, const uin
   ck.b0 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8));
   ck.b1 = __ldg(reinterpret_cast<const float4*>(j.ref + rb + c * 8 + 4));
   if (j.mode == 0) {
-    ck.pa = __ldg(reinterpret_cast<const uint4*>(fr + ra + c * 8));
-    ck.pb = __ldg(reinterpret_cast<const uint4*>(fr + rb + c * 8));
+    ck.pa = ld_u4_hint(reinterpret_cast<const uint4*>(fr + ra + c * 8), pol_evict_first());
+    ck.pb = ld_u4_hint(reinterpret_cast<const uint4*>(fr + rb + c * 8), pol_evict_first());
   }
 }
 // convert + normalise + subtract the reference, stage z[j] = d_a[j] + i d_b[j]
@@ -521,7 +601,7 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
       __syncthreads();
       const float2* src = rowT + (size_t)q * H;
 #pragma unroll
-      for (int t = 0; t < 32; ++t) u[t] = __ldcg(&src[t * P::T + tau]);
+      for (int t = 0; t < 32; ++t) u[t] = ld_f2_cg_hint(&src[t * P::T + tau], pol_evict_first());
     }
 
     // ---------------- the FFT itself (one call site: the code is large) ----------------
@@ -562,7 +642,7 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
         const int kxl = e & 1, ft = (e >> 1) % FcR, kx = 2 * (e / (2 * FcR)) + kxl;
         const float2* b = sm + (size_t)ft * P::Sf;
         const float2 A = b[kx], B = b[kx ? L - kx : n];
-        *reinterpret_cast<float4*>(rowT + (size_t)kx * H + y0 + 2 * ft) = make_float4(A.x, A.y, B.x, B.y);
+        st_f4_hint(reinterpret_cast<float4*>(rowT + (size_t)kx * H + y0 + 2 * ft), make_float4(A.x, A.y, B.x, B.y), pol_evict_last());
       }
       if (tid < FcR) {
         *reinterpret_cast<float4*>(rowT + (size_t)n * H + y0 + 2 * tid) =
@@ -575,7 +655,7 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
         float2* dst = j.dst + (size_t)slot * Pn + (size_t)q * H;
         const float sc = j.scale;
 #pragma unroll
-        for (int r = 0; r < 32; ++r) dst[out_index<L>(tau, r)] = make_float2(u[r].x * sc, u[r].y * sc);
+        for (int r = 0; r < 32; ++r) st_f2_hint(&dst[out_index<L>(tau, r)], make_float2(u[r].x * sc, u[r].y * sc), pol_evict_first());
       }
       signal_count(&j.cnt[1 + 2 * j.nf + f]);
     }

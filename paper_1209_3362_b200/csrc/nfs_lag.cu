@@ -640,7 +640,10 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 bool lag_plan(Ctx& c, int smem_sm) {
   const std::vector<int32_t>& L = c.lags;
   // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
-  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
+  #ifndef NFS_LAG_SMEM_DIV
+#define NFS_LAG_SMEM_DIV kLagMinBlocks
+#endif
+  size_t budget = (size_t)std::max(0, smem_sm / NFS_LAG_SMEM_DIV - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
   budget = std::min(budget, (size_t)c.max_smem_optin);
   // atoms
   std::vector<Atom> atoms;
