@@ -142,6 +142,39 @@ def test_scaled_configs(binding, oracle, idx, W, N, lags, n_b, batch, per_pixel)
 
 
 # --------------------------------------------------------------------------------------------------------------
+# randomised lag lists, batch sizes and push splits: every mix of lag runs and isolated lags the plan can produce
+# --------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(10))
+def test_random_lag_lists_batches_and_splits(binding, oracle, seed):
+    rng = np.random.default_rng(1000 + seed)
+    W = int(rng.choice([32, 64]))
+    N = int(rng.integers(3, 260))
+    n_l = int(rng.integers(1, 60))
+    top = int(rng.choice([n_l, 2 * n_l, 6 * n_l, 400]))
+    lags = sorted(int(v) for v in rng.choice(np.arange(1, max(top, n_l) + 1), size=n_l, replace=False))
+    batch = int(rng.choice([0, 1, 13, 26, 27, 64, 300]))
+    split = int(rng.choice([0, 1, 7, 50, 97]))
+    n_b = int(rng.choice([8, 16, 33]))
+    cfg = synth.config(1, W=W, N=N, lags=lags, n_qbins=n_b)
+    cfg.seed = 500 + seed
+    st = synth.make_stack(cfg, "cuda")
+    ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=True)
+    g = gpu_run(binding, st, lags, n_b, batch=batch, split=split or None)
+    check_against_oracle(g, ref, W)
+
+
+def test_many_folds_in_one_launch(binding, oracle):
+    """One launch of 4000 steps: the fp32 partial sums are folded into the fp64 totals seven times inside it."""
+    lags = [1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 15, 100, 1000, 3999, 4000]
+    cfg = synth.config(0, W=32, N=4000, lags=lags, n_qbins=8)
+    st = synth.make_stack(cfg, "cuda")
+    ref = oracle.structure_function(st.cpu().numpy(), lags, 8, want_2d=True)
+    g = gpu_run(binding, st, lags, 8, batch=4096)
+    assert g["n_pairs"].tolist() == [3999, 3998, 3997, 3996, 3995, 3994, 3993, 3992, 3991, 3990, 3985, 3900, 3000, 1, 0]
+    check_against_oracle(g, ref, 32)
+
+
+# --------------------------------------------------------------------------------------------------------------
 # edge cases (SURVEY.md §7 H5)
 # --------------------------------------------------------------------------------------------------------------
 def test_lags_beyond_N_and_single_frame(binding, oracle):
