@@ -117,9 +117,11 @@ NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
 NFS_API int nfs_set_profiling(nfs_ctx* ctx, int enable);
 NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
 
-/* Lag-accumulation kernel variant: 0 = tiled shared-memory kernel (default), 1 = plain per-pixel
- * kernel reading the ring through L1/L2 (kept as an in-library cross-check; same results up to
- * fp32 summation order).  Not a backend switch: both are CUDA kernels of this library. */
+/* Lag-accumulation kernel variant: 0 = tiled shared-memory kernel, launch shape chosen per batch (default),
+ * 1 = plain per-pixel kernel reading the ring through L1/L2 (kept as an in-library cross-check; same results
+ * up to fp32 summation order), 2 = tiled kernel, always one CTA per (pixel tile, lag group), 3 = tiled kernel,
+ * always persistent CTAs claiming pixel tiles (2 and 3 give bit-identical results to 0: they only change which
+ * CTA handles which tile).  Not a backend switch: all are CUDA kernels of this library. */
 NFS_API int nfs_set_lag_kernel(nfs_ctx* ctx, int variant);
 
 /* Host-only introspection of the lag plan of step S5 (which lags are accumulated
@@ -127,8 +129,9 @@ NFS_API int nfs_set_lag_kernel(nfs_ctx* ctx, int variant);
  * nfs_create would build for `lags` (HOST, strictly increasing, >= 1) on a device with `smem_per_sm`
  * bytes of shared memory per SM and `smem_optin` bytes per CTA, and writes it to out (HOST, cap int32):
  *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA]
- *   per group (21 values): first task, number of tasks, tau_min, tau_max, flags (bit 0: one task of the
- *     group accumulates the I sums), then for consumer warps 0..15 the task (relative) it runs or -1
+ *   per group (23 values): first task, number of tasks, tau_min, tau_max, flags (bit 0: one task of the
+ *     group accumulates the I sums), then for consumer warps 0..15 the task (relative) it runs or -1, then the
+ *     first persistent CTA of the group and their number (planned here for 2 x 148 resident CTAs)
  *   per task (4 values): smallest lag, number of lags, index of its first lag in `lags`, kind (bit 0:
  *     0 = run of consecutive lags on the register-window path, 1 = lag list; bit 1: also accumulates I)
  * Returns the number of int32 written (> 0), or NFS_ERR_INVALID_ARG (bad list, cap too small, a single

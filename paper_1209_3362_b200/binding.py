@@ -110,7 +110,7 @@ def nfs_finalize(handle, n_lags, n_qbins):
 def nfs_plan_lags(lags, smem_per_sm=233472, smem_optin=232448):
     """Host-only lag plan (no CUDA call): dict(stages, smem, groups=[...], tasks=[...]); see include/nfs.h."""
     lags = np.ascontiguousarray(lags, dtype=np.int32)
-    cap = 4 + 25 * (len(lags) + 1)
+    cap = 4 + 27 * (len(lags) + 1)
     out = np.zeros(cap, dtype=np.int32)
     n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(smem_per_sm), int(smem_optin), _dp(out, C.c_int32), cap)
     if n < 0:
@@ -119,10 +119,10 @@ def nfs_plan_lags(lags, smem_per_sm=233472, smem_optin=232448):
     o = 4
     groups, tasks = [], []
     for _ in range(ng):
-        g = out[o:o + 21]
+        g = out[o:o + 23]
         groups.append(dict(task0=int(g[0]), ntasks=int(g[1]), tau_min=int(g[2]), tau_max=int(g[3]), flags=int(g[4]),
-                           warp_task=[int(v) for v in g[5:21]]))
-        o += 21
+                           warp_task=[int(v) for v in g[5:21]], cta0=int(g[21]), nctas=int(g[22])))
+        o += 23
     for _ in range(nt):
         t = out[o:o + 4]
         tasks.append(dict(tau0=int(t[0]), cnt=int(t[1]), l0=int(t[2]), kind=int(t[3])))

@@ -133,15 +133,17 @@ bool build_tables(Ctx& c) {
 
   // lag plan (nfs_lag.cu): tasks per consumer warp, groups per CTA, pipeline depth
   const std::vector<int32_t>& L = c.lags;
-  int dev = 0, smem_sm = 0;
+  int dev = 0, smem_sm = 0, n_sm = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
-  if (!lag_plan(c, smem_sm)) {
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (!lag_plan(c, smem_sm, kLagMinBlocks * std::max(1, n_sm), (int)(c.P / kTilePx))) {
     c.status = NFS_ERR_INVALID_ARG;
     return false;
   }
   if (!dev_alloc(c, &c.d_tasks, c.tasks.size())) return false;
   if (!dev_alloc(c, &c.d_groups, c.groups.size())) return false;
+  if (!dev_alloc(c, &c.d_claim, c.groups.size())) return false;
   if (!dev_alloc(c, &c.d_lags, (size_t)c.n_lags)) return false;
   if (!NFS_CUDA(c, cudaMemcpy(c.d_tasks, c.tasks.data(), sizeof(LagTask) * c.tasks.size(), cudaMemcpyHostToDevice)))
     return false;
@@ -153,7 +155,7 @@ bool build_tables(Ctx& c) {
 
 void free_all(Ctx& c) {
   void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.I2,      c.I1,      c.sums,     c.tw,     c.tw_out,
-                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags, c.d_tasks, c.d_groups, c.fft_cnt};
+                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags, c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
@@ -388,8 +390,9 @@ int64_t nfs_device_bytes(const nfs_ctx* h) { return h ? h->c.dev_bytes : 0; }
 int64_t nfs_num_launches(const nfs_ctx* h) { return h ? h->c.n_launches : 0; }
 
 int nfs_set_lag_kernel(nfs_ctx* h, int variant) {
-  if (!h || variant < 0 || variant > 1) return NFS_ERR_INVALID_ARG;
-  h->c.lag_variant = variant;
+  if (!h || variant < 0 || variant > 3) return NFS_ERR_INVALID_ARG;
+  h->c.lag_variant = variant == 1 ? 1 : 0;
+  h->c.lag_persistent = variant == 2 ? 0 : (variant == 3 ? 1 : -1);
   return NFS_OK;
 }
 
@@ -402,8 +405,8 @@ int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_opt
   c.n_lags = n_lags;
   c.Lmax = lags[n_lags - 1];
   c.max_smem_optin = smem_optin;
-  if (!lag_plan(c, smem_per_sm)) return NFS_ERR_INVALID_ARG;
-  const size_t need = 4 + c.groups.size() * 21 + c.tasks.size() * 4;
+  if (!lag_plan(c, smem_per_sm, kLagMinBlocks * 148, 1 << 20)) return NFS_ERR_INVALID_ARG;
+  const size_t need = 4 + c.groups.size() * 23 + c.tasks.size() * 4;
   if (need > (size_t)cap) return NFS_ERR_INVALID_ARG;
   int32_t* o = out;
   *o++ = (int32_t)c.groups.size();
@@ -413,6 +416,7 @@ int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_opt
   for (const LagGroup& g : c.groups) {
     *o++ = g.task0, *o++ = g.ntasks, *o++ = g.tau_min, *o++ = g.tau_max, *o++ = g.flags;
     for (int w = 0; w < 16; ++w) *o++ = g.warp_task[w];
+    *o++ = g.cta0, *o++ = g.nctas;
   }
   for (const LagTask& t : c.tasks) *o++ = t.tau0, *o++ = t.cnt, *o++ = t.l0, *o++ = t.kind;
   return (int)need;

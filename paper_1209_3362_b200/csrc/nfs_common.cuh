@@ -53,6 +53,7 @@ struct LagGroup {
   int task0, ntasks;
   int tau_min, tau_max;
   int flags;  // bit 0: one task of this group accumulates the I sums (the group runs for every batch)
+  int cta0, nctas;  // persistent CTAs [cta0, cta0 + nctas) of the launch work on this group (share ~ its work)
   signed char warp_task[16];  // task (relative to task0) run by consumer warp w, or -1: placed so that the
                               // four SM sub-partitions (warp id mod 4) carry equal work
 };
@@ -101,7 +102,10 @@ struct Ctx {
   int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
   LagTask* d_tasks = nullptr;
   LagGroup* d_groups = nullptr;
+  int* d_claim = nullptr;        // [n_groups] next pixel tile of each group, zeroed before every k_lag_tiled launch
   int lag_stages = kMinStages;   // pipeline stages of k_lag_tiled (chosen by lag_plan)
+  int lag_grid = 0;              // persistent CTAs of k_lag_tiled (sum of the groups' shares)
+  int lag_persistent = -1;       // -1: chosen per launch (launch_lag_tiled); 0 / 1: forced (nfs_set_lag_kernel 2 / 3)
   size_t lag_smem = 0;           // dynamic shared memory of k_lag_tiled
   std::vector<LagTask> tasks;
   std::vector<LagGroup> groups;
@@ -148,7 +152,7 @@ int launch_lag_simple(Ctx& c, int64_t t0, int b);
 int launch_lag_tiled(Ctx& c, int64_t t0, int b);
 // host only (no CUDA call): tasks, groups, pipeline depth from the lag list, the shared memory per SM and
 // c.max_smem_optin; false if a lag group cannot fit shared memory
-bool lag_plan(Ctx& c, int smem_per_sm);
+bool lag_plan(Ctx& c, int smem_per_sm, int cta_slots, int ntiles);
 bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)

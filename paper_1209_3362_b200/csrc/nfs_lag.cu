@@ -319,24 +319,33 @@ __device__ __forceinline__ void sparse_masked_dispatch(int cnt, int ns, f2x (&ac
   }
 }
 
+template <bool PERS>
 __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
                 int b, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
                 const int32_t* __restrict__ lags, double* __restrict__ totals, double* __restrict__ I2,
-                double2* __restrict__ I1) {
+                double2* __restrict__ I1, int ntiles, int* __restrict__ claim) {
   constexpr int G = kG;
   static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
   static_assert(kSparseMax == 6, "sparse_chunk_dispatch lists cases 0..5 and the default");
   static_assert(kMaxTasks <= 16 && kMaxTasks % 4 == 0, "warp_task[16], whole sub-partition rounds");
   extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ int s_lags[kMaxTasks * kG];  // the lags of each sparse task, for the warm-up path
-  const int gi = blockIdx.x % ngroups;  // groups of one pixel tile run side by side (they share L2 lines)
+  __shared__ int s_tile[kMaxStages];      // tile of the item whose first step uses this stage, or -1: no more work
+  // persistent launch: group gi owns CTAs [cta0, cta0 + nctas), which claim the group's pixel tiles one after
+  // the other (claim[gi], zeroed before the launch) and run through them without draining the shared-memory
+  // pipeline.  One-tile launch: CTA = (tile, group), the groups of a tile side by side (they share L2 lines).
+  int gi = 0;
+  if constexpr (PERS) {
+    while (gi + 1 < ngroups && (int)blockIdx.x >= groups[gi].cta0 + groups[gi].nctas) ++gi;
+  } else {
+    gi = blockIdx.x % ngroups;
+  }
   const LagGroup& grp = groups[gi];
   const int tau_min = grp.tau_min, tau_max = grp.tau_max;
   // no frame pair of this group exists yet (the group that accumulates the I sums always runs)
   if (grp.flags == 0 && (int64_t)tau_min > t0 + b - 1) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
   const int LEAD = lag_lead(tau_min, tau_max);
   const int NSLOT = LEAD + stages;
   const int DEPTH = NSLOT * kChunk;
@@ -346,6 +355,11 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   f2x* OLD = reinterpret_cast<f2x*>(smraw + 128);           // [(NSLOT + 1) * kChunk][32]
   f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * kRowF2;   // [stages][kChunk][32]
   const int nchunks = (b + kChunk - 1) / kChunk;
+  // One item (pixel tile) = LEAD prologue steps that only bring OLD chunks (the window), then nchunks steps that
+  // bring OLD chunk j and NEW chunk j - LEAD and are consumed.  Steps are numbered through all items of the
+  // CTA: step v uses pipeline stage v % stages and puts its OLD chunk into ring slot v % NSLOT, which held the
+  // OLD chunk of step v - NSLOT = v - LEAD - stages, last read by the consumers at step v - stages.
+  const int V = nchunks + LEAD;
 
   if (tid == 0) {
     const unsigned nt = (unsigned)grp.ntasks;
@@ -359,22 +373,55 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
 
   if (warp == kMaxTasks) {
     // ------------------------------- producer -------------------------------
-    const int64_t E0 = t0 - tau_min - (int64_t)LEAD * kChunk;  // frame held by OLD row 0
-    int st = 0;
+    const int64_t E0 = t0 - tau_min - (int64_t)LEAD * kChunk;  // frame held by row 0 of an item's OLD chunk 0
+    int st = 0, slot = 0;
     unsigned ph = 0;  // parity of this stage's current use
-    for (int c = 0; c < nchunks; ++c) {
-      if (c >= stages) mbar_wait_relaxed(&empty[st], ph ^ 1u);
-      unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
-                                  nullptr, &full[st], lane);
-      for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
-        const int slot = m % NSLOT;
-        f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
-        f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
-        bytes += load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)m * kChunk, dst, dup, &full[st], lane);
+    if constexpr (PERS) {
+      for (;;) {
+        int tile = 0;
+        if (lane == 0) tile = atomicAdd(&claim[gi], 1);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        if (tile >= ntiles) {  // tell the consumers; nothing is loaded for this step
+          mbar_wait_relaxed(&empty[st], ph ^ 1u);
+          if (lane == 0) {
+            s_tile[st] = -1;
+            mbar_arrive(&full[st]);
+          }
+          break;
+        }
+        const int64_t p0 = (int64_t)tile * kTilePx;
+        for (int j = 0; j < V; ++j) {
+          mbar_wait_relaxed(&empty[st], ph ^ 1u);  // passes at once on the first use of a stage
+          if (j == 0 && lane == 0) s_tile[st] = tile;  // ordered before the consumers' read by the arrive below
+          f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
+          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
+          unsigned bytes = load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)j * kChunk, dst, dup, &full[st], lane);
+          if (j >= LEAD)
+            bytes += load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)(j - LEAD) * kChunk,
+                                NEW + (size_t)st * kChunk * kRowF2, nullptr, &full[st], lane);
+          bytes = __reduce_add_sync(0xffffffffu, bytes);
+          if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
+          if (++st == stages) st = 0, ph ^= 1u;
+          if (++slot == NSLOT) slot = 0;
+        }
       }
-      bytes = __reduce_add_sync(0xffffffffu, bytes);
-      if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
-      if (++st == stages) st = 0, ph ^= 1u;
+    } else {
+      // one pixel tile: the whole window (OLD chunks 0..LEAD) comes with the first chunk, no prologue steps
+      const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
+      for (int c = 0; c < nchunks; ++c) {
+        if (c >= stages) mbar_wait_relaxed(&empty[st], ph ^ 1u);
+        unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
+                                    nullptr, &full[st], lane);
+        for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
+          f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
+          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
+          bytes += load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)m * kChunk, dst, dup, &full[st], lane);
+          if (++slot == NSLOT) slot = 0;
+        }
+        bytes = __reduce_add_sync(0xffffffffu, bytes);
+        if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
+        if (++st == stages) st = 0, ph ^= 1u;
+      }
     }
     return;
   }
@@ -398,7 +445,6 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   bool wvalid = false;  // dense: the register window matches the current block start
   int tau_lo, tau_hi;   // smallest / largest lag of the task
   if (dense) {
-    o0 = (offbase - tk.tau0) % DEPTH;
     tau_lo = tk.tau0;
     tau_hi = tk.tau0 + cnt - 1;
   } else if (cnt == 0) {  // I sums only
@@ -408,11 +454,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     tau_hi = lags[tk.l0 + cnt - 1];
 #pragma unroll
     for (int i = 0; i < G; ++i)
-      if (i < cnt) {
-        const int lg = lags[tk.l0 + i];
-        w[i] = (f2x)(unsigned)((offbase - lg) % DEPTH);
-        if (lane == 0) s_lags[warp * G + i] = lg;  // read back by this warp only (warm-up path)
-      }
+      if (i < cnt && lane == 0) s_lags[warp * G + i] = lags[tk.l0 + i];  // read back by this warp only
   }
   __syncwarp();
   // batch-relative step from which every lag (j_all) / any lag (j_any) of the task has a frame pair
@@ -421,14 +463,44 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   const int t0c = (int)min((int64_t)1 << 30, t0);  // only compared against lags < 2^30 in the warm-up path
   const f2x* oldl = OLD + lane;
 
-  const int64_t p = p0 + lane;
-  int st = 0;
+  int st = 0, slot0 = 0;  // slot0: ring slot of the current item's OLD chunk 0
   unsigned ph = 0;
+  for (int item = 0; PERS || item == 0; ++item) {
+  int tile = (int)(blockIdx.x / ngroups);
+  bool waited = false;  // PERS: the barrier of the item's first step has been passed already
+  if constexpr (PERS) {
+    mbar_wait(&full[st], ph);  // first step of the next item
+    tile = s_tile[st];
+    if (tile < 0) break;
+    waited = true;
+  }
+  const int64_t p = (int64_t)tile * kTilePx + lane;
+  // per-item state: OLD rows of the item's first step
+  const int base_row = slot0 * kChunk + offbase;
+  wvalid = false;
+  if (dense) {
+    o0 = (base_row - tk.tau0) % DEPTH;
+  } else {
+#pragma unroll
+    for (int i = 0; i < G; ++i)
+      if (i < cnt) w[i] = (f2x)(unsigned)((base_row - s_lags[warp * G + i]) % DEPTH);
+  }
+  slot0 = (slot0 + V) % NSLOT;
+  // prologue steps: the window is being filled, nothing to consume
+#pragma unroll 1
+  for (int j = 0; PERS && j < LEAD; ++j) {
+    if (!waited) mbar_wait(&full[st], ph);
+    waited = false;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[st]);
+    if (++st == stages) st = 0, ph ^= 1u;
+  }
   for (int cseg = 0; cseg < nchunks; cseg += kFoldChunks) {  // fp32 partial sums span one segment of chunks
   const int cend = min(nchunks, cseg + kFoldChunks);
 #pragma unroll 1
   for (int c = cseg; c < cend; ++c) {
-    mbar_wait(&full[st], ph);
+    if (!waited) mbar_wait(&full[st], ph);
+    waited = false;
     const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
     const int j0 = c * kChunk;
     if (j0 >= j_all && j0 + kChunk <= b) {
@@ -540,7 +612,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     i2 = 0ull, i1 = 0ull;
   }
   }
-
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -637,7 +709,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 }
 }  // namespace
 
-bool lag_plan(Ctx& c, int smem_sm) {
+bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
   const std::vector<int32_t>& L = c.lags;
   // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
   #ifndef NFS_LAG_SMEM_DIV
@@ -708,6 +780,45 @@ bool lag_plan(Ctx& c, int smem_sm) {
   if (smem > (size_t)c.max_smem_optin) return false;  // a single task's own lag span does not fit
   c.lag_stages = stages;
   c.lag_smem = smem;
+  // persistent CTAs: the cta_slots resident CTAs of the device are shared out in proportion to the groups' work
+  // per pixel tile (FP32 work of the tasks + a constant for streaming the window), at least one CTA each
+  {
+    const int ng = (int)c.groups.size();
+    std::vector<double> wgt(ng);
+    double wsum = 0.0;
+    for (int g = 0; g < ng; ++g) {
+      double wg = 40.0;
+      for (int k = 0; k < c.groups[g].ntasks; ++k) {
+        const LagTask& t = c.tasks[c.groups[g].task0 + k];
+        wg += ((t.kind & 1) == 0 ? 4.0 * t.cnt + 2.0 : 5.0 * t.cnt + 1.0) + ((t.kind & 2) ? 5.0 : 0.0);
+      }
+      wgt[g] = wg;
+      wsum += wg;
+    }
+    const int slots = std::max(cta_slots, ng);
+    int used = 0;
+    for (int g = 0; g < ng; ++g) {
+      int n = (int)(slots * wgt[g] / wsum);
+      n = std::max(1, std::min(n, std::max(1, ntiles)));
+      c.groups[g].nctas = n;
+      used += n;
+    }
+    // hand the CTAs rounding left over to the heaviest groups
+    for (int left = slots - used; left > 0;) {
+      int best = -1;
+      for (int g = 0; g < ng; ++g)
+        if (c.groups[g].nctas < ntiles && (best < 0 || wgt[g] / c.groups[g].nctas > wgt[best] / c.groups[best].nctas)) best = g;
+      if (best < 0) break;
+      c.groups[best].nctas += 1;
+      --left;
+    }
+    int at = 0;
+    for (int g = 0; g < ng; ++g) {
+      c.groups[g].cta0 = at;
+      at += c.groups[g].nctas;
+    }
+    c.lag_grid = at;
+  }
   return true;
 }
 
@@ -748,12 +859,27 @@ bool lag_make_tensor_map(Ctx& c) {
 }
 
 int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
-  cudaFuncSetAttribute(k_lag_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
   const int ngroups = (int)c.groups.size();
-  const unsigned grid = (unsigned)((c.P / kTilePx) * ngroups);
+  const int ntiles = (int)(c.P / kTilePx);
+  // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold) weighs: batches of one or two
+  // chunks, and two unequal lag groups sharing the device by work.  With many groups, CTAs of the same pixel tile
+  // launched side by side share the NEW frames in L2 and open the same DRAM pages, which measured faster
+  // (config 4: 663 against 852 ms; config 2: 13.95 against 14.18 ms; config 3: 45.0 against 42.5 ms).
+  const bool persistent = c.lag_persistent >= 0 ? c.lag_persistent != 0 : (b <= 2 * kChunk || ngroups == 2);
+  const unsigned grid = persistent ? (unsigned)c.lag_grid : (unsigned)ntiles * (unsigned)ngroups;
   ProfScope ps(c, kKLag);
-  k_lag_tiled<<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.lag_stages,
-                                                                      c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1);
+  if (persistent) {
+    cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream);
+    k_lag_tiled<true><<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups,
+                                                                              c.lag_stages, c.d_tasks, c.d_groups, c.d_lags,
+                                                                              c.totals, c.I2, c.I1, ntiles, c.d_claim);
+  } else {
+    k_lag_tiled<false><<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups,
+                                                                               c.lag_stages, c.d_tasks, c.d_groups, c.d_lags,
+                                                                               c.totals, c.I2, c.I1, ntiles, c.d_claim);
+  }
   return 1;
 }
 

@@ -136,9 +136,13 @@ def test_scaled_configs(binding, oracle, idx, W, N, lags, n_b, batch, per_pixel)
     cfg = synth.config(idx, W=W, N=N, lags=lags, n_qbins=n_b)
     st = synth.make_stack(cfg, "cuda")
     ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=per_pixel)
-    for variant in ((0, 1) if W <= 512 else (0,)):
+    first = None
+    for variant in ((0, 1, 2, 3) if W <= 512 else (0, 2, 3)):
         g = gpu_run(binding, st, lags, n_b, batch=batch, variant=variant, want_2d=per_pixel)
         check_against_oracle(g, ref, W, per_pixel=per_pixel)
+        if variant != 1:  # the launch shape of the tiled kernel (one tile per CTA / persistent CTAs) changes no bit
+            first = first or g
+            assert np.array_equal(g["D"], first["D"]) and np.array_equal(g["I_q"], first["I_q"])
 
 
 # --------------------------------------------------------------------------------------------------------------
@@ -159,8 +163,9 @@ def test_random_lag_lists_batches_and_splits(binding, oracle, seed):
     cfg.seed = 500 + seed
     st = synth.make_stack(cfg, "cuda")
     ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=True)
-    g = gpu_run(binding, st, lags, n_b, batch=batch, split=split or None)
-    check_against_oracle(g, ref, W)
+    for variant in (2, 3):
+        g = gpu_run(binding, st, lags, n_b, batch=batch, split=split or None, variant=variant)
+        check_against_oracle(g, ref, W)
 
 
 def test_many_folds_in_one_launch(binding, oracle):

@@ -52,6 +52,12 @@ def check_plan(lags, plan):
         n_I += has_I
         assert (g["tau_min"], g["tau_max"]) == (lo, hi)
     assert n_I == 1
+    # persistent CTAs: contiguous shares, at least one per group, all resident slots handed out
+    at = 0
+    for g in groups:
+        assert g["cta0"] == at and g["nctas"] >= 1
+        at += g["nctas"]
+    assert at == max(2 * 148, len(groups))
     assert len(seen_tasks) == len(tasks)
     assert np.all(covered == 1), "every lag is accumulated by exactly one task"
     assert 2 <= plan["stages"] <= 8
