@@ -192,6 +192,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="internal batch size (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-hbm-regime", action="store_true", help="skip the small-batch run of the lag kernel")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -307,6 +308,8 @@ def run_ours(args, cfg):
                     hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9,
                              peak_gbs=peaks["hbm_gbs"], frac=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9 / peaks["hbm_gbs"],
                              note="of measured copy peak; HBM is not the binding roofline for dense lags (DESIGN.md §7.2)"))
+    if world == 1 and not args.no_hbm_regime and not args.batch:
+        roofline["hbm_bound_regime"] = run_hbm_regime(torch, binding, stack, cfg, P, peaks)
     fft_ms = ktimes["fft"][0]
     fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N      # one round trip between the passes
     fft_bytes_min = (2.0 * cfg.W * cfg.H + 8.0 * P) * cfg.N   # intermediate kept in L2 (what k_fft does)
@@ -334,6 +337,33 @@ def run_ours(args, cfg):
     print(json.dumps(out), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def run_hbm_regime(torch, binding, stack, cfg, P, peaks):
+    """The same lag kernel where HBM is its binding roofline (BASELINE.json metric: "lag-accumulation HBM GB/s"):
+    batches of one 26-step chunk, so that every launch re-reads the whole lag window and touches the fp64 totals
+    once per 26 frames.  Algorithmic bytes per launch = P (8 (b + Lmax) + 16 n_lags); time = CUDA
+    events around every k_lag_tiled launch on the library's stream, one warm-up stack then two timed."""
+    B = 26
+    st = torch.cuda.Stream(device=stack.device)
+    h = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=st, batch_frames=B)
+    h.set_profiling(True)
+    steps = 2
+    for i in range(1 + steps):
+        h.reset()
+        h.push(stack)
+        h.finalize()
+        if i == 0:
+            h.kernel_times()
+    ms, n = h.kernel_times()["lag_accum"]
+    h.close()
+    nb = (cfg.N + B - 1) // B
+    alg = P * (8.0 * (cfg.N + nb * cfg.lags[-1]) + 16.0 * len(cfg.lags) * nb)  # bytes per stack
+    ach = alg / (ms / steps * 1e-3) / 1e9
+    return dict(internal_batch=B, launches_per_step=n / steps, ms_per_step=ms / steps, algorithmic_gb_per_step=alg / 1e9,
+                achieved_gbs=ach, peak_gbs=peaks["hbm_gbs"], frac=ach / peaks["hbm_gbs"],
+                alu_floor_ms=(sum(max(0, cfg.N - t) for t in cfg.lags) * P * 4.0) / (SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6) * 1e3,
+                note="same kernel and stack, batches of 26 frames: algorithmic HBM time exceeds the ALU floor, HBM is the bound")
 
 
 def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
