@@ -92,3 +92,25 @@ def structure_function(frames, lags, n_b):
     D = [azimuthal(m)[0] for m in D2d]
     I_q, counts = azimuthal(I2d)
     return dict(sums=sums, D2d=D2d, I2d=I2d, D=D, I_q=I_q, counts=counts, n_pairs=n_pairs)
+
+
+def variance_spectrum(frames, n_b):
+    """Step 7: V2d = (1/N) sum_t |F_t - <F>_t|^2 per pixel and its azimuthal mean,
+    in explicit loops.  Returns dict with V2d[ky][kx], V_q[b], counts[b]."""
+    N = len(frames)
+    H, W = len(frames[0]), len(frames[0][0])
+    F = [dft2_unitary(normalise(fr)[1]) for fr in frames]
+    V2d = [[0.0] * W for _ in range(H)]
+    for ky in range(H):
+        for kx in range(W):
+            m = sum(F[t][ky][kx] for t in range(N)) / N
+            V2d[ky][kx] = sum(abs(F[t][ky][kx] - m) ** 2 for t in range(N)) / N
+    s = [0.0] * n_b
+    c = [0] * n_b
+    for ky in range(H):
+        for kx in range(W):
+            b = qbin(kx, ky, W, H, n_b)
+            if b >= 0:
+                s[b] += V2d[ky][kx]
+                c[b] += 1
+    return dict(V2d=V2d, V_q=[s[b] / c[b] if c[b] else 0.0 for b in range(n_b)], counts=c)

@@ -26,6 +26,9 @@
  * No blocking or fusion beyond a pixel-tiled loop order and OpenMP over pixel tiles in the
  * pair loop (it is still the explicit pair loop of step 3).  No -ffast-math.
  *
+ *   7. V2d(k) = (1/N) sum_t |F_t(k) - <F(k)>_t|^2 and its azimuthal mean: see
+ *        nfso_variance_spectrum below.
+ *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force DFT, numpy.fft, Parseval,
  * constant stack, gain invariance, travelling plane wave closed form, telegraph stack, ramp,
  * linearity (real-space difference then DFT), white noise D = 2 sigma^2 = 2 I, bin-count brute
@@ -293,6 +296,54 @@ int nfso_structure_function(const uint16_t* frames, int N, int W, int H, const i
   if (!D2d_out) free(D2d);
   if (!I2d_out) free(I2d);
   return NFSO_OK;
+}
+
+/* ---- variance form of the static-free spectrum (reading R9b) ------------
+ *
+ *   7. M(k)   = (1/N) sum_t F_t(k)                       time-averaged field (the static image: beam, fringes)
+ *      V2d(k) = (1/N) sum_t |F_t(k) - M(k)|^2            power of the fluctuations alone
+ *      V(b)   = azimuthal mean of V2d (same bins as step 5-6)
+ *
+ * PAPER.md:L21-25, Eq. 1: the difference spectrum is 2a{T(q) I_s(q) [1 - f(q,tau)] + B(q)}; for lags beyond the
+ * relaxation time (f -> 0) it reaches the plateau 2a{T I_s + B}, and the variance of the field in time is half
+ * of that plateau: for all N(N-1)/2 pairs, sum_tau (N - tau) D2d(k,tau) = N^2 V2d(k) (pin P10).  Written as its
+ * two-pass definition: pass 1 forms M, pass 2 transforms every frame again and sums |F_t - M|^2 (O(P) memory). */
+int nfso_variance_spectrum(const uint16_t* frames, int N, int W, int H, int n_b, int method, double* V_q,
+                           int64_t* counts, double* V2d_out) {
+  if (!frames || N < 1 || W < 1 || H < 1 || n_b < 1 || !V_q) return NFSO_ERR_ARG;
+  const long P = (long)W * H;
+  cplx* M = (cplx*)calloc((size_t)P, sizeof(cplx));
+  cplx* F = (cplx*)malloc(sizeof(cplx) * (size_t)P);
+  double* tmp = (double*)malloc(sizeof(double) * (size_t)P);
+  double* V2d = V2d_out ? V2d_out : (double*)malloc(sizeof(double) * (size_t)P);
+  if (!M || !F || !tmp || !V2d) return NFSO_ERR_MEM;
+  int rc = NFSO_OK;
+  for (int t = 0; t < N && !rc; ++t) { /* pass 1: the mean field */
+    rc = transform_frame(frames + (size_t)t * P, W, H, method, tmp, F);
+    if (!rc)
+      for (long k = 0; k < P; ++k) M[k] += F[k];
+  }
+  if (!rc) {
+    for (long k = 0; k < P; ++k) M[k] /= (double)N;
+    memset(V2d, 0, sizeof(double) * (size_t)P);
+    for (int t = 0; t < N && !rc; ++t) { /* pass 2: squared deviations from it */
+      rc = transform_frame(frames + (size_t)t * P, W, H, method, tmp, F);
+      if (!rc)
+        for (long k = 0; k < P; ++k) {
+          cplx d = F[k] - M[k];
+          V2d[k] += creal(d) * creal(d) + cimag(d) * cimag(d);
+        }
+    }
+  }
+  if (!rc) {
+    for (long k = 0; k < P; ++k) V2d[k] /= (double)N;
+    azimuthal_mean(V2d, W, H, n_b, V_q, counts);
+  }
+  free(M);
+  free(F);
+  free(tmp);
+  if (!V2d_out) free(V2d);
+  return rc;
 }
 
 /* ---- same definition, frames streamed through a window of Lmax+1 transforms ------------------

@@ -132,3 +132,19 @@ def structure_function_sampled(frames, lags, sample_ky, sample_kx):
     if rc:
         raise RuntimeError("oracle structure_function_sampled rc=%d" % rc)
     return Result(D2d=D2d, I2d=I2d, n_pairs=npairs)
+
+
+def variance_spectrum(frames, n_b, method=0, want_2d=False):
+    """Step 7: V2d(k) = (1/N) sum_t |F_t(k) - <F(k)>_t|^2 and its azimuthal mean.
+
+    Returns Result(V_q [n_b], counts [n_b] int64, V2d [H][W] or None)."""
+    f = _frames(frames)
+    N, H, W = f.shape
+    V_q = np.zeros(n_b, dtype=np.float64)
+    cnt = np.zeros(n_b, dtype=np.int64)
+    V2d = np.zeros((H, W), dtype=np.float64) if want_2d else None
+    rc = lib().nfso_variance_spectrum(_p(f, C.c_uint16), N, W, H, int(n_b), int(method), _p(V_q, C.c_double),
+                                      _p(cnt, C.c_int64), _p(V2d, C.c_double))
+    if rc:
+        raise RuntimeError("oracle variance_spectrum rc=%d" % rc)
+    return Result(V_q=V_q, counts=cnt, V2d=V2d)

@@ -313,3 +313,74 @@ def test_p13_golden_vector(oracle):
     np.testing.assert_allclose(g["I"], survey_I, rtol=2e-12, atol=1e-20)
     np.testing.assert_allclose(g["D"][2], [0, 2.216787015730e-4, 5.658843130045e-4, 2.315592755608e-3], rtol=2e-12)
     np.testing.assert_allclose(g["D"][3], [0, 8.178509086745e-4, 3.902731171114e-4, 1.481795127132e-3], rtol=2e-12)
+
+
+# ---- P14: variance form of the fluctuation spectrum (oracle step 7) -------------------
+def test_p14_variance_bruteforce_python_loops(oracle):
+    # an independent statement in pure-Python loops (oracle/brute_force.py) on a tiny stack
+    fr = _rng(21).integers(100, 4000, (5, 8, 8)).astype(np.uint16)
+    r = oracle.variance_spectrum(fr, 4, want_2d=True)
+    b = bf.variance_spectrum(fr.tolist(), 4)
+    assert r.counts.tolist() == b["counts"]
+    np.testing.assert_allclose(r.V2d, np.array(b["V2d"]), rtol=1e-10, atol=1e-18)
+    np.testing.assert_allclose(r.V_q, np.array(b["V_q"]), rtol=1e-10)
+    # method 1 (brute-force DFT inside the C oracle) agrees with the radix-2 path
+    r1 = oracle.variance_spectrum(fr, 4, method=1, want_2d=True)
+    np.testing.assert_allclose(r1.V2d, r.V2d, rtol=1e-9, atol=1e-18)
+
+
+def test_p14_variance_is_tied_to_D_by_the_all_pairs_identity(oracle):
+    # sum_tau (N - tau) D2d(k, tau) over ALL lags 1..N-1 = N^2 V2d(k): the pair loop (pinned by P4-P7, P10)
+    # fixes the variance; a dropped mean, a 1/(N-1) divisor or a transposed map fails here
+    N = 9
+    fr = _rng(22).integers(100, 4000, (N, 16, 32)).astype(np.uint16)
+    lags = list(range(1, N))
+    d = oracle.structure_function(fr, lags, 8, want_2d=True)
+    v = oracle.variance_spectrum(fr, 8, want_2d=True)
+    lhs = sum((N - tau) * d.D2d[l] for l, tau in enumerate(lags)) / N ** 2
+    assert np.max(np.abs(lhs - v.V2d)) < 1e-10 * v.V2d.max()
+    assert np.array_equal(v.counts, d.counts)
+    # binned: the same identity on the azimuthal means
+    lhs_b = sum((N - tau) * d.D[l] for l, tau in enumerate(lags)) / N ** 2
+    np.testing.assert_allclose(lhs_b, v.V_q, rtol=1e-10, atol=1e-18)
+
+
+def test_p14_static_images_have_no_variance_and_gain_does_not_matter(oracle):
+    one = np.rint(_plane_wave_frames(1, 32, 64, 10, 4, 0.0, 20000.0, 4000.0)[0]).astype(np.uint16)
+    r = oracle.variance_spectrum(np.repeat(one[None], 6, axis=0), 16, want_2d=True)
+    assert np.all(r.V2d < 1e-25) and np.all(r.V_q < 1e-25)     # a static fringe is in I(q), not in V(q)
+    base = _rng(23).integers(50, 500, (5, 16, 16)).astype(np.uint16)
+    gains = np.array([1, 3, 2, 7, 5], dtype=np.uint16)[:, None, None]
+    a = oracle.variance_spectrum(base, 8, want_2d=True)
+    b = oracle.variance_spectrum(base * gains, 8, want_2d=True)
+    np.testing.assert_allclose(a.V2d, b.V2d, rtol=1e-9, atol=1e-22)
+
+
+def test_p14_travelling_wave_closed_form(oracle):
+    # I_t = A + B cos(k0.x - omega t) with omega N = 2 pi m: the field at +-k0 is (B/2A) sqrt(WH) e^{-+ i omega t},
+    # its time mean vanishes over whole periods, so V2d(+-k0) = (B/2A)^2 WH exactly and 0 elsewhere
+    N, H, W, kx0, ky0, A, B = 16, 16, 32, 5, 3, 1000.0, 100.0
+    om = 2 * math.pi * 3 / N
+    F = np.array([oracle.transform_f64(im / A) for im in _plane_wave_frames(N, H, W, kx0, ky0, om, A, B)])
+    V = np.mean(np.abs(F - F.mean(axis=0)) ** 2, axis=0)
+    expect = (B / (2 * A)) ** 2 * W * H
+    assert abs(V[ky0, kx0] - expect) < 1e-12 * expect and abs(V[H - ky0, W - kx0] - expect) < 1e-12 * expect
+    # and through the whole oracle on uint16 frames: one |q| bin holds 2 * expect / c_b (quantisation floor aside)
+    A, B, n_b = 20000.0, 4000.0, 16
+    fr = np.array([np.rint(f) for f in _plane_wave_frames(N, H, W, kx0, ky0, om, A, B)]).astype(np.uint16)
+    r = oracle.variance_spectrum(fr, n_b)
+    b0 = oracle.qbin(kx0, ky0, W, H, n_b)
+    expect = 2 * (B / (2 * A)) ** 2 * W * H / r.counts[b0]
+    assert abs(r.V_q[b0] - expect) < 2e-4 * expect
+    assert np.delete(r.V_q, b0).max() < 1e-4 * expect
+
+
+def test_p14_white_noise_variance_is_half_the_D_plateau(oracle):
+    rng = _rng(24)
+    N, H, W, mu, sig, n_b = 200, 32, 32, 10000.0, 300.0, 16
+    fr = np.rint(rng.normal(mu, sig, (N, H, W))).astype(np.uint16)
+    v = oracle.variance_spectrum(fr, n_b)
+    var = (sig / mu) ** 2 * (1.0 - 1.0 / N)     # the sample mean takes 1/N of the variance
+    for b in range(n_b):
+        if v.counts[b]:
+            assert abs(v.V_q[b] / var - 1.0) < 6.0 / math.sqrt(v.counts[b] * N / 2.0)
