@@ -99,6 +99,16 @@ NFS_API int nfs_get_pair_counts(nfs_ctx* ctx, int64_t* n_pairs);
 NFS_API int nfs_get_D2d(nfs_ctx* ctx, int lag_index, double* out);
 NFS_API int nfs_get_I2d(nfs_ctx* ctx, double* out);
 
+/* Variance form of the fluctuation spectrum: V2d(k) = <|F_t(k) - <F(k)>_t|^2>_t, the power
+ * of the field's fluctuations in time with the static image (beam, fringes) removed — half the large-lag plateau
+ * 2a{T I_s + B} of the difference spectrum of PAPER.md:L23-25, Eq. 1 (for all lags 1..N-1,
+ * sum_tau (N - tau) D2d(k,tau) = N^2 V2d(k)).  Built at no extra cost from the sums the lag kernel keeps for I(q).
+ *   nfs_get_variance  V_q HOST [n_qbins]: azimuthal mean of V2d over the same |q| bins as D and I (empty bin: 0.0).
+ *   nfs_get_V2d       out HOST [H][W/2+1], same layout as nfs_get_I2d.
+ * Both synchronise the stream, are non-destructive snapshots, and return NFS_ERR_STATE before the first frame. */
+NFS_API int nfs_get_variance(nfs_ctx* ctx, double* V_q);
+NFS_API int nfs_get_V2d(nfs_ctx* ctx, double* out);
+
 /* Number of frames pushed so far; ring capacity in frames; bytes of device memory held. */
 NFS_API int64_t nfs_num_frames(const nfs_ctx* ctx);
 NFS_API int nfs_ring_capacity(const nfs_ctx* ctx);

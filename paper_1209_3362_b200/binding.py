@@ -30,6 +30,8 @@ SYMBOLS = [
     ("nfs_get_pair_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
     ("nfs_get_D2d", C.c_int, [_P, C.c_int, C.POINTER(C.c_double)]),
     ("nfs_get_I2d", C.c_int, [_P, C.POINTER(C.c_double)]),
+    ("nfs_get_variance", C.c_int, [_P, C.POINTER(C.c_double)]),
+    ("nfs_get_V2d", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_num_frames", C.c_int64, [_P]),
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
@@ -172,6 +174,16 @@ class NFS:
     def I2d(self):
         out = np.zeros((self.H, self.W // 2 + 1), dtype=np.float64)
         _check(self.lib.nfs_get_I2d(self.handle, _dp(out, C.c_double)), self.handle)
+        return out
+
+    def variance(self):
+        out = np.zeros(self.n_qbins, dtype=np.float64)
+        _check(self.lib.nfs_get_variance(self.handle, _dp(out, C.c_double)), self.handle)
+        return out
+
+    def V2d(self):
+        out = np.zeros((self.H, self.W // 2 + 1), dtype=np.float64)
+        _check(self.lib.nfs_get_V2d(self.handle, _dp(out, C.c_double)), self.handle)
         return out
 
     def set_lag_kernel(self, variant):

@@ -278,7 +278,7 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   if (!dev_alloc(c, &c.I1, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.sums, (size_t)c.B + 1)) goto fail;
   if (!dev_alloc(c, &c.fft_cnt, 1 + 3 * (size_t)c.B)) goto fail;
-  if (!dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 1) * c.n_qbins)) goto fail;
+  if (!dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 2) * c.n_qbins)) goto fail;
   if (!dev_alloc(c, &c.d_tmp, (size_t)c.P)) goto fail;
   if (!dev_alloc(c, &c.d_flags, 1)) goto fail;
   if (!build_tables(c)) goto fail;
@@ -381,6 +381,31 @@ int nfs_get_I2d(nfs_ctx* h, double* out) {
   if (!flush_pending(c)) return c.status;
   c.n_launches += launch_I2d(c, c.d_tmp);
   if (!check_launch(c, "I2d launch")) return c.status;
+  return get_plane(c, out);
+}
+
+int nfs_get_variance(nfs_ctx* h, double* V_q) {
+  if (!h || !V_q) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (c.status != NFS_OK) return c.status;
+  if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
+  c.n_launches += launch_bin(c);
+  if (!check_launch(c, "bin launch")) return c.status;
+  if (!NFS_CUDA(c, cudaMemcpyAsync(V_q, c.d_out + (size_t)(c.n_lags + 1) * c.n_qbins, sizeof(double) * c.n_qbins,
+                                   cudaMemcpyDeviceToHost, c.stream)))
+    return c.status;
+  return sync_and_check(c);
+}
+
+int nfs_get_V2d(nfs_ctx* h, double* out) {
+  if (!h || !out) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (c.status != NFS_OK) return c.status;
+  if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
+  c.n_launches += launch_V2d(c, c.d_tmp);
+  if (!check_launch(c, "V2d launch")) return c.status;
   return get_plane(c, out);
 }
 

@@ -19,7 +19,18 @@ __device__ __forceinline__ double i2d_value(const double* __restrict__ I2, const
   return (I2[p] + 2.0 * (s1.x * rx + s1.y * ry)) * invN + (rx * rx + ry * ry);
 }
 
-// grid (n_qbins, n_lags + 1), 128 threads.  Row l < n_lags: D(b, tau_l); row n_lags: I(b).
+// value of the variance-form spectrum at pixel p (half the plateau
+// of Eq. 1): V2d = <|F_t - <F>_t|^2>_t = sum|F'|^2 / N - |sum F'|^2 / N^2.  The variance does not depend on the
+// reference frame subtracted before the transform, so F_r does not enter; F' = F - F_0 is of the size of the
+// fluctuations, so the difference does not cancel.
+__device__ __forceinline__ double v2d_value(const double* __restrict__ I2, const double2* __restrict__ I1, int64_t p,
+                                            double invN) {
+  const double2 s1 = I1[p];
+  const double mx = s1.x * invN, my = s1.y * invN;
+  return fmax(I2[p] * invN - (mx * mx + my * my), 0.0);
+}
+
+// grid (n_qbins, n_lags + 2), 128 threads.  Row l < n_lags: D(b, tau_l); row n_lags: I(b); row n_lags + 1: V(b).
 __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, const double* __restrict__ I2,
                                              const double2* __restrict__ I1, const float2* __restrict__ Fref,
                                              const uint32_t* __restrict__ perm, const int32_t* __restrict__ bin_start,
@@ -42,8 +53,10 @@ __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, 
     double v;
     if (row < n_lags)
       v = totals[(int64_t)row * P + p] * inv;
-    else
+    else if (row == n_lags)
       v = i2d_value(I2, I1, Fref, p, inv);
+    else
+      v = v2d_value(I2, I1, p, inv);
     acc += wgt * v;
     wsum += wgt;
   }
@@ -72,6 +85,12 @@ __global__ void __launch_bounds__(256) k_I2d(const double* __restrict__ I2, cons
   if (p < P) dst[p] = i2d_value(I2, I1, Fref, p, 1.0 / (double)N);
 }
 
+__global__ void __launch_bounds__(256) k_V2d(const double* __restrict__ I2, const double2* __restrict__ I1, int64_t P,
+                                             int64_t N, double* __restrict__ dst) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < P) dst[p] = v2d_value(I2, I1, p, 1.0 / (double)N);
+}
+
 __global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int64_t P, double inv,
                                              double* __restrict__ dst) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -79,7 +98,7 @@ __global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int
 }
 
 int launch_bin(Ctx& c) {
-  dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 1));
+  dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 2));
   ProfScope ps(c, kKBin);
   k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.I2, c.I1, c.Fref, c.perm, c.bin_start, c.d_lags, c.n_lags, c.n_qbins,
                                     c.P, c.n_frames, c.d_out);
@@ -88,6 +107,11 @@ int launch_bin(Ctx& c) {
 
 int launch_I2d(Ctx& c, double* d_dst) {
   k_I2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, c.n_frames, d_dst);
+  return 1;
+}
+
+int launch_V2d(Ctx& c, double* d_dst) {
+  k_V2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.P, c.n_frames, d_dst);
   return 1;
 }
 

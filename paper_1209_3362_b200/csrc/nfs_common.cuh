@@ -97,7 +97,7 @@ struct Ctx {
   int32_t* d_lags = nullptr;     // [n_lags]
   uint32_t* perm = nullptr;      // [n_binned] pixel index | (weight-2 flag << 31), grouped by bin
   int32_t* bin_start = nullptr;  // [n_qbins + 1]
-  double* d_out = nullptr;       // [(n_lags + 1)][n_qbins] binned results
+  double* d_out = nullptr;       // [(n_lags + 2)][n_qbins] binned results: D rows, I row, V row
   double* d_tmp = nullptr;       // [P] scratch for the 2-D getters
   int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
   LagTask* d_tasks = nullptr;
@@ -155,8 +155,9 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b);
 bool lag_plan(Ctx& c, int smem_per_sm, int cta_slots, int ntiles);
 bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
 // nfs_bin.cu
-int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1) and I (row n_lags)
+int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1), I (row n_lags), V (row n_lags+1)
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
+int launch_V2d(Ctx& c, double* d_dst);       // d_dst[P] = V2d (variance form) in ring layout
 int launch_D2d(Ctx& c, int l, double* d_dst);
 
 }  // namespace nfs

@@ -221,3 +221,50 @@ def test_config4_shape_streamed_sampled_pixels(binding, oracle):
         worst = max(worst, float((np.abs(g - r)[m] / r[m]).max()))
     assert worst < 1e-3, worst
     assert np.all(np.isfinite(D)) and np.all(D[:, cnt > 0] > 0)
+
+
+# --------------------------------------------------------------------------------------------------------------
+# variance form of the fluctuation spectrum: nfs_get_variance / nfs_get_V2d
+# --------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("idx,W,N,batch,split", [(0, 64, 32, 0, 0), (1, 128, 300, 0, 0), (1, 256, 700, 128, 100),
+                                                 (2, 512, 120, 0, 0), (3, 1024, 40, 16, 0)])
+def test_variance_spectrum_against_oracle(binding, oracle, idx, W, N, batch, split):
+    n_b = max(8, W // 4)
+    lags = [1, 2, 3, 5, 8, 13, 21]
+    cfg = synth.config(idx, W=W, N=N, lags=lags, n_qbins=n_b)
+    st = synth.make_stack(cfg, "cuda")
+    ref = oracle.variance_spectrum(st.cpu().numpy(), n_b, want_2d=True)
+    nfs = binding.NFS(W, W, lags, n_b, batch_frames=batch)
+    if split:
+        for i in range(0, N, split):
+            nfs.push(st[i:i + split].contiguous())
+    else:
+        nfs.push(st)
+    V = nfs.variance()
+    V2d = nfs.V2d()
+    D, I_q, cnt = nfs.finalize()
+    assert np.array_equal(V, nfs.variance()), "a snapshot: asking twice changes nothing"
+    nfs.close()
+    nz = ref.counts > 0
+    assert np.array_equal(cnt, ref.counts)
+    assert np.all(V[~nz] == 0.0)
+    eV = float(np.max(np.abs(V[nz] - ref.V_q[nz]) / ref.V_q[nz]))
+    assert eV < 1e-4, "binned V rel err %.3e" % eV
+    r2 = ref.V2d[:, :W // 2 + 1]
+    m = r2 > 1e-6 * r2.max()
+    eP = float(np.max(np.abs(V2d[m] - r2[m]) / r2[m]))
+    assert eP < 1e-3, "per-pixel V2d rel err %.3e" % eP
+    assert V2d[0, 0] < 1e-9 * r2.max()          # every normalised frame has the same DC value
+    # for long lags the difference spectrum approaches twice the variance, never far above it
+    assert np.all(D[-1][nz] < 4.0 * V[nz] * 1.01 + 1e-30)
+
+
+def test_variance_of_a_constant_stack_vanishes(binding):
+    one = torch.randint(100, 4000, (64, 64), dtype=torch.int32, device="cuda").to(torch.uint16)
+    st = one[None].repeat(20, 1, 1).contiguous()
+    nfs = binding.NFS(64, 64, [1, 2], 16)
+    nfs.push(st)
+    # F'_t = FFT(i_t - r) is the same tiny rounding residual for every frame; what is left of its variance is the
+    # rounding of the sums (the oracle's two-pass form leaves < 1e-25 as well), against fluctuation spectra of order 1e-4
+    assert np.all(nfs.variance() < 1e-18) and np.all(nfs.V2d() < 1e-18)
+    nfs.close()
