@@ -2,13 +2,17 @@
 // for every new frame s of a batch and every requested lag tau ("only the square
 // moduli of FFT differences are evaluated N(N-1)/2 times"; L25 average over the measurement time).
 //
-// k_lag_tiled (default): a CTA owns 32 consecutive Fourier pixels and one group of lags; a producer
-// warp streams the batch through shared memory with TMA tensor copies (cp.async.bulk.tensor + mbarrier):
-// a NEW stream (frames s) and an OLD stream delayed by the group's lags.  A consumer warp owns up to
+// k_lag_tiled (default): a CTA works on 32 consecutive Fourier pixels and one group of lags at a time; a
+// producer warp streams the batch through shared memory with TMA tensor copies (cp.async.bulk.tensor +
+// mbarrier): a NEW stream (frames s) and an OLD stream delayed by the group's lags.  A consumer warp owns up to
 // kG lags: for a run of contiguous lags it keeps a rotating register window of the kG most recent OLD
 // frames, so one step costs two LDS.64 and kG pair-updates (packed sub.f32x2 + fma.rn.f32x2: two issue
-// slots per update); isolated lags take one LDS.64 per update.  fp32 partial sums per batch are
-// folded into the fp64 totals once per batch (BASELINE.json north_star (4)).
+// slots per update); isolated lags take one LDS.64 per update.  fp32 partial sums are folded into the fp64
+// totals every kFoldChunks chunks and at the end of a tile (BASELINE.json north_star (4)).  One warp of the
+// lightest group also adds the batch to the I sums (sum |F'|^2, sum F').
+// Two launch shapes (template parameter PERS, chosen per batch by launch_lag_tiled): one CTA per (pixel tile,
+// lag group), or persistent CTAs that claim the pixel tiles of their group and keep the pipeline full across
+// tiles.  Results do not depend on the shape.
 // k_lag_simple: plain per-pixel kernel through L1/L2, kept as an in-library cross-check.
 #include <algorithm>
 
@@ -94,8 +98,11 @@ __global__ void __launch_bounds__(128) k_lag_simple(const float2* __restrict__ r
 //                                E0 + e, E0 = t0 - tau_min - LEAD*kChunk, at row e % (NSLOT*kChunk); the
 //                                last kChunk rows duplicate slot 0 so kG consecutive rows never wrap
 //   NEW  [stages * kChunk]       the batch's own frames, chunk c in stage c % stages
-// full[stage]: the producer's arrival + the bytes of its copies for consumer chunk c (NEW chunk c, OLD
-// chunk c + LEAD; chunk 0 also brings OLD chunks 0..LEAD-1).  empty[stage]: the consumer warps.
+// full[stage]: the producer's arrival + the bytes of its copies for one pipeline step; empty[stage]: the
+// consumer warps.  One tile per CTA: step = consumer chunk c (NEW chunk c, OLD chunk c + LEAD; chunk 0 also
+// brings OLD chunks 0..LEAD-1).  Persistent: every tile has LEAD prologue steps that bring one OLD chunk each,
+// then one step per chunk (OLD chunk j, NEW chunk j - LEAD); steps and ring slots are numbered through all the
+// tiles of the CTA, so the next tile's window streams in while the last chunks of the current one are consumed.
 // `stages` (2..kMaxStages) is chosen at create from the shared memory the widest lag group leaves, so
 // that the producer runs several chunks (each ~3 us of math) ahead of the HBM/L2 latency.
 // A chunk of frames that is contiguous in the HBM ring is one 2-D TMA box (cp.async.bulk.tensor,
