@@ -195,6 +195,9 @@ __device__ __forceinline__ void st_f4_hint(float4* p, float4 v, unsigned long lo
 #ifndef NFS_FFT_NT
 #define NFS_FFT_NT 128
 #endif
+#ifndef NFS_FFT_NT_LARGE
+#define NFS_FFT_NT_LARGE 256
+#endif
 #ifndef NFS_FFT_DR
 #define NFS_FFT_DR 0
 #define NFS_FFT_DC 0
@@ -205,8 +208,8 @@ constexpr int kMaxSlots = 40;
 template <int L>
 struct Plan {
   static constexpr int T = L / 32;                       // threads per FFT
-  static constexpr int NT = L <= 1024 ? (L >= 512 ? NFS_FFT_NT : 256) : 512;  // threads per CTA
-  static constexpr int minBlocks = L <= 1024 ? 512 / NT : 1;  // CTAs per SM the kernel is compiled for
+  static constexpr int NT = L <= 1024 ? (L >= 512 ? NFS_FFT_NT : 256) : NFS_FFT_NT_LARGE;  // threads per CTA
+  static constexpr int minBlocks = 512 / NT;  // CTAs per SM the kernel is compiled for (128 registers per thread)
   static constexpr int Fc = NT / T;                      // FFTs per CTA item
   static constexpr bool two = L > 1024;                  // two-level plan
   static constexpr int Mi = two ? L / 1024 : T;          // lanes per (inner) FFT
