@@ -217,7 +217,7 @@ def run_ours(args, cfg):
         raise RuntimeError("bench.py --impl ours needs a CUDA device: the hot path has no CPU fallback")
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    if world > 1 or os.environ.get("NFS_BENCH_FORCE_DIST"):  # the env switch exercises the N > 1 code path on one GPU
         import torch.distributed as dist_mod
 
         dist = dist_mod
