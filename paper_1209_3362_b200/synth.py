@@ -68,10 +68,14 @@ def config(idx: int, W: int = 0, N: int = 0, lags=None, n_qbins: int = 0) -> Sta
                 poisson=True, nrf=3, chunk=0),
         4: dict(W=1024, N=10000, lags=list(range(1, 1001)), n_qbins=256, q0W=10.24, gamma0=0.01, A=8000.0, bits=14,
                 poisson=True, nrf=0, chunk=256),
+        # not a BASELINE.json config: the workload of the paper's only timing (Fig. 3: 512 x 512 px,
+        # N = 2048 images, all N - 1 = 2047 lags, full 2-D spectra kept), generator of config 1
+        5: dict(W=512, N=2048, lags=list(range(1, 2048)), n_qbins=128, q0W=10.24, gamma0=0.05, A=2000.0, bits=12,
+                poisson=False, nrf=0, chunk=0),
     }[idx]
     w = W or base["W"]
     return StackConfig(
-        name="config%d" % idx if not (W or N or lags or n_qbins) else "config%d-scaled" % idx,
+        name=("config%d" % idx if idx < 5 else "paper-fig3") if not (W or N or lags or n_qbins) else "config%d-scaled" % idx,
         W=w, H=w, N=N or base["N"], lags=list(lags) if lags is not None else base["lags"],
         n_qbins=n_qbins or base["n_qbins"], sigma_b=0.3125 * w, q0=base["q0W"] / w, gamma0=base["gamma0"],
         A=base["A"], bits=base["bits"], poisson=base["poisson"], n_random_fringes=base["nrf"], seed=idx,
