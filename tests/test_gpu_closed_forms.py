@@ -268,3 +268,30 @@ def test_variance_of_a_constant_stack_vanishes(binding):
     # rounding of the sums (the oracle's two-pass form leaves < 1e-25 as well), against fluctuation spectra of order 1e-4
     assert np.all(nfs.variance() < 1e-18) and np.all(nfs.V2d() < 1e-18)
     nfs.close()
+
+
+def test_all_lags_identity_ties_D_to_the_variance_on_the_gpu(binding, oracle):
+    """The paper's own case (all N - 1 lags, N(N-1)/2 pairs) at reduced size: every lag 1..N-1 in
+    one context (16 lag groups), parity with the oracle, and the identity sum_tau (N - tau) D2d(k,tau) = N^2 V2d(k)
+    between two outputs that come from different accumulators (pair totals vs. the I sums)."""
+    W, N, n_b = 64, 200, 16
+    lags = list(range(1, N))
+    cfg = synth.config(1, W=W, N=N, lags=lags, n_qbins=n_b)
+    st = synth.make_stack(cfg, "cuda")
+    nfs = binding.NFS(W, W, lags, n_b)
+    nfs.push(st)
+    D, I_q, cnt = nfs.finalize()
+    V2d = nfs.V2d()
+    V = nfs.variance()
+    acc = np.zeros_like(V2d)
+    for l, tau in enumerate(lags):
+        acc += (N - tau) * nfs.D2d(l)
+    nfs.close()
+    m = V2d > 1e-6 * V2d.max()
+    assert np.max(np.abs(acc[m] / N ** 2 - V2d[m]) / V2d[m]) < 2e-5
+    ref = oracle.structure_function(st.cpu().numpy(), lags, n_b)
+    nz = ref.counts > 0
+    assert np.array_equal(cnt, ref.counts)
+    assert np.max(np.abs(D[:, nz] - ref.D[:, nz]) / ref.D[:, nz]) < 1e-4
+    lhs = sum((N - tau) * D[l] for l, tau in enumerate(lags)) / N ** 2
+    assert np.max(np.abs(lhs[nz] - V[nz]) / V[nz]) < 2e-5
