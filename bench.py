@@ -28,7 +28,7 @@ SM_COUNT = 148
 FP32_LANES_PER_SM = 128
 # DRAM bytes (read + write) of one k_lag_tiled launch from the committed `ncu --set full` capture
 # (profiles/r01_lag_ncu.md), keyed by (workload, internal batch, frames); other workloads report null.
-NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {("config2", 1024, 2000): 0.5 * (5.268e9 + 5.490e9)}  # profiles/r01_lag_ncu.md
+NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {("config2", 1024, 2000): 0.5 * (5.272e9 + 5.497e9)}  # profiles/r01_lag_ncu.md
 
 
 def load_peaks():
