@@ -371,26 +371,29 @@ def run_hbm_regime(torch, binding, stack, cfg, P, peaks):
 
 
 def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
-    """Stack in pinned host memory; chunks of `chunk` frames double-buffered through two device staging
-    buffers on a copy stream, pushed through the C-ABI, result read back by nfs_finalize."""
+    """Stack in pinned host memory; chunks of `chunk` frames go through a ring of device staging buffers on a
+    copy stream (enough of them to keep copying while a lag kernel of a whole batch runs: a staging buffer is
+    free again only when the work enqueued by its push has finished), are pushed through the C-ABI, and the
+    result is read back by nfs_finalize."""
     chunk = cfg.chunk or 256
     chunk = min(chunk, cfg.N)
     host = torch.empty(stack.shape, dtype=torch.uint16, pin_memory=True)
     host.copy_(stack)
     torch.cuda.synchronize()
-    stage = [torch.empty((chunk, cfg.H, cfg.W), dtype=torch.uint16, device=dev) for _ in range(2)]
+    n_stage = max(2, min(6, (cfg.N + chunk - 1) // chunk))
+    stage = [torch.empty((chunk, cfg.H, cfg.W), dtype=torch.uint16, device=dev) for _ in range(n_stage)]
     copy_stream = torch.cuda.Stream(device=dev)
-    copied = [torch.cuda.Event() for _ in range(2)]
-    consumed = [torch.cuda.Event() for _ in range(2)]
+    copied = [torch.cuda.Event() for _ in range(n_stage)]
+    consumed = [torch.cuda.Event() for _ in range(n_stage)]
 
     def step():
         nfs.reset()
         i, k = 0, 0
         while i < cfg.N:
             m = min(chunk, cfg.N - i)
-            b = k & 1
+            b = k % n_stage
             with torch.cuda.stream(copy_stream):
-                if k >= 2:
+                if k >= n_stage:
                     copy_stream.wait_event(consumed[b])
                 stage[b][:m].copy_(host[i:i + m], non_blocking=True)
                 copied[b].record(copy_stream)
@@ -418,7 +421,8 @@ def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
     del host
     return dict(value=world * cfg.N / dt, unit="frames/s", h2d_bytes_per_step=int(stack.numel() * 2),
                 d2h_bytes_per_step=int(D.nbytes + I.nbytes + 4), ms_per_step=dt * 1e3, chunk_frames=chunk,
-                note="pinned host stack -> 2 device staging buffers (copy stream) -> nfs_push_frames -> nfs_finalize")
+                staging_buffers=n_stage,
+                note="pinned host stack -> ring of device staging buffers (copy stream) -> nfs_push_frames -> nfs_finalize")
 
 
 if __name__ == "__main__":
