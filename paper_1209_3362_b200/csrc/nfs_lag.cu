@@ -326,10 +326,10 @@ __device__ __forceinline__ void sparse_masked_dispatch(int cnt, int ns, f2x (&ac
   }
 }
 
-template <bool PERS>
+template <bool PERS, bool SKIP>
 __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
-    k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P, int64_t t0,
-                int b, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
+    k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P,
+                int64_t t0_batch, int b_batch, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
                 const int32_t* __restrict__ lags, double* __restrict__ totals, double* __restrict__ I2,
                 double2* __restrict__ I1, int ntiles, int* __restrict__ claim) {
   constexpr int G = kG;
@@ -351,7 +351,19 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   const LagGroup& grp = groups[gi];
   const int tau_min = grp.tau_min, tau_max = grp.tau_max;
   // no frame pair of this group exists yet (the group that accumulates the I sums always runs)
-  if (grp.flags == 0 && (int64_t)tau_min > t0 + b - 1) return;
+  if (grp.flags == 0 && (int64_t)tau_min > t0_batch + b_batch - 1) return;
+  // SKIP (launched only while some group's smallest lag still reaches back before frame 0): such a group skips
+  // the whole chunks in which it has no pair, i.e. it works on the batch cut at the front (the I sums need every
+  // frame: that group keeps the whole batch).  Otherwise t0 and b stay kernel parameters (no registers).
+  int64_t t0 = t0_batch;
+  int b = b_batch;
+  if constexpr (SKIP) {
+    if (grp.flags == 0 && (int64_t)tau_min > t0) {
+      const int skip = (int)(((int64_t)tau_min - t0) / kChunk) * kChunk;
+      t0 += skip;
+      b -= skip;
+    }
+  }
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int LEAD = lag_lead(tau_min, tau_max);
   const int NSLOT = LEAD + stages;
@@ -866,8 +878,10 @@ bool lag_make_tensor_map(Ctx& c) {
 }
 
 int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
-  cudaFuncSetAttribute(k_lag_tiled<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
-  cudaFuncSetAttribute(k_lag_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
+  cudaFuncSetAttribute(k_lag_tiled<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
   const int ngroups = (int)c.groups.size();
   const int ntiles = (int)(c.P / kTilePx);
   // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold) weighs: batches of one or two
@@ -877,16 +891,15 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   const bool persistent = c.lag_persistent >= 0 ? c.lag_persistent != 0 : (b <= 2 * kChunk || ngroups == 2);
   const unsigned grid = persistent ? (unsigned)c.lag_grid : (unsigned)ntiles * (unsigned)ngroups;
   ProfScope ps(c, kKLag);
-  if (persistent) {
-    cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream);
-    k_lag_tiled<true><<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups,
-                                                                              c.lag_stages, c.d_tasks, c.d_groups, c.d_lags,
-                                                                              c.totals, c.I2, c.I1, ntiles, c.d_claim);
-  } else {
-    k_lag_tiled<false><<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups,
-                                                                               c.lag_stages, c.d_tasks, c.d_groups, c.d_lags,
-                                                                               c.totals, c.I2, c.I1, ntiles, c.d_claim);
-  }
+  // some group (other than the one that accumulates the I sums) has whole chunks without a pair in this batch
+  bool skip = false;
+  for (const LagGroup& g : c.groups) skip |= g.flags == 0 && (int64_t)g.tau_min - t0 >= kChunk && (int64_t)g.tau_min <= t0 + b - 1;
+  auto kern = persistent ? (skip ? k_lag_tiled<true, true> : k_lag_tiled<true, false>)
+                         : (skip ? k_lag_tiled<false, true> : k_lag_tiled<false, false>);
+  if (persistent) cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream);
+  kern<<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.lag_stages,
+                                                              c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1, ntiles,
+                                                              c.d_claim);
   return 1;
 }
 
