@@ -479,7 +479,6 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   // batch-relative step from which every lag (j_all) / any lag (j_any) of the task has a frame pair
   const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi - t0));
   const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo - t0));
-  const int t0c = (int)min((int64_t)1 << 30, t0);  // only compared against lags < 2^30 in the warm-up path
   const f2x* oldl = OLD + lane;
 
   int st = 0, slot0 = 0;  // slot0: ring slot of the current item's OLD chunk 0
@@ -731,10 +730,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
   const std::vector<int32_t>& L = c.lags;
   // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
-  #ifndef NFS_LAG_SMEM_DIV
-#define NFS_LAG_SMEM_DIV kLagMinBlocks
-#endif
-  size_t budget = (size_t)std::max(0, smem_sm / NFS_LAG_SMEM_DIV - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
+  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
   budget = std::min(budget, (size_t)c.max_smem_optin);
   // atoms
   std::vector<Atom> atoms;
