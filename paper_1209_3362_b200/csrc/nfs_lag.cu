@@ -880,11 +880,18 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   cudaFuncSetAttribute(k_lag_tiled<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
   const int ngroups = (int)c.groups.size();
   const int ntiles = (int)(c.P / kTilePx);
-  // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold) weighs: batches of one or two
-  // chunks, and two unequal lag groups sharing the device by work.  With many groups, CTAs of the same pixel tile
-  // launched side by side share the NEW frames in L2 and open the same DRAM pages, which measured faster
-  // (config 4: 663 against 852 ms; config 2: 13.95 against 14.18 ms; config 3: 45.0 against 42.5 ms).
-  const bool persistent = c.lag_persistent >= 0 ? c.lag_persistent != 0 : (b <= 2 * kChunk || ngroups == 2);
+  // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold: ~8 us) outweighs its work: batches
+  // of one or two chunks — provided the window prologue of a tile (LEAD steps) hides inside the pipeline depth and
+  // the device is shared by at most two groups.  Measured on the B200 (profiles/r01_summary.md): lags 1..100,
+  // batch 26: 35.8 -> 26.2 ms per 2000 frames; lags 1..208 (two groups): 66.5 -> 51.4 ms.  Elsewhere one CTA per
+  // (tile, group) is as fast or faster: with a long window (isolated far lags) every tile costs LEAD barrier rounds
+  // before its first chunk (lags 1..60 + 9 isolated lags <= 500, batch 26: 67 -> 147 ms); with many groups the
+  // CTAs of a pixel tile launched side by side share the NEW frames in L2 and open the same DRAM pages (config 4:
+  // 663 -> 852 ms); at long batches the fixed cost is amortised anyway (config 2: 13.95 -> 14.18 ms).
+  int max_lead = 0;
+  for (const LagGroup& g : c.groups) max_lead = std::max(max_lead, lag_lead(g.tau_min, g.tau_max));
+  const bool persistent = c.lag_persistent >= 0 ? c.lag_persistent != 0
+                                                : (b <= 2 * kChunk && ngroups <= 2 && max_lead <= c.lag_stages);
   const unsigned grid = persistent ? (unsigned)c.lag_grid : (unsigned)ntiles * (unsigned)ngroups;
   ProfScope ps(c, kKLag);
   // some group (other than the one that accumulates the I sums) has whole chunks without a pair in this batch
