@@ -158,7 +158,7 @@ def run_reference(args, cfg):
     """--impl reference: the CPU oracle on the box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    from paper_1209_3362_b200 import synth
+    import synth
 
     gen = synth.SynthStack(cfg, "cpu")
     n_s = oracle_sample_frames(cfg)
@@ -197,7 +197,7 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
-    from paper_1209_3362_b200 import synth
+    import synth
 
     cfg = synth.config(args.config)
     if args.frames:
@@ -209,7 +209,8 @@ def main():
 
 def run_ours(args, cfg):
     import torch
-    from paper_1209_3362_b200 import binding, synth
+    import synth
+    from paper_1209_3362_b200 import binding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

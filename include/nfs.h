@@ -16,10 +16,12 @@
  *      DC pixel excluded, bin index by exact integer arithmetic                (L25; R6, R7)
  *
  * Every step runs in hand-written CUDA kernels; there is no CPU fallback and no cuFFT.
- * One context = one CUDA stream = not thread-safe; contexts are independent; no global state.
+ * One context = one CUDA device (the one current at nfs_create; later calls switch to it) = one CUDA
+ * stream = not thread-safe; contexts are independent; no global state.
  * All functions return 0 (NFS_OK) or a negative nfs_status; nothing throws or aborts across
- * this boundary.  Errors NFS_ERR_CUDA and NFS_ERR_ZERO_MEAN are sticky: once raised every later
- * call on the context returns them until nfs_reset().
+ * this boundary (a failed host allocation inside the library returns NFS_ERR_OOM).  Errors NFS_ERR_CUDA
+ * and NFS_ERR_ZERO_MEAN are sticky: once raised every later call on the context returns them until
+ * nfs_reset() (which clears NFS_ERR_ZERO_MEAN only; a CUDA error is final).
  */
 #ifndef NFS_H_
 #define NFS_H_
@@ -40,13 +42,15 @@ typedef struct nfs_ctx nfs_ctx; /* opaque, owned by the library */
 
 typedef enum nfs_status {
   NFS_OK = 0,
-  NFS_ERR_INVALID_ARG = -1, /* NULL pointer; W or H not a power of two in [32,4096]; n_lags < 1; lags not
-                               strictly increasing or < 1; n_qbins < 1; n < 1; index out of range   */
+  NFS_ERR_INVALID_ARG = -1, /* NULL pointer; W or H not a power of two in [32,4096]; n_lags < 1 or > 65533; lags
+                               not strictly increasing or < 1; n_qbins < 1; n < 1; d_frames not 16-byte aligned;
+                               index out of range                                                   */
   NFS_ERR_OOM = -2,         /* ring + accumulators do not fit the free device memory (checked at create) */
   NFS_ERR_CUDA = -3,        /* first failing CUDA call (sticky)                                        */
   NFS_ERR_ZERO_MEAN = -4,   /* a pushed frame summed to zero: its normalisation (L21) is undefined.
                                Detected on the device, surfaced by the next synchronising call (sticky) */
-  NFS_ERR_STATE = -5,       /* call not valid in this state (e.g. finalize before any frame)           */
+  NFS_ERR_STATE = -5,       /* call not valid in this state (finalize before any frame; a 2-D difference
+                               spectrum asked of a bin-only context)                                   */
   NFS_ERR_UNSUPPORTED = -6  /* W != H (all of the paper's sizes, L33, are square)                      */
 } nfs_status;
 
@@ -65,14 +69,25 @@ typedef enum nfs_status {
  * pending (and at every finalize/getter).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
  * Whatever the batch, fp32 partial sums never span more than 520 frames before they are folded into
  * the fp64 totals.
+ * nfs_create_opts additionally takes flags:
+ *   NFS_FLAG_BIN_ONLY   keep only the |q|-binned sums of the difference spectra ("store the
+ *                       entire 2D power spectra, which might be unnecessary"): the [n_lags][H][W/2+1] fp64
+ *                       accumulators (4.2 GB for 1000 lags at 1024^2) shrink to a scratch for one group of
+ *                       <= 104 lags plus [n_lags][n_qbins]; nfs_finalize returns the same D, I, counts (same
+ *                       fixed summation order within a bin: run-to-run bit-identical); nfs_get_D2d returns
+ *                       NFS_ERR_STATE.
  */
+#define NFS_FLAG_BIN_ONLY 1u
 NFS_API int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream);
 NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
-                  int batch_frames);
+                          int batch_frames);
+NFS_API int nfs_create_opts(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                            int batch_frames, unsigned flags);
 
 /*
  * nfs_push_frames — steps 1-4 for n more frames.
- *   d_frames  DEVICE [n][H][W] uint16, row-major, x fastest, pitch W, no padding.
+ *   d_frames  DEVICE [n][H][W] uint16, row-major, x fastest, pitch W, no padding, 16-byte aligned (the
+ *             kernels read it with 128-bit loads; anything else returns NFS_ERR_INVALID_ARG).
  * Stream-ordered and asynchronous to the host: d_frames must stay valid and unmodified until the
  * work enqueued by this call on the context's stream has run (record an event after the call).
  * Frames are numbered in push order; results do not depend on how a stack is split across calls
@@ -91,11 +106,13 @@ NFS_API int nfs_push_frames(nfs_ctx* ctx, const uint16_t* d_frames, int n);
  */
 NFS_API int nfs_finalize(nfs_ctx* ctx, double* D_q_tau, double* I_q, int64_t* counts);
 
-/* n_pairs HOST [n_lags]: N - tau, or 0 when tau >= N (N(N-1)/2 pairs over N-1 lags). */
+/* n_pairs HOST [n_lags]: N - tau, or 0 when tau >= N (N(N-1)/2 pairs over N-1 lags).  Host-only;
+ * returns the sticky error of the context if one is set. */
 NFS_API int nfs_get_pair_counts(nfs_ctx* ctx, int64_t* n_pairs);
 
 /* Averaged 2-D spectra on the half plane, HOST [H][W/2+1] double, FFT order (ky = 0..H/2-1,-H/2..-1;
- * kx = 0..W/2), unitary scale (|F(0)|^2 = W*H for a normalised frame).  Synchronise the stream. */
+ * kx = 0..W/2), unitary scale (|F(0)|^2 = W*H for a normalised frame).  Synchronise the stream.
+ * nfs_get_D2d returns NFS_ERR_STATE on a context created with NFS_FLAG_BIN_ONLY. */
 NFS_API int nfs_get_D2d(nfs_ctx* ctx, int lag_index, double* out);
 NFS_API int nfs_get_I2d(nfs_ctx* ctx, double* out);
 
@@ -121,32 +138,33 @@ NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
  * on the context's stream.  nfs_get_kernel_times synchronises, returns the accumulated milliseconds
  * and launch counts per class since the last call — ms/launches are HOST [NFS_NUM_KERNEL_CLASSES], in
  * the order: 0 reference set-up at the first frame (sum, reference image), 1 FFT (one persistent
- * kernel per batch: frame sums, row pass, column pass), 2 I accumulation, 3 lag accumulation,
+ * kernel per batch: frame sums, row pass, column pass), 2 unused, 3 lag accumulation (with the I sums),
  * 4 binning — and clears them. */
 #define NFS_NUM_KERNEL_CLASSES 5
 NFS_API int nfs_set_profiling(nfs_ctx* ctx, int enable);
 NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
 
-/* Lag-accumulation kernel variant: 0 = tiled shared-memory kernel, launch shape chosen per batch (default),
- * 1 = plain per-pixel kernel reading the ring through L1/L2 (kept as an in-library cross-check; same results
- * up to fp32 summation order), 2 = tiled kernel, always one CTA per (pixel tile, lag group), 3 = tiled kernel,
- * always persistent CTAs claiming pixel tiles (2 and 3 give bit-identical results to 0: they only change which
- * CTA handles which tile).  Not a backend switch: all are CUDA kernels of this library. */
-NFS_API int nfs_set_lag_kernel(nfs_ctx* ctx, int variant);
+/* Launch shape of the lag-accumulation kernel: 0 = chosen per batch (default), 1 = always one CTA per (pixel tile,
+ * lag group), 2 = always persistent CTAs that claim pixel tiles.  The same kernel code handles the same tile either
+ * way (results are bit-identical); used by the tests and by bench.py's small-batch measurement. */
+NFS_API int nfs_set_launch_shape(nfs_ctx* ctx, int shape);
 
 /* Host-only introspection of the lag plan of step S5 (which lags are accumulated
  * together); makes no CUDA call, so the host logic is testable without a GPU.  Builds the plan
- * nfs_create would build for `lags` (HOST, strictly increasing, >= 1) on a device with `smem_per_sm`
- * bytes of shared memory per SM and `smem_optin` bytes per CTA, and writes it to out (HOST, cap int32):
- *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA]
+ * nfs_create would build for `lags` (HOST, strictly increasing, >= 1) and frames of n_px Fourier pixels on a
+ * device with n_sm SMs, `smem_per_sm` bytes of shared memory per SM and `smem_optin` bytes per CTA, and writes it
+ * to out (HOST, cap int32):
+ *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA, pixels per tile (32 | 64), CTAs per SM]
  *   per group (23 values): first task, number of tasks, tau_min, tau_max, flags (bit 0: one task of the
- *     group accumulates the I sums), then for consumer warps 0..15 the task (relative) it runs or -1, then the
- *     first persistent CTA of the group and their number (planned here for 2 x 148 resident CTAs)
+ *     group accumulates the I sums; bit 1: single stream, the batch's frames are the head of the window),
+ *     then for task slots 0..15 the task (relative) a consumer warp of that slot runs or -1, then the
+ *     first persistent CTA of the group and their number
  *   per task (4 values): smallest lag, number of lags, index of its first lag in `lags`, kind (bit 0:
  *     0 = run of consecutive lags on the register-window path, 1 = lag list; bit 1: also accumulates I)
  * Returns the number of int32 written (> 0), or NFS_ERR_INVALID_ARG (bad list, cap too small, a single
  * task's lag span exceeding shared memory). */
-NFS_API int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_optin, int32_t* out, int cap);
+NFS_API int nfs_plan_lags(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,
+                          int cap);
 
 /* Forget all frames (accumulators, ring, reference, sticky errors); keeps the plan and the memory. */
 NFS_API int nfs_reset(nfs_ctx* ctx);

@@ -29,6 +29,11 @@
  *   7. V2d(k) = (1/N) sum_t |F_t(k) - <F(k)>_t|^2 and its azimuthal mean: see
  *        nfso_variance_spectrum below.
  *
+ * nfso_structure_function_half is the same definition evaluated on the half plane kx <= W/2 only (the other
+ * half is its Hermitian mirror, the image being real; SURVEY.md 8(c) "half-plane fast variant", pin P11: equal
+ * to the full-plane function to 1e-12 on configs 0 and 1).  It exists so that the full-size parity tests of
+ * BASELINE.json configs 1-4 finish in minutes; the timed cpu_baseline stays the full-plane function.
+ *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force DFT, numpy.fft, Parseval,
  * constant stack, gain invariance, travelling plane wave closed form, telegraph stack, ramp,
  * linearity (real-space difference then DFT), white noise D = 2 sigma^2 = 2 I, bin-count brute
@@ -222,6 +227,18 @@ void nfso_azimuthal_mean(const double* map2d, int W, int H, int n_b, double* out
 
 #define PIX_TILE 256
 
+/* wall-clock seconds of the two stages of the last nfso_structure_function call (bench.py's cpu_baseline
+ * reports them): [0] steps 1-2 (normalise + transform), [1] steps 3-4 (pair loop, I2d). */
+static double g_stage_seconds[2] = {0.0, 0.0};
+static double now_seconds(void) {
+#ifdef _OPENMP
+  return omp_get_wtime();
+#else
+  return 0.0;
+#endif
+}
+void nfso_last_stage_seconds(double* out2) { out2[0] = g_stage_seconds[0]; out2[1] = g_stage_seconds[1]; }
+
 /*
  * frames  [N][H][W] uint16 row-major.        lags [n_lags] (>=1, strictly increasing).
  * D       [n_lags][n_b]   azimuthal means of D2d.    I_q [n_b].   counts [n_b].
@@ -239,14 +256,20 @@ int nfso_structure_function(const uint16_t* frames, int N, int W, int H, const i
   cplx* F = (cplx*)malloc(sizeof(cplx) * (size_t)N * P);
   double* D2d = D2d_out ? D2d_out : (double*)malloc(sizeof(double) * (size_t)n_lags * P);
   double* I2d = I2d_out ? I2d_out : (double*)malloc(sizeof(double) * (size_t)P);
-  if (!F || !D2d || !I2d) return NFSO_ERR_MEM;
+  if (!F || !D2d || !I2d) {
+    free(F);
+    if (!D2d_out) free(D2d);
+    if (!I2d_out) free(I2d);
+    return NFSO_ERR_MEM;
+  }
   int rc_all = NFSO_OK;
+  const double t_start = now_seconds();
 
   /* steps 1-2: every frame is normalised and transformed exactly once (L31) */
 #pragma omp parallel for schedule(dynamic, 1)
   for (int t = 0; t < N; ++t) {
     double* tmp = (double*)malloc(sizeof(double) * (size_t)P);
-    int rc = transform_frame(frames + (size_t)t * P, W, H, method, tmp, F + (size_t)t * P);
+    int rc = tmp ? transform_frame(frames + (size_t)t * P, W, H, method, tmp, F + (size_t)t * P) : NFSO_ERR_MEM;
     if (rc) {
 #pragma omp critical
       rc_all = rc;
@@ -254,6 +277,7 @@ int nfso_structure_function(const uint16_t* frames, int N, int W, int H, const i
     free(tmp);
   }
   if (rc_all) { free(F); if (!D2d_out) free(D2d); if (!I2d_out) free(I2d); return rc_all; }
+  const double t_fft = now_seconds();
 
   /* step 3: explicit pair loop, pixel-tiled */
   memset(D2d, 0, sizeof(double) * (size_t)n_lags * P);
@@ -287,6 +311,8 @@ int nfso_structure_function(const uint16_t* frames, int N, int W, int H, const i
     }
     I2d[k] = s / (double)N;
   }
+  g_stage_seconds[0] = t_fft - t_start;
+  g_stage_seconds[1] = now_seconds() - t_fft;
 
   /* steps 5-6 */
   for (int l = 0; l < n_lags; ++l) azimuthal_mean(D2d + (size_t)l * P, W, H, n_b, D + (size_t)l * n_b, NULL);
@@ -296,6 +322,125 @@ int nfso_structure_function(const uint16_t* frames, int N, int W, int H, const i
   if (!D2d_out) free(D2d);
   if (!I2d_out) free(I2d);
   return NFSO_OK;
+}
+
+/* ---- steps 1-6 on the half plane kx = 0..W/2 ("half-plane fast variant", pin P11) -------------
+ *
+ * The image is real, so F_t(W-kx, H-ky) = conj F_t(kx, ky): every full-plane pixel with kx > W/2 repeats the
+ * value |.|^2 of its mirror with kx < W/2, which lies at the same |q| and therefore in the same bin.  The
+ * definition is evaluated for kx <= W/2 only and a bin mean weights the columns 0 < kx < W/2 twice (columns 0
+ * and W/2 map onto themselves): c_b and the sums are those of the full plane.
+ * Every frame is still normalised and transformed in full (steps 1-2, the same transform_frame); the explicit
+ * pair loop (step 3) runs pixel tile by pixel tile over a contiguous copy of the tile's time series (loop order
+ * and memory management only).  Memory: N * H * (W/2+1) complex128.
+ *
+ * D [n_lags][n_b], I_q [n_b], counts [n_b], n_pairs [n_lags] as in nfso_structure_function.
+ * D2d_out optional [n_lags][H][W/2+1], I2d_out optional [H][W/2+1]  (half plane, FFT order). */
+int nfso_structure_function_half(const uint16_t* frames, int N, int W, int H, const int32_t* lags, int n_lags,
+                                 int n_b, double* D, double* I_q, int64_t* counts, int64_t* n_pairs,
+                                 double* D2d_out, double* I2d_out) {
+  if (!frames || !lags || N < 1 || W < 2 || H < 1 || n_lags < 1 || n_b < 1) return NFSO_ERR_ARG;
+  for (int l = 0; l < n_lags; ++l)
+    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return NFSO_ERR_ARG;
+  const long P = (long)W * H;
+  const int Wh = W / 2 + 1;
+  const long Ph = (long)Wh * H;
+  cplx* F = (cplx*)malloc(sizeof(cplx) * (size_t)N * Ph); /* [t][ky][kx <= W/2] */
+  double* D2d = D2d_out ? D2d_out : (double*)malloc(sizeof(double) * (size_t)n_lags * Ph);
+  double* I2d = I2d_out ? I2d_out : (double*)malloc(sizeof(double) * (size_t)Ph);
+  int rc_all = (F && D2d && I2d) ? NFSO_OK : NFSO_ERR_MEM;
+
+  /* steps 1-2: every frame normalised and transformed exactly once, in full; the half plane is kept */
+  if (!rc_all) {
+#pragma omp parallel
+    {
+      double* tmp = (double*)malloc(sizeof(double) * (size_t)P);
+      cplx* Ff = (cplx*)malloc(sizeof(cplx) * (size_t)P);
+#pragma omp for schedule(dynamic, 1)
+      for (int t = 0; t < N; ++t) {
+        int rc = (tmp && Ff) ? transform_frame(frames + (size_t)t * P, W, H, 0, tmp, Ff) : NFSO_ERR_MEM;
+        if (rc) {
+#pragma omp critical
+          rc_all = rc;
+          continue;
+        }
+        for (int ky = 0; ky < H; ++ky)
+          for (int kx = 0; kx < Wh; ++kx) F[(size_t)t * Ph + (long)ky * Wh + kx] = Ff[(long)ky * W + kx];
+      }
+      free(tmp);
+      free(Ff);
+    }
+  }
+
+  /* steps 3-4: explicit pair loop over a contiguous copy of each pixel tile's time series.  The tile is sized
+   * so that the copy (N * tile complex128) stays in a core's cache. */
+  if (!rc_all) {
+    long tile = (long)(1 << 20) / (16L * N);
+    if (tile > PIX_TILE) tile = PIX_TILE;
+    if (tile < 4) tile = 4;
+#pragma omp parallel
+    {
+      cplx* ts = (cplx*)malloc(sizeof(cplx) * (size_t)N * tile); /* [t][k - k0] */
+      double* acc = (double*)malloc(sizeof(double) * (size_t)tile);
+#pragma omp for schedule(dynamic, 1)
+      for (long k0 = 0; k0 < Ph; k0 += tile) {
+        if (!ts || !acc) {
+#pragma omp critical
+          rc_all = NFSO_ERR_MEM;
+          continue;
+        }
+        const long nk = k0 + tile < Ph ? tile : Ph - k0;
+        for (int t = 0; t < N; ++t)
+          for (long k = 0; k < nk; ++k) ts[(size_t)t * tile + k] = F[(size_t)t * Ph + k0 + k];
+        for (int l = 0; l < n_lags; ++l) {
+          const int tau = lags[l];
+          for (long k = 0; k < nk; ++k) acc[k] = 0.0;
+          for (int t = 0; t + tau < N; ++t) {
+            const cplx* a = ts + (size_t)t * tile;
+            const cplx* b = ts + (size_t)(t + tau) * tile;
+            for (long k = 0; k < nk; ++k) {
+              cplx d = a[k] - b[k];
+              acc[k] += creal(d) * creal(d) + cimag(d) * cimag(d);
+            }
+          }
+          for (long k = 0; k < nk; ++k) D2d[(size_t)l * Ph + k0 + k] = tau < N ? acc[k] / (double)(N - tau) : 0.0;
+        }
+        for (long k = 0; k < nk; ++k) acc[k] = 0.0;
+        for (int t = 0; t < N; ++t)
+          for (long k = 0; k < nk; ++k) {
+            cplx f = ts[(size_t)t * tile + k];
+            acc[k] += creal(f) * creal(f) + cimag(f) * cimag(f);
+          }
+        for (long k = 0; k < nk; ++k) I2d[k0 + k] = acc[k] / (double)N;
+      }
+      free(ts);
+      free(acc);
+    }
+  }
+
+  /* steps 5-6 with the Hermitian weights: 2 for 0 < kx < W/2, 1 for kx = 0 and kx = W/2 */
+  if (!rc_all) {
+    for (int l = 0; l < n_lags; ++l) n_pairs[l] = lags[l] < N ? (int64_t)(N - lags[l]) : 0;
+    for (int row = 0; row <= n_lags; ++row) {
+      const double* map = row < n_lags ? D2d + (size_t)row * Ph : I2d;
+      double* out = row < n_lags ? D + (size_t)row * n_b : I_q;
+      for (int b = 0; b < n_b; ++b) { out[b] = 0.0; counts[b] = 0; }
+      for (int ky = 0; ky < H; ++ky)
+        for (int kx = 0; kx < Wh; ++kx) {
+          int b = nfso_qbin(kx, ky, W, H, n_b);
+          if (b < 0) continue;
+          int w = (kx == 0 || 2 * kx == W) ? 1 : 2;
+          out[b] += (double)w * map[(long)ky * Wh + kx];
+          counts[b] += w;
+        }
+      for (int b = 0; b < n_b; ++b)
+        if (counts[b] > 0) out[b] /= (double)counts[b];
+    }
+  }
+  free(F);
+  if (!D2d_out) free(D2d);
+  if (!I2d_out) free(I2d);
+  return rc_all;
 }
 
 /* ---- variance form of the static-free spectrum (reading R9b) ------------

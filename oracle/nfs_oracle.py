@@ -113,6 +113,34 @@ def structure_function(frames, lags, n_b, method=0, want_2d=False, windowed=Fals
     return Result(D=D, I_q=I_q, counts=cnt, n_pairs=npairs, D2d=D2d, I2d=I2d)
 
 
+def structure_function_half(frames, lags, n_b, want_2d=False):
+    """The definition on the half plane kx <= W/2 (Hermitian weights in the bin means; pin P11: equal to
+    structure_function).  Returns Result(D, I_q, counts, n_pairs, D2d [n_l][H][W/2+1] or None, I2d [H][W/2+1] or None)."""
+    f = _frames(frames)
+    N, H, W = f.shape
+    lg = np.ascontiguousarray(lags, dtype=np.int32)
+    n_l = lg.size
+    D = np.zeros((n_l, n_b), dtype=np.float64)
+    I_q = np.zeros(n_b, dtype=np.float64)
+    cnt = np.zeros(n_b, dtype=np.int64)
+    npairs = np.zeros(n_l, dtype=np.int64)
+    D2d = np.zeros((n_l, H, W // 2 + 1), dtype=np.float64) if want_2d else None
+    I2d = np.zeros((H, W // 2 + 1), dtype=np.float64) if want_2d else None
+    rc = lib().nfso_structure_function_half(
+        _p(f, C.c_uint16), N, W, H, _p(lg, C.c_int32), n_l, int(n_b), _p(D, C.c_double), _p(I_q, C.c_double),
+        _p(cnt, C.c_int64), _p(npairs, C.c_int64), _p(D2d, C.c_double), _p(I2d, C.c_double))
+    if rc:
+        raise RuntimeError("oracle structure_function_half rc=%d" % rc)
+    return Result(D=D, I_q=I_q, counts=cnt, n_pairs=npairs, D2d=D2d, I2d=I2d)
+
+
+def last_stage_seconds():
+    """(seconds of steps 1-2, seconds of steps 3-4) of the last structure_function call."""
+    out = (C.c_double * 2)()
+    lib().nfso_last_stage_seconds(out)
+    return float(out[0]), float(out[1])
+
+
 def structure_function_sampled(frames, lags, sample_ky, sample_kx):
     """The definition restricted to sampled Fourier pixels (full transform of every frame).
 

@@ -25,6 +25,7 @@ _P = C.c_void_p
 SYMBOLS = [
     ("nfs_create", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P]),
     ("nfs_create_ex", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int]),
+    ("nfs_create_opts", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int, C.c_uint]),
     ("nfs_push_frames", C.c_int, [_P, _P, C.c_int]),
     ("nfs_finalize", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_get_pair_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
@@ -36,8 +37,8 @@ SYMBOLS = [
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
     ("nfs_num_launches", C.c_int64, [_P]),
-    ("nfs_set_lag_kernel", C.c_int, [_P, C.c_int]),
-    ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
+    ("nfs_set_launch_shape", C.c_int, [_P, C.c_int]),
+    ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
     ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
     ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_reset", C.c_int, [_P]),
@@ -46,7 +47,9 @@ SYMBOLS = [
     ("nfs_last_cuda_error", C.c_char_p, [_P]),
 ]
 
-KERNEL_CLASSES = ["ref_setup", "fft", "accum_I", "lag_accum", "bin"]
+KERNEL_CLASSES = ["ref_setup", "fft", "unused", "lag_accum", "bin"]
+NFS_FLAG_BIN_ONLY = 1
+SHAPE_AUTO, SHAPE_ONE_TILE, SHAPE_PERSISTENT = 0, 1, 2
 
 _lib = None
 
@@ -88,11 +91,11 @@ def _dp(a, t):
 
 
 # ---- functions with the C names -----------------------------------------------------------------------
-def nfs_create(W, H, lags, n_qbins, cuda_stream=None, batch_frames=0):
+def nfs_create(W, H, lags, n_qbins, cuda_stream=None, batch_frames=0, flags=0):
     lg = np.ascontiguousarray(lags, dtype=np.int32)
     h = _P()
-    rc = load_library().nfs_create_ex(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins),
-                                      _P(cuda_stream) if cuda_stream else None, int(batch_frames))
+    rc = load_library().nfs_create_opts(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins),
+                                        _P(cuda_stream) if cuda_stream else None, int(batch_frames), int(flags))
     _check(rc)
     return h
 
@@ -109,16 +112,18 @@ def nfs_finalize(handle, n_lags, n_qbins):
     return D, I_q, cnt
 
 
-def nfs_plan_lags(lags, smem_per_sm=233472, smem_optin=232448):
-    """Host-only lag plan (no CUDA call): dict(stages, smem, groups=[...], tasks=[...]); see include/nfs.h."""
+def nfs_plan_lags(lags, n_px=1024 * 513, smem_per_sm=233472, smem_optin=232448, n_sm=148):
+    """Host-only lag plan (no CUDA call): dict(stages, smem, tile_px, ctas_per_sm, groups=[...], tasks=[...]); see
+    include/nfs.h."""
     lags = np.ascontiguousarray(lags, dtype=np.int32)
-    cap = 4 + 27 * (len(lags) + 1)
+    cap = 6 + 27 * (len(lags) + 1)
     out = np.zeros(cap, dtype=np.int32)
-    n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(smem_per_sm), int(smem_optin), _dp(out, C.c_int32), cap)
+    n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(n_px), int(smem_per_sm), int(smem_optin), int(n_sm),
+                                     _dp(out, C.c_int32), cap)
     if n < 0:
         raise NFSError(n)
-    ng, nt, stages, smem = (int(v) for v in out[:4])
-    o = 4
+    ng, nt, stages, smem, tile_px, per_sm = (int(v) for v in out[:6])
+    o = 6
     groups, tasks = [], []
     for _ in range(ng):
         g = out[o:o + 23]
@@ -129,7 +134,7 @@ def nfs_plan_lags(lags, smem_per_sm=233472, smem_optin=232448):
         t = out[o:o + 4]
         tasks.append(dict(tau0=int(t[0]), cnt=int(t[1]), l0=int(t[2]), kind=int(t[3])))
         o += 4
-    return dict(stages=stages, smem=smem, groups=groups, tasks=tasks)
+    return dict(stages=stages, smem=smem, tile_px=tile_px, ctas_per_sm=per_sm, groups=groups, tasks=tasks)
 
 
 def nfs_destroy(handle):
@@ -138,21 +143,40 @@ def nfs_destroy(handle):
 
 # ---- convenience wrapper ----------------------------------------------------------------------------------
 class NFS:
-    """One context.  `push(frames)` takes a CUDA uint16 torch tensor [n][H][W] (contiguous)."""
+    """One context on a torch CUDA stream.  `push(frames)` takes a CUDA uint16 torch tensor [n][H][W] (contiguous).
 
-    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0):
+    The context's work is enqueued on `stream` (default: a stream of its own).  push() orders that stream after the
+    work already enqueued on torch's current stream (so a tensor written just before the call is complete when the
+    kernels read it) and tells the caching allocator that the tensor is in use on the context's stream (so a
+    temporary passed to push() is not recycled while the kernels still read it): include/nfs.h puts both duties on
+    the caller of nfs_push_frames."""
+
+    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False):
+        import torch
+
         self.lib = load_library()
         self.W, self.H, self.n_qbins = int(W), int(H), int(n_qbins)
         self.lags = [int(t) for t in lags]
-        self._stream = stream  # torch.cuda.Stream or None (library-owned stream)
-        self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None,
-                                 batch_frames)
+        self.bin_only = bool(bin_only)
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.Stream()
+        self._stream = stream  # without a device nfs_create itself reports NFS_ERR_CUDA: no fallback
+        self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None, batch_frames,
+                                 NFS_FLAG_BIN_ONLY if bin_only else 0)
+
+    @property
+    def stream(self):
+        return self._stream
 
     def push(self, frames):
         import torch
 
         assert frames.is_cuda and frames.dtype == torch.uint16 and frames.is_contiguous()
         assert frames.dim() == 3 and frames.shape[1] == self.H and frames.shape[2] == self.W
+        cur = torch.cuda.current_stream(frames.device)
+        if cur != self._stream:
+            self._stream.wait_stream(cur)
+            frames.record_stream(self._stream)
         nfs_push_frames(self.handle, frames.data_ptr(), frames.shape[0])
 
     def push_ptr(self, ptr, n):
@@ -186,8 +210,8 @@ class NFS:
         _check(self.lib.nfs_get_V2d(self.handle, _dp(out, C.c_double)), self.handle)
         return out
 
-    def set_lag_kernel(self, variant):
-        _check(self.lib.nfs_set_lag_kernel(self.handle, int(variant)), self.handle)
+    def set_launch_shape(self, shape):
+        _check(self.lib.nfs_set_launch_shape(self.handle, int(shape)), self.handle)
 
     def set_profiling(self, enable):
         _check(self.lib.nfs_set_profiling(self.handle, int(bool(enable))), self.handle)

@@ -29,25 +29,23 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, out: str = LIB, defines=()) -> str:
-    """Compiles the four .cu files and links `out`.  `defines` (e.g. ["NFS_LAG_STAGES=3"]) overrides the
-    tuning constants of nfs_common.cuh / nfs_fft.cu for experiments; the default build passes none."""
-    if not force and out == LIB and not defines and not needs_build():
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compiles the four .cu files (in parallel) and links libnfs_b200.so beside this file."""
+    if not force and not needs_build():
         return LIB
-    objs = []
-    tag = "" if out == LIB else "." + os.path.basename(out)
+    objs, procs = [], []
     for s in SOURCES:
-        o = os.path.join(CSRC, s.replace(".cu", tag + ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else [])
-        subprocess.check_call(cmd + ["-c", os.path.join(CSRC, s), "-o", o])
+        o = os.path.join(CSRC, s.replace(".cu", ".o"))
+        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
+        procs.append((s, subprocess.Popen(cmd + ["-c", os.path.join(CSRC, s), "-o", o])))
         objs.append(o)
-    tmp = out + ".tmp.%d" % os.getpid()
+    failed = [s for s, p in procs if p.wait() != 0]
+    if failed:
+        raise RuntimeError("nvcc failed on " + ", ".join(failed))
+    tmp = LIB + ".tmp.%d" % os.getpid()
     subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs)
-    os.replace(tmp, out)
-    if out != LIB:
-        for o in objs:
-            os.remove(o)
-    return out
+    os.replace(tmp, LIB)
+    return LIB
 
 
 if __name__ == "__main__":

@@ -20,19 +20,6 @@ namespace {
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
-// record the first CUDA error (sticky)
-bool cuda_ok(Ctx& c, cudaError_t e, const char* what) {
-  if (e == cudaSuccess) return true;
-  if (c.status == NFS_OK) {
-    c.status = NFS_ERR_CUDA;
-    c.cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
-  }
-  return false;
-}
-#define NFS_CUDA(c, call) cuda_ok((c), (call), #call)
-
-bool check_launch(Ctx& c, const char* what) { return cuda_ok(c, cudaGetLastError(), what); }
-
 template <typename T>
 bool dev_alloc(Ctx& c, T** p, size_t count) {
   void* q = nullptr;
@@ -43,26 +30,32 @@ bool dev_alloc(Ctx& c, T** p, size_t count) {
   return true;
 }
 
-uint64_t isqrt_u64(uint64_t v) {
-  uint64_t r = (uint64_t)sqrt((double)v);
-  while (r * r > v) --r;
-  while ((r + 1) * (r + 1) <= v) ++r;
-  return r;
-}
-
-// |q| bin of half-plane pixel (kx in [0, W/2], ky in [0, H)) by exact integer arithmetic (reading R6):
-// b = isqrt(floor(4 nb^2 (kx'^2 H^2 + ky'^2 W^2) / (W^2 H^2))); DC and b >= nb excluded (-1).
-int qbin_of(int kx, int ky, int W, int H, int nb) {
-  const int64_t sx = kx;  // kx <= W/2; the Nyquist index has |kx'| = W/2
-  const int64_t sy = ky < H / 2 ? ky : ky - H;
-  if (sx == 0 && sy == 0) return -1;
-  const unsigned __int128 num = (unsigned __int128)(4ull * (uint64_t)nb * (uint64_t)nb) *
-                                ((unsigned __int128)((uint64_t)(sx * sx) * (uint64_t)H * (uint64_t)H) +
-                                 (unsigned __int128)((uint64_t)(sy * sy) * (uint64_t)W * (uint64_t)W));
-  const unsigned __int128 den = (unsigned __int128)((uint64_t)W * (uint64_t)W) * ((uint64_t)H * (uint64_t)H);
-  const uint64_t b = isqrt_u64((uint64_t)(num / den));
-  return b >= (uint64_t)nb ? -1 : (int)b;
-}
+// |q| bins of the half plane (reading R6: b = floor(n_b |q| / q_Nyquist), uniform half-open bins on [0, pi) rad/px).
+// A pixel with signed FFT-order indices (sx, sy) has (|q| / q_Nyquist)^2 = 4 (sx^2 H^2 + sy^2 W^2) / (W^2 H^2); it
+// lies in bin b iff  b^2 W^2 H^2 <= 4 n_b^2 (sx^2 H^2 + sy^2 W^2) < (b + 1)^2 W^2 H^2.  The lower edges
+// edge[b] = b^2 W^2 H^2 are tabulated once in 128-bit integers and a pixel's bin is found by bisection on them:
+// exact, no division, no square root.
+typedef unsigned __int128 u128;
+struct BinEdges {
+  std::vector<u128> edge;  // [n_b + 1]
+  u128 scale;              // 4 n_b^2
+  BinEdges(int W, int H, int nb) : edge((size_t)nb + 1), scale((u128)4 * (u128)nb * (u128)nb) {
+    const u128 wh2 = (u128)((uint64_t)W * (uint64_t)W) * (u128)((uint64_t)H * (uint64_t)H);
+    for (int b = 0; b <= nb; ++b) edge[(size_t)b] = (u128)((uint64_t)b * (uint64_t)b) * wh2;
+  }
+  // m = sx^2 H^2 + sy^2 W^2 (< 2^47 for frames up to 4096^2).  Returns -1 for the DC pixel and beyond the last edge.
+  int bin_of(uint64_t m) const {
+    if (m == 0) return -1;
+    const u128 v = scale * (u128)m;
+    if (v >= edge.back()) return -1;
+    size_t lo = 0, hi = edge.size() - 1;  // invariant: edge[lo] <= v < edge[hi]
+    while (hi - lo > 1) {
+      const size_t mid = (lo + hi) / 2;
+      (edge[mid] <= v ? lo : hi) = mid;
+    }
+    return (int)lo;
+  }
+};
 
 // host tables: twiddles, bin map, lag plan
 bool build_tables(Ctx& c) {
@@ -100,47 +93,42 @@ bool build_tables(Ctx& c) {
     }
   }
 
-  // bin map in ring layout: p = kx*H + ky
-  std::vector<int32_t> start(nb + 1, 0);
-  c.counts.assign(nb, 0);
-  std::vector<int32_t> binof((size_t)c.P);
-  for (int ky = 0; ky < H; ++ky)
+  // bin map in ring layout p = kx*H + ky: pixels grouped by bin in ascending p (fixed order, good locality), each
+  // entry carrying its Hermitian weight: the columns 0 < kx < W/2 stand for two pixels of the full plane
+  {
+    const BinEdges edges(W, H, nb);
+    const uint64_t H2 = (uint64_t)H * (uint64_t)H, W2 = (uint64_t)W * (uint64_t)W;
+    std::vector<int32_t> binof((size_t)c.P);
+    std::vector<int32_t> start((size_t)nb + 1, 0);
+    c.counts.assign((size_t)nb, 0);
     for (int kx = 0; kx <= n; ++kx) {
-      const int64_t p = (int64_t)kx * H + ky;
-      const int b = qbin_of(kx, ky, W, H, nb);
-      binof[p] = b;
-      if (b >= 0) {
-        start[b + 1] += 1;
-        c.counts[b] += (kx == 0 || kx == n) ? 1 : 2;
+      const uint64_t mx = (uint64_t)kx * (uint64_t)kx * H2;  // the Nyquist column kx = W/2 has |sx| = W/2
+      for (int ky = 0; ky < H; ++ky) {
+        const uint64_t ay = (uint64_t)std::min(ky, H - ky);  // |sy| of FFT-order index ky
+        const int b = edges.bin_of(mx + ay * ay * W2);
+        binof[(size_t)kx * H + ky] = b;
+        if (b < 0) continue;
+        start[(size_t)b + 1] += 1;
+        c.counts[(size_t)b] += (kx == 0 || kx == n) ? 1 : 2;
       }
     }
-  for (int b = 0; b < nb; ++b) start[b + 1] += start[b];
-  std::vector<uint32_t> perm((size_t)start[nb] ? (size_t)start[nb] : 1);
-  {
+    for (int b = 0; b < nb; ++b) start[(size_t)b + 1] += start[(size_t)b];
+    std::vector<uint32_t> perm((size_t)start[(size_t)nb] ? (size_t)start[(size_t)nb] : 1);
     std::vector<int32_t> fill(start.begin(), start.end() - 1);
-    for (int64_t p = 0; p < c.P; ++p) {  // ascending p inside each bin: fixed order, good locality
-      const int b = binof[p];
+    for (int64_t p = 0; p < c.P; ++p) {
+      const int b = binof[(size_t)p];
       if (b < 0) continue;
-      const bool interior = p >= (int64_t)H && p < (int64_t)H * n;  // 0 < kx < n: Hermitian weight 2
-      perm[fill[b]++] = (uint32_t)p | (interior ? 0x80000000u : 0u);
+      const bool twice = p >= (int64_t)H && p < (int64_t)H * n;  // 0 < kx < n
+      perm[(size_t)fill[(size_t)b]++] = (uint32_t)p | (twice ? 0x80000000u : 0u);
     }
+    if (!dev_alloc(c, &c.perm, perm.size())) return false;
+    if (!dev_alloc(c, &c.bin_start, (size_t)nb + 1)) return false;
+    if (!NFS_CUDA(c, cudaMemcpy(c.perm, perm.data(), sizeof(uint32_t) * perm.size(), cudaMemcpyHostToDevice))) return false;
+    if (!NFS_CUDA(c, cudaMemcpy(c.bin_start, start.data(), sizeof(int32_t) * ((size_t)nb + 1), cudaMemcpyHostToDevice)))
+      return false;
   }
-  if (!dev_alloc(c, &c.perm, perm.size())) return false;
-  if (!dev_alloc(c, &c.bin_start, (size_t)nb + 1)) return false;
-  if (!NFS_CUDA(c, cudaMemcpy(c.perm, perm.data(), sizeof(uint32_t) * perm.size(), cudaMemcpyHostToDevice))) return false;
-  if (!NFS_CUDA(c, cudaMemcpy(c.bin_start, start.data(), sizeof(int32_t) * (nb + 1), cudaMemcpyHostToDevice)))
-    return false;
 
-  // lag plan (nfs_lag.cu): tasks per consumer warp, groups per CTA, pipeline depth
-  const std::vector<int32_t>& L = c.lags;
-  int dev = 0, smem_sm = 0, n_sm = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
-  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  if (!lag_plan(c, smem_sm, kLagMinBlocks * std::max(1, n_sm), (int)(c.P / kTilePx))) {
-    c.status = NFS_ERR_INVALID_ARG;
-    return false;
-  }
+  // lag plan tables (nfs_lag.cu)
   if (!dev_alloc(c, &c.d_tasks, c.tasks.size())) return false;
   if (!dev_alloc(c, &c.d_groups, c.groups.size())) return false;
   if (!dev_alloc(c, &c.d_claim, c.groups.size())) return false;
@@ -149,13 +137,13 @@ bool build_tables(Ctx& c) {
     return false;
   if (!NFS_CUDA(c, cudaMemcpy(c.d_groups, c.groups.data(), sizeof(LagGroup) * c.groups.size(), cudaMemcpyHostToDevice)))
     return false;
-  if (!NFS_CUDA(c, cudaMemcpy(c.d_lags, L.data(), sizeof(int32_t) * c.n_lags, cudaMemcpyHostToDevice))) return false;
+  if (!NFS_CUDA(c, cudaMemcpy(c.d_lags, c.lags.data(), sizeof(int32_t) * c.n_lags, cudaMemcpyHostToDevice))) return false;
   return true;
 }
 
 void free_all(Ctx& c) {
-  void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.I2,      c.I1,      c.sums,     c.tw,     c.tw_out,
-                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags, c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim};
+  void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.totals_b, c.I2,      c.I1,       c.sums,    c.tw,     c.tw_out,
+                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
@@ -163,9 +151,13 @@ void free_all(Ctx& c) {
   if (c.own_stream && c.stream) cudaStreamDestroy(c.stream);
 }
 
+size_t totals_rows(const Ctx& c) { return (size_t)(c.bin_only ? c.max_group_lags : c.n_lags); }
+
 bool zero_state(Ctx& c) {
   bool ok = true;
-  ok &= NFS_CUDA(c, cudaMemsetAsync(c.totals, 0, sizeof(double) * (size_t)c.n_lags * c.P, c.stream));
+  ok &= NFS_CUDA(c, cudaMemsetAsync(c.totals, 0, sizeof(double) * totals_rows(c) * c.P, c.stream));
+  if (c.bin_only)
+    ok &= NFS_CUDA(c, cudaMemsetAsync(c.totals_b, 0, sizeof(double) * (size_t)c.n_lags * c.n_qbins, c.stream));
   ok &= NFS_CUDA(c, cudaMemsetAsync(c.I2, 0, sizeof(double) * (size_t)c.P, c.stream));
   ok &= NFS_CUDA(c, cudaMemsetAsync(c.I1, 0, sizeof(double2) * (size_t)c.P, c.stream));
   ok &= NFS_CUDA(c, cudaMemsetAsync(c.d_flags, 0, sizeof(int), c.stream));
@@ -173,6 +165,15 @@ bool zero_state(Ctx& c) {
   c.n_acc = 0;
   c.n_launches = 0;
   return ok;
+}
+
+// every entry point that touches the device runs on the context's device
+bool enter(Ctx& c) {
+  if (c.status != NFS_OK) return false;
+  int dev = -1;
+  if (!NFS_CUDA(c, cudaGetDevice(&dev))) return false;
+  if (dev != c.device && !NFS_CUDA(c, cudaSetDevice(c.device))) return false;
+  return true;
 }
 
 // synchronise and surface device-side flags
@@ -192,36 +193,34 @@ void ring_to_plane(const Ctx& c, const double* src, double* out) {
     for (int x = 0; x <= n; ++x) out[(size_t)y * (n + 1) + x] = src[(size_t)x * H + y];
 }
 
-// steps S5 (+ the I accumulators) for the frames transformed since the last accumulation
+// step S5 (+ the I accumulators) for the frames transformed since the last accumulation
 bool flush_pending(Ctx& c) {
   const int b = (int)(c.n_frames - c.n_acc);
   if (b <= 0) return true;
-  if (c.lag_variant == 1) {  // in-library cross-check path: plain kernels
-    c.n_launches += launch_accum_I(c, c.n_acc, b);
-    c.n_launches += launch_lag_simple(c, c.n_acc, b);
-  } else {  // k_lag_tiled also accumulates the I sums of the batch
-    c.n_launches += launch_lag_tiled(c, c.n_acc, b);
-  }
-  if (!check_launch(c, "lag launch")) return false;
+  c.n_launches += launch_lag_tiled(c, c.n_acc, b);
+  if (!NFS_CUDA(c, cudaGetLastError())) return false;
+  if (c.status != NFS_OK) return false;
   c.n_acc = c.n_frames;
   return true;
 }
 
-}  // namespace
+bool lags_ok(const int32_t* lags, int n_lags) {
+  if (!lags || n_lags < 1) return false;
+  for (int l = 0; l < n_lags; ++l)
+    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return false;
+  return true;
+}
 
-extern "C" {
-
-int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
-                  int batch_frames) {
+int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream, int batch_frames,
+                unsigned flags) {
   if (!out) return NFS_ERR_INVALID_ARG;
   *out = nullptr;
-  if (!lags || n_lags < 1 || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
+  if (!lags_ok(lags, n_lags) || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
     return NFS_ERR_INVALID_ARG;
+  if ((flags & ~(unsigned)NFS_FLAG_BIN_ONLY) != 0) return NFS_ERR_INVALID_ARG;
   if (!is_pow2(W) || !is_pow2(H) || W < 32 || H < 32 || W > 4096 || H > 4096) return NFS_ERR_INVALID_ARG;
   if (W != H) return NFS_ERR_UNSUPPORTED;
-  for (int l = 0; l < n_lags; ++l)
-    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return NFS_ERR_INVALID_ARG;
-  if (n_lags > 65535 * kG) return NFS_ERR_INVALID_ARG;
+  if (n_lags > 65533) return NFS_ERR_INVALID_ARG;  // one grid row of the binning kernel per lag (+ I and V)
 
   nfs_ctx* h = new (std::nothrow) nfs_ctx();
   if (!h) return NFS_ERR_OOM;
@@ -236,76 +235,125 @@ int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, 
   c.Lmax = lags[n_lags - 1];
   c.B = batch_frames > 0 ? batch_frames : 1024;
   c.R = c.Lmax + c.B;
+  c.bin_only = (flags & NFS_FLAG_BIN_ONLY) != 0;
 
-  int dev = 0;
-  if (!NFS_CUDA(c, cudaGetDevice(&dev))) goto fail;
-  cudaDeviceGetAttribute(&c.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (cuda_stream) {
-    c.stream = reinterpret_cast<cudaStream_t>(cuda_stream);
-  } else {
-    if (!NFS_CUDA(c, cudaStreamCreateWithFlags(&c.stream, cudaStreamNonBlocking))) goto fail;
-    c.own_stream = true;
+  bool ok = NFS_CUDA(c, cudaGetDevice(&c.device));
+  int smem_sm = 0;
+  ok = ok && NFS_CUDA(c, cudaDeviceGetAttribute(&c.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c.device));
+  ok = ok && NFS_CUDA(c, cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, c.device));
+  ok = ok && NFS_CUDA(c, cudaDeviceGetAttribute(&c.n_sm, cudaDevAttrMultiProcessorCount, c.device));
+  if (ok) {
+    if (cuda_stream) {
+      c.stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    } else {
+      ok = NFS_CUDA(c, cudaStreamCreateWithFlags(&c.stream, cudaStreamNonBlocking));
+      c.own_stream = ok;
+    }
   }
-  {
+  if (ok && !lag_plan(c, smem_sm, c.n_sm, c.P)) {
+    c.status = NFS_ERR_INVALID_ARG;  // a lag task's own span does not fit shared memory
+    ok = false;
+  }
+  if (ok) {
     // memory plan: everything is sized before the first frame arrives
     size_t free_b = 0, total_b = 0;
-    if (!NFS_CUDA(c, cudaMemGetInfo(&free_b, &total_b))) goto fail;
+    ok = NFS_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     // default batch: 1024 frames, halved (down to 128) while the ring would take more than a third of the free memory
-    while (batch_frames == 0 && c.B > 128 && (double)c.R * (double)c.P * 8.0 > (double)free_b / 3.0) {
+    while (ok && batch_frames == 0 && c.B > 128 && (double)c.R * (double)c.P * 8.0 > (double)free_b / 3.0) {
       c.B /= 2;
       c.R = c.Lmax + c.B;
     }
-    const double need = (double)c.P * ((double)c.R * 8 + 8 + (double)c.n_lags * 8 + 8 + 16 + 8) +
-                        (double)fft_rowT_elems(c) * 8 +
-                        (double)W * H * 4 + (double)(n_lags + 1) * n_qbins * 8 + (64 << 20);
-    if (need > (double)free_b) {
-      free_all(c);
-      delete h;
-      return NFS_ERR_OOM;
+    const double need = (double)c.P * ((double)c.R * 8 + 8 + (double)totals_rows(c) * 8 + 8 + 16 + 8) +
+                        (double)fft_rowT_elems(c) * 8 + (double)W * H * 4 + (double)(2 * n_lags + 2) * n_qbins * 8 +
+                        (64 << 20);
+    if (ok && need > (double)free_b) {
+      c.status = NFS_ERR_OOM;
+      ok = false;
     }
   }
-  if (!dev_alloc(c, &c.ring, (size_t)c.R * c.P)) goto fail;
-  if (!lag_make_tensor_map(c)) {
-    c.status = NFS_ERR_CUDA;
-    c.cuda_err = "cuTensorMapEncodeTiled failed";
-    goto fail;
+  ok = ok && dev_alloc(c, &c.ring, (size_t)c.R * c.P);
+  ok = ok && lag_configure(c);
+  ok = ok && fft_configure(c);
+  ok = ok && dev_alloc(c, &c.rowbuf, fft_rowT_elems(c));
+  ok = ok && dev_alloc(c, &c.ref, (size_t)W * H);
+  ok = ok && dev_alloc(c, &c.Fref, (size_t)c.P);
+  ok = ok && dev_alloc(c, &c.totals, totals_rows(c) * c.P);
+  if (c.bin_only) ok = ok && dev_alloc(c, &c.totals_b, (size_t)c.n_lags * c.n_qbins);
+  ok = ok && dev_alloc(c, &c.I2, (size_t)c.P);
+  ok = ok && dev_alloc(c, &c.I1, (size_t)c.P);
+  ok = ok && dev_alloc(c, &c.sums, (size_t)c.B + 1);
+  ok = ok && dev_alloc(c, &c.fft_cnt, fft_cnt_elems(c));
+  ok = ok && dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 2) * c.n_qbins);
+  ok = ok && dev_alloc(c, &c.d_tmp, (size_t)c.P);
+  ok = ok && dev_alloc(c, &c.d_flags, 1);
+  ok = ok && build_tables(c);
+  ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)c.R * c.P, c.stream));
+  ok = ok && zero_state(c);
+  ok = ok && NFS_CUDA(c, cudaStreamSynchronize(c.stream));
+  if (ok) {
+    *out = h;
+    return NFS_OK;
   }
-  if (!dev_alloc(c, &c.rowbuf, fft_rowT_elems(c))) goto fail;
-  if (!dev_alloc(c, &c.ref, (size_t)W * H)) goto fail;
-  if (!dev_alloc(c, &c.Fref, (size_t)c.P)) goto fail;
-  if (!dev_alloc(c, &c.totals, (size_t)c.n_lags * c.P)) goto fail;
-  if (!dev_alloc(c, &c.I2, (size_t)c.P)) goto fail;
-  if (!dev_alloc(c, &c.I1, (size_t)c.P)) goto fail;
-  if (!dev_alloc(c, &c.sums, (size_t)c.B + 1)) goto fail;
-  if (!dev_alloc(c, &c.fft_cnt, 1 + 3 * (size_t)c.B)) goto fail;
-  if (!dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 2) * c.n_qbins)) goto fail;
-  if (!dev_alloc(c, &c.d_tmp, (size_t)c.P)) goto fail;
-  if (!dev_alloc(c, &c.d_flags, 1)) goto fail;
-  if (!build_tables(c)) goto fail;
-  if (!NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)c.R * c.P, c.stream))) goto fail;
-  if (!zero_state(c)) goto fail;
-  if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) goto fail;
-  *out = h;
-  return NFS_OK;
-
-fail : {
   const int st = (c.status != NFS_OK) ? c.status : NFS_ERR_CUDA;
   const bool oom = c.cuda_err.find("out of memory") != std::string::npos;
   free_all(c);
   delete h;
   return oom ? NFS_ERR_OOM : st;
 }
+
+int get_plane(Ctx& c, double* out) {
+  std::vector<double> tmp((size_t)c.P);
+  if (!NFS_CUDA(c, cudaMemcpyAsync(tmp.data(), c.d_tmp, sizeof(double) * c.P, cudaMemcpyDeviceToHost, c.stream)))
+    return c.status;
+  const int st = sync_and_check(c);
+  if (st != NFS_OK) return st;
+  ring_to_plane(c, tmp.data(), out);
+  return NFS_OK;
+}
+
+// common entry of the calls that read results: valid context, on its device, at least one frame, pairs up to date
+int ready(nfs_ctx* h) {
+  if (!h) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (!enter(c)) return c.status;
+  if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
+  return NFS_OK;
+}
+
+}  // namespace
+
+// Nothing may throw across the C boundary: allocation failures of the host-side containers become NFS_ERR_OOM.
+#define NFS_GUARDED(expr)            \
+  try {                              \
+    return (expr);                   \
+  } catch (const std::bad_alloc&) {  \
+    return NFS_ERR_OOM;              \
+  } catch (...) {                    \
+    return NFS_ERR_STATE;            \
+  }
+
+extern "C" {
+
+int nfs_create_opts(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                    int batch_frames, unsigned flags) {
+  NFS_GUARDED(create_impl(out, W, H, lags, n_lags, n_qbins, cuda_stream, batch_frames, flags))
+}
+
+int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                  int batch_frames) {
+  return nfs_create_opts(out, W, H, lags, n_lags, n_qbins, cuda_stream, batch_frames, 0u);
 }
 
 int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream) {
-  return nfs_create_ex(out, W, H, lags, n_lags, n_qbins, cuda_stream, 0);
+  return nfs_create_opts(out, W, H, lags, n_lags, n_qbins, cuda_stream, 0, 0u);
 }
 
-int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) {
+static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n) {
   if (!h || !d_frames || n < 1) return NFS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(d_frames) & 15u) != 0) return NFS_ERR_INVALID_ARG;  // 128-bit loads
   Ctx& c = h->c;
-  if (c.status != NFS_OK) return c.status;
+  if (!enter(c)) return c.status;
   const int64_t fpx = (int64_t)c.W * c.H;
   int done = 0;
   while (done < n) {
@@ -315,22 +363,21 @@ int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) {
     const uint16_t* fr = d_frames + (int64_t)done * fpx;
     if (c.n_frames == 0) c.n_launches += launch_make_ref(c, fr);
     c.n_launches += launch_fft_frames(c, fr, b, c.n_frames);
-    if (!check_launch(c, "fft launch")) return c.status;
+    if (c.status != NFS_OK) return c.status;
     c.n_frames += b;
     done += b;
     if (c.n_frames - c.n_acc == c.B && !flush_pending(c)) return c.status;
   }
   return NFS_OK;
 }
+int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) { NFS_GUARDED(push_impl(h, d_frames, n)) }
 
-int nfs_finalize(nfs_ctx* h, double* D_q_tau, double* I_q, int64_t* counts) {
-  if (!h) return NFS_ERR_INVALID_ARG;
+static int finalize_impl(nfs_ctx* h, double* D_q_tau, double* I_q, int64_t* counts) {
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
   Ctx& c = h->c;
-  if (c.status != NFS_OK) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
-  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_bin(c);
-  if (!check_launch(c, "bin launch")) return c.status;
+  if (c.status != NFS_OK) return c.status;
   const size_t nD = (size_t)c.n_lags * c.n_qbins;
   if (D_q_tau)
     if (!NFS_CUDA(c, cudaMemcpyAsync(D_q_tau, c.d_out, sizeof(double) * nD, cudaMemcpyDeviceToHost, c.stream)))
@@ -343,101 +390,84 @@ int nfs_finalize(nfs_ctx* h, double* D_q_tau, double* I_q, int64_t* counts) {
   if (counts) memcpy(counts, c.counts.data(), sizeof(int64_t) * c.n_qbins);
   return NFS_OK;
 }
+int nfs_finalize(nfs_ctx* h, double* D, double* I_q, int64_t* counts) { NFS_GUARDED(finalize_impl(h, D, I_q, counts)) }
 
 int nfs_get_pair_counts(nfs_ctx* h, int64_t* n_pairs) {
   if (!h || !n_pairs) return NFS_ERR_INVALID_ARG;
   const Ctx& c = h->c;
+  if (c.status != NFS_OK) return c.status;
   for (int l = 0; l < c.n_lags; ++l) n_pairs[l] = c.lags[l] < c.n_frames ? c.n_frames - c.lags[l] : 0;
   return NFS_OK;
 }
 
-static int get_plane(Ctx& c, double* out) {
-  std::vector<double> tmp((size_t)c.P);
-  if (!NFS_CUDA(c, cudaMemcpyAsync(tmp.data(), c.d_tmp, sizeof(double) * c.P, cudaMemcpyDeviceToHost, c.stream)))
-    return c.status;
-  const int st = sync_and_check(c);
-  if (st != NFS_OK) return st;
-  ring_to_plane(c, tmp.data(), out);
-  return NFS_OK;
-}
-
-int nfs_get_D2d(nfs_ctx* h, int lag_index, double* out) {
+static int D2d_impl(nfs_ctx* h, int lag_index, double* out) {
   if (!h || !out) return NFS_ERR_INVALID_ARG;
+  if (lag_index < 0 || lag_index >= h->c.n_lags) return NFS_ERR_INVALID_ARG;
+  if (h->c.bin_only) return NFS_ERR_STATE;  // the 2-D difference spectra are not kept in this mode
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
   Ctx& c = h->c;
-  if (lag_index < 0 || lag_index >= c.n_lags) return NFS_ERR_INVALID_ARG;
-  if (c.status != NFS_OK) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
-  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_D2d(c, lag_index, c.d_tmp);
-  if (!check_launch(c, "D2d launch")) return c.status;
+  if (c.status != NFS_OK) return c.status;
   return get_plane(c, out);
 }
+int nfs_get_D2d(nfs_ctx* h, int lag_index, double* out) { NFS_GUARDED(D2d_impl(h, lag_index, out)) }
 
-int nfs_get_I2d(nfs_ctx* h, double* out) {
+static int plane_impl(nfs_ctx* h, double* out, int which) {
   if (!h || !out) return NFS_ERR_INVALID_ARG;
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
   Ctx& c = h->c;
+  c.n_launches += which == 0 ? launch_I2d(c, c.d_tmp) : launch_V2d(c, c.d_tmp);
   if (c.status != NFS_OK) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
-  if (!flush_pending(c)) return c.status;
-  c.n_launches += launch_I2d(c, c.d_tmp);
-  if (!check_launch(c, "I2d launch")) return c.status;
   return get_plane(c, out);
 }
+int nfs_get_I2d(nfs_ctx* h, double* out) { NFS_GUARDED(plane_impl(h, out, 0)) }
+int nfs_get_V2d(nfs_ctx* h, double* out) { NFS_GUARDED(plane_impl(h, out, 1)) }
 
-int nfs_get_variance(nfs_ctx* h, double* V_q) {
-  if (!h || !V_q) return NFS_ERR_INVALID_ARG;
+static int variance_impl(nfs_ctx* h, double* V_q) {
+  if (!V_q) return NFS_ERR_INVALID_ARG;
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
   Ctx& c = h->c;
-  if (c.status != NFS_OK) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
-  if (!flush_pending(c)) return c.status;
   c.n_launches += launch_bin(c);
-  if (!check_launch(c, "bin launch")) return c.status;
+  if (c.status != NFS_OK) return c.status;
   if (!NFS_CUDA(c, cudaMemcpyAsync(V_q, c.d_out + (size_t)(c.n_lags + 1) * c.n_qbins, sizeof(double) * c.n_qbins,
                                    cudaMemcpyDeviceToHost, c.stream)))
     return c.status;
   return sync_and_check(c);
 }
-
-int nfs_get_V2d(nfs_ctx* h, double* out) {
-  if (!h || !out) return NFS_ERR_INVALID_ARG;
-  Ctx& c = h->c;
-  if (c.status != NFS_OK) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
-  if (!flush_pending(c)) return c.status;
-  c.n_launches += launch_V2d(c, c.d_tmp);
-  if (!check_launch(c, "V2d launch")) return c.status;
-  return get_plane(c, out);
-}
+int nfs_get_variance(nfs_ctx* h, double* V_q) { NFS_GUARDED(variance_impl(h, V_q)) }
 
 int64_t nfs_num_frames(const nfs_ctx* h) { return h ? h->c.n_frames : 0; }
 int nfs_ring_capacity(const nfs_ctx* h) { return h ? h->c.R : 0; }
 int64_t nfs_device_bytes(const nfs_ctx* h) { return h ? h->c.dev_bytes : 0; }
 int64_t nfs_num_launches(const nfs_ctx* h) { return h ? h->c.n_launches : 0; }
 
-int nfs_set_lag_kernel(nfs_ctx* h, int variant) {
-  if (!h || variant < 0 || variant > 3) return NFS_ERR_INVALID_ARG;
-  h->c.lag_variant = variant == 1 ? 1 : 0;
-  h->c.lag_persistent = variant == 2 ? 0 : (variant == 3 ? 1 : -1);
+int nfs_set_launch_shape(nfs_ctx* h, int shape) {
+  if (!h || shape < 0 || shape > 2) return NFS_ERR_INVALID_ARG;
+  h->c.lag_shape = shape;
   return NFS_OK;
 }
 
-int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_optin, int32_t* out, int cap) {
-  if (!lags || n_lags < 1 || !out || cap < 4) return NFS_ERR_INVALID_ARG;
-  for (int l = 0; l < n_lags; ++l)
-    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return NFS_ERR_INVALID_ARG;
+static int plan_impl(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,
+                     int cap) {
+  if (!lags_ok(lags, n_lags) || !out || cap < 6 || n_px < 32 || n_sm < 1) return NFS_ERR_INVALID_ARG;
   Ctx c;
   c.lags.assign(lags, lags + n_lags);
   c.n_lags = n_lags;
   c.Lmax = lags[n_lags - 1];
   c.max_smem_optin = smem_optin;
-  if (!lag_plan(c, smem_per_sm, kLagMinBlocks * 148, 1 << 20)) return NFS_ERR_INVALID_ARG;
-  const size_t need = 4 + c.groups.size() * 23 + c.tasks.size() * 4;
+  if (!lag_plan(c, smem_per_sm, n_sm, (int64_t)n_px)) return NFS_ERR_INVALID_ARG;
+  const size_t need = 6 + c.groups.size() * 23 + c.tasks.size() * 4;
   if (need > (size_t)cap) return NFS_ERR_INVALID_ARG;
   int32_t* o = out;
   *o++ = (int32_t)c.groups.size();
   *o++ = (int32_t)c.tasks.size();
   *o++ = c.lag_stages;
   *o++ = (int32_t)c.lag_smem;
+  *o++ = c.lag_tpx;
+  *o++ = c.lag_ctas_per_sm;
   for (const LagGroup& g : c.groups) {
     *o++ = g.task0, *o++ = g.ntasks, *o++ = g.tau_min, *o++ = g.tau_max, *o++ = g.flags;
     for (int w = 0; w < 16; ++w) *o++ = g.warp_task[w];
@@ -446,6 +476,9 @@ int nfs_plan_lags(const int32_t* lags, int n_lags, int smem_per_sm, int smem_opt
   for (const LagTask& t : c.tasks) *o++ = t.tau0, *o++ = t.cnt, *o++ = t.l0, *o++ = t.kind;
   return (int)need;
 }
+int nfs_plan_lags(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out, int cap) {
+  NFS_GUARDED(plan_impl(lags, n_lags, n_px, smem_per_sm, smem_optin, n_sm, out, cap))
+}
 
 int nfs_set_profiling(nfs_ctx* h, int enable) {
   if (!h) return NFS_ERR_INVALID_ARG;
@@ -453,10 +486,10 @@ int nfs_set_profiling(nfs_ctx* h, int enable) {
   return NFS_OK;
 }
 
-int nfs_get_kernel_times(nfs_ctx* h, double* ms, int64_t* launches) {
+static int times_impl(nfs_ctx* h, double* ms, int64_t* launches) {
   if (!h) return NFS_ERR_INVALID_ARG;
   Ctx& c = h->c;
-  if (c.status != NFS_OK) return c.status;
+  if (!enter(c)) return c.status;
   if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
   for (size_t i = 0; i < c.ev_class.size(); ++i) {
     float t = 0.f;
@@ -475,6 +508,7 @@ int nfs_get_kernel_times(nfs_ctx* h, double* ms, int64_t* launches) {
   }
   return NFS_OK;
 }
+int nfs_get_kernel_times(nfs_ctx* h, double* ms, int64_t* launches) { NFS_GUARDED(times_impl(h, ms, launches)) }
 
 int nfs_reset(nfs_ctx* h) {
   if (!h) return NFS_ERR_INVALID_ARG;
@@ -482,7 +516,7 @@ int nfs_reset(nfs_ctx* h) {
   cudaStreamSynchronize(c.stream);
   cudaGetLastError();
   if (c.status == NFS_ERR_ZERO_MEAN) c.status = NFS_OK;
-  if (c.status != NFS_OK) return c.status;  // a CUDA error is not recoverable by reset
+  if (!enter(c)) return c.status;  // a CUDA error is not recoverable by reset
   if (!zero_state(c)) return c.status;
   if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
   return NFS_OK;

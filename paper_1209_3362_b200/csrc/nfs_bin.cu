@@ -31,7 +31,9 @@ __device__ __forceinline__ double v2d_value(const double* __restrict__ I2, const
 }
 
 // grid (n_qbins, n_lags + 2), 128 threads.  Row l < n_lags: D(b, tau_l); row n_lags: I(b); row n_lags + 1: V(b).
-__global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, const double* __restrict__ I2,
+// binned != nullptr (bin-only mode): the D rows come from the weighted bin sums kept by k_bin_accumulate.
+__global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, const double* __restrict__ binned,
+                                             const double* __restrict__ I2,
                                              const double2* __restrict__ I1, const float2* __restrict__ Fref,
                                              const uint32_t* __restrict__ perm, const int32_t* __restrict__ bin_start,
                                              const int32_t* __restrict__ lags, int n_lags, int n_qbins, int64_t P,
@@ -52,7 +54,7 @@ __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, 
     const double wgt = (e >> 31) ? 2.0 : 1.0;
     double v;
     if (row < n_lags)
-      v = totals[(int64_t)row * P + p] * inv;
+      v = binned ? 0.0 : totals[(int64_t)row * P + p] * inv;
     else if (row == n_lags)
       v = i2d_value(I2, I1, Fref, p, inv);
     else
@@ -72,10 +74,33 @@ __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, 
   }
   __syncthreads();
   if (threadIdx.x == 0) {
-    const double a = (sa[0] + sa[1]) + (sa[2] + sa[3]);
+    double a = (sa[0] + sa[1]) + (sa[2] + sa[3]);
     const double w = (sw[0] + sw[1]) + (sw[2] + sw[3]);
+    if (binned && row < n_lags) a = binned[(int64_t)row * n_qbins + b] * inv;
     out[(int64_t)row * n_qbins + b] = (w > 0.0 && inv > 0.0) ? a / w : 0.0;
   }
+}
+
+// bin-only mode (the full 2-D spectra need not be stored): binned[l_first + row][b] += sum over the
+// bin's pixels of weight * scratch[row][p], the per-pixel pair sums one lag group accumulated in one batch.  Same
+// fixed order as k_bin, one writer per address, launches stream ordered: bit-identical from run to run.
+__global__ void __launch_bounds__(128) k_bin_accumulate(const double* __restrict__ scratch, const uint32_t* __restrict__ perm,
+                                                        const int32_t* __restrict__ bin_start, int n_qbins, int64_t P,
+                                                        double* __restrict__ binned) {
+  const int b = blockIdx.x, row = blockIdx.y;
+  const int beg = bin_start[b], end = bin_start[b + 1];
+  double acc = 0.0;
+  for (int i = beg + (int)threadIdx.x; i < end; i += 128) {
+    const uint32_t e = perm[i];
+    const double v = scratch[(int64_t)row * P + (int64_t)(e & 0x7fffffffu)];
+    acc += (e >> 31) ? 2.0 * v : v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  __shared__ double sa[4];
+  if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) binned[(int64_t)row * n_qbins + b] += (sa[0] + sa[1]) + (sa[2] + sa[3]);
 }
 
 __global__ void __launch_bounds__(256) k_I2d(const double* __restrict__ I2, const double2* __restrict__ I1,
@@ -100,18 +125,30 @@ __global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int
 int launch_bin(Ctx& c) {
   dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 2));
   ProfScope ps(c, kKBin);
-  k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.I2, c.I1, c.Fref, c.perm, c.bin_start, c.d_lags, c.n_lags, c.n_qbins,
-                                    c.P, c.n_frames, c.d_out);
+  k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.bin_only ? c.totals_b : nullptr, c.I2, c.I1, c.Fref, c.perm, c.bin_start,
+                                    c.d_lags, c.n_lags, c.n_qbins, c.P, c.n_frames, c.d_out);
+  NFS_CUDA(c, cudaGetLastError());
+  return 1;
+}
+
+int launch_bin_accumulate(Ctx& c, int l_first, int n_rows) {
+  dim3 grid((unsigned)c.n_qbins, (unsigned)n_rows);
+  ProfScope ps(c, kKBin);
+  k_bin_accumulate<<<grid, 128, 0, c.stream>>>(c.totals, c.perm, c.bin_start, c.n_qbins, c.P,
+                                               c.totals_b + (size_t)l_first * c.n_qbins);
+  NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
 int launch_I2d(Ctx& c, double* d_dst) {
   k_I2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, c.n_frames, d_dst);
+  NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
 int launch_V2d(Ctx& c, double* d_dst) {
   k_V2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.P, c.n_frames, d_dst);
+  NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
@@ -119,6 +156,7 @@ int launch_D2d(Ctx& c, int l, double* d_dst) {
   const int64_t np = c.n_frames - (int64_t)c.lags[l];
   const double inv = np > 0 ? 1.0 / (double)np : 0.0;
   k_D2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.totals + (int64_t)l * c.P, c.P, inv, d_dst);
+  NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 

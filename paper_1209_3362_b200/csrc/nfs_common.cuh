@@ -20,28 +20,14 @@
 namespace nfs {
 
 // ---- lag-accumulation plan (built on the host at create, nfs_lag.cu: lag_plan) ---------------------
-#ifndef NFS_LAG_BPC
-#define NFS_LAG_BPC 2
-#endif
-#ifndef NFS_LAG_MAXT
-#define NFS_LAG_MAXT 8
-#endif
-#ifndef NFS_LAG_MINB
-#define NFS_LAG_MINB 2
-#endif
-#ifndef NFS_LAG_MAXSTAGES
-#define NFS_LAG_MAXSTAGES 6
-#endif
-constexpr int kG = 13;        // lags per warp task (register window depth)
-constexpr int kTilePx = 32;   // Fourier pixels per CTA tile (one warp width)
-constexpr int kMaxTasks = NFS_LAG_MAXT;   // consumer warps (lag tasks) per CTA: kMaxTasks / 4 per SM sub-partition
-constexpr int kLagMinBlocks = NFS_LAG_MINB;  // CTAs per SM the kernel is compiled for
-constexpr int kChunk = kG * NFS_LAG_BPC;  // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
+constexpr int kG = 13;            // lags per register-window task (window depth)
+constexpr int kTaskSlots = 8;     // lag tasks per group: one consumer warp each per 32-pixel sub-tile
+constexpr int kChunk = 2 * kG;    // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
 constexpr int kMinStages = 2;
-constexpr int kMaxStages = NFS_LAG_MAXSTAGES;  // pipeline depth is chosen at create from the shared memory left
-constexpr int kFoldChunks = 20;  // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (520) steps
-constexpr int kSparseMax = 6;  // lags per lag-list task (one LDS.64 per pair update, exact-count code paths)
-constexpr int kDenseMin = 7;  // contiguous runs of >= kDenseMin lags use the register-window path
+constexpr int kMaxStages = 8;     // pipeline depth is chosen at create from the shared memory left
+constexpr int kFoldChunks = 20;   // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (520) steps
+constexpr int kSparseMax = 6;     // lags per lag-list task (one LDS.64 per pair update, exact-count code paths)
+constexpr int kDenseMin = 2;      // runs of >= kDenseMin consecutive lags use the register-window path
 
 struct LagTask {
   int tau0;  // smallest lag of the task
@@ -53,13 +39,14 @@ struct LagGroup {
   int task0, ntasks;
   int tau_min, tau_max;
   int flags;  // bit 0: one task of this group accumulates the I sums (the group runs for every batch)
+              // bit 1: single stream: the batch's own frames are read from the head of the window ring
   int cta0, nctas;  // persistent CTAs [cta0, cta0 + nctas) of the launch work on this group (share ~ its work)
-  signed char warp_task[16];  // task (relative to task0) run by consumer warp w, or -1: placed so that the
-                              // four SM sub-partitions (warp id mod 4) carry equal work
+  signed char warp_task[16];  // task (relative to task0) run by consumer warp slot w < kTaskSlots, or -1: placed so
+                              // that the four SM sub-partitions (warp id mod 4) carry equal work
 };
 
 // kernel classes for the optional per-kernel CUDA-event timing (nfs_set_profiling)
-enum KernelClass { kKSum = 0, kKFft = 1, kKAccI = 2, kKLag = 3, kKBin = 4, kNumKernelClasses = 5 };
+enum KernelClass { kKSum = 0, kKFft = 1, kKAux = 2, kKLag = 3, kKBin = 4, kNumKernelClasses = 5 };
 
 struct Ctx {
   int W = 0, H = 0, n = 0;  // n = W/2
@@ -67,6 +54,9 @@ struct Ctx {
   int n_lags = 0, n_qbins = 0, Lmax = 0;
   int B = 0;   // internal batch (frames)
   int R = 0;   // ring slots
+  int device = 0;
+  int n_sm = 0;
+  bool bin_only = false;  // accumulate |q|-binned totals only (no 2-D spectra kept)
   std::vector<int32_t> lags;
   std::vector<int64_t> counts;  // full-plane pixel count per bin
   cudaStream_t stream = nullptr;
@@ -74,7 +64,6 @@ struct Ctx {
   int64_t n_frames = 0;  // frames pushed (all transformed into the ring)
   int64_t n_acc = 0;     // of those, frames whose pairs are already in the totals
   int64_t n_launches = 0;
-  int lag_variant = 0;
   int status = 0;  // sticky
   std::string cuda_err;
   int64_t dev_bytes = 0;
@@ -82,16 +71,17 @@ struct Ctx {
 
   // device memory
   float2* ring = nullptr;
-  CUtensorMap ring_map;          // 2-D TMA descriptor of the ring (nfs_lag.cu)
+  CUtensorMap ring_map;          // 2-D TMA descriptor of the ring (nfs_lag.cu): box = tile pixels x kChunk slots
   float2* rowbuf = nullptr;      // [slots][P] output of the row pass (transposed, L2 resident)
   float* ref = nullptr;          // [H][W]
   float2* Fref = nullptr;        // [P] unitary FFT of ref
-  double* totals = nullptr;      // [n_lags][P]
+  double* totals = nullptr;      // [n_lags][P]; bin-only mode: scratch [max lags of a group][P]
+  double* totals_b = nullptr;    // bin-only mode: [n_lags][n_qbins] weighted sums over the bin's pixels
   double* I2 = nullptr;          // [P]  sum_t |F'_t|^2
   double2* I1 = nullptr;         // [P]  sum_t F'_t
-  unsigned long long* sums = nullptr;  // [B] exact pixel sums of the frames of a batch
-  unsigned int* fft_cnt = nullptr;     // [1 + 3 B] work-queue head and per-frame completion counters
-  int fft_grid = 0;                    // CTAs of the persistent FFT kernel (set at the first launch)
+  unsigned long long* sums = nullptr;  // [B + 1] exact pixel sums of the frames of a batch; [B] = S_0
+  unsigned int* fft_cnt = nullptr;     // work-queue head and per-frame completion counters of k_fft
+  int fft_grid = 0;                    // CTAs of the persistent FFT kernel (set at create)
   float2* tw = nullptr;          // inner twiddle table (nfs_fft.cu)
   float2* tw_out = nullptr;      // outer twiddle table, W > 1024 only
   int32_t* d_lags = nullptr;     // [n_lags]
@@ -102,11 +92,14 @@ struct Ctx {
   int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
   LagTask* d_tasks = nullptr;
   LagGroup* d_groups = nullptr;
-  int* d_claim = nullptr;        // [n_groups] next pixel tile of each group, zeroed before every k_lag_tiled launch
+  int* d_claim = nullptr;        // [n_groups] next pixel tile of each group, zeroed before every persistent launch
   int lag_stages = kMinStages;   // pipeline stages of k_lag_tiled (chosen by lag_plan)
+  int lag_tpx = 32;              // Fourier pixels per CTA tile: 32 (8 consumer warps) or 64 (16 consumer warps)
+  int lag_ctas_per_sm = 1;       // resident CTAs per SM the plan counts on
   int lag_grid = 0;              // persistent CTAs of k_lag_tiled (sum of the groups' shares)
-  int lag_persistent = -1;       // -1: chosen per launch (launch_lag_tiled); 0 / 1: forced (nfs_set_lag_kernel 2 / 3)
+  int lag_shape = 0;             // 0: chosen per launch (launch_lag_tiled); 1 / 2: forced one-tile / persistent
   size_t lag_smem = 0;           // dynamic shared memory of k_lag_tiled
+  int max_group_lags = 0;        // most lags in one group (bin-only scratch rows)
   std::vector<LagTask> tasks;
   std::vector<LagGroup> groups;
 
@@ -119,6 +112,17 @@ struct Ctx {
   int64_t prof_n[kNumKernelClasses] = {0, 0, 0, 0, 0};
 };
 
+// record the first CUDA error of the context (sticky)
+inline bool cuda_ok(Ctx& c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  if (c.status == NFS_OK) {
+    c.status = NFS_ERR_CUDA;
+    c.cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+  }
+  return false;
+}
+#define NFS_CUDA(c, call) ::nfs::cuda_ok((c), (call), #call)
+
 // RAII: records an event pair around the launches enqueued in its scope when profiling is on
 struct ProfScope {
   Ctx& c;
@@ -127,35 +131,36 @@ struct ProfScope {
     if (!c.prof) return;
     while (c.ev_pool.size() < c.ev_used + 2) {
       cudaEvent_t e;
-      cudaEventCreate(&e);
+      if (!NFS_CUDA(c, cudaEventCreate(&e))) return;
       c.ev_pool.push_back(e);
     }
     cudaEvent_t start = c.ev_pool[c.ev_used];
     stop = c.ev_pool[c.ev_used + 1];
     c.ev_used += 2;
     c.ev_class.push_back(cls);
-    cudaEventRecord(start, c.stream);
+    NFS_CUDA(c, cudaEventRecord(start, c.stream));
   }
   ~ProfScope() {
-    if (stop) cudaEventRecord(stop, c.stream);
+    if (stop) NFS_CUDA(c, cudaEventRecord(stop, c.stream));
   }
 };
 
-// ---- kernel launchers (each returns the number of kernel launches it enqueued; sets cudaGetLastError) ----
+// ---- kernel launchers (each returns the number of kernel launches it enqueued; CUDA errors go to c.status) ----
 // nfs_fft.cu
+bool fft_configure(Ctx& c);                                       // once at create: kernel attributes, grid size
 int launch_make_ref(Ctx& c, const uint16_t* frame0);              // S_0, ref = i_0, Fref = FFT(ref)
 int launch_fft_frames(Ctx& c, const uint16_t* frames, int nf, int64_t t_first);  // ring[t_first..] = FFT(i_t - ref)
 size_t fft_rowT_elems(const Ctx& c);                              // float2 elements of the row-pass buffer
+size_t fft_cnt_elems(const Ctx& c);                               // unsigned ints of the work-queue counters
 // nfs_lag.cu
-int launch_accum_I(Ctx& c, int64_t t0, int b);
-int launch_lag_simple(Ctx& c, int64_t t0, int b);
 int launch_lag_tiled(Ctx& c, int64_t t0, int b);
-// host only (no CUDA call): tasks, groups, pipeline depth from the lag list, the shared memory per SM and
+// host only (no CUDA call): tasks, groups, tile width, pipeline depth from the lag list, the shared memory per SM and
 // c.max_smem_optin; false if a lag group cannot fit shared memory
-bool lag_plan(Ctx& c, int smem_per_sm, int cta_slots, int ntiles);
-bool lag_make_tensor_map(Ctx& c);  // after the ring is allocated
+bool lag_plan(Ctx& c, int smem_per_sm, int n_sm, int64_t P);
+bool lag_configure(Ctx& c);        // once at create, after the ring is allocated: tensor map, kernel attributes
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1), I (row n_lags), V (row n_lags+1)
+int launch_bin_accumulate(Ctx& c, int l_first, int n_rows);  // bin-only mode: totals_b[l_first..] += binned scratch rows
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
 int launch_V2d(Ctx& c, double* d_dst);       // d_dst[P] = V2d (variance form) in ring layout
 int launch_D2d(Ctx& c, int l, double* d_dst);

@@ -22,6 +22,8 @@
 // L > 1024: a 32-point register pass over L/32 threads, then 32 independent FFTs of length L/32 done the
 // same way by 2 or 4 lanes each.  Twiddles between passes come from fp64-computed tables laid out so
 // that consecutive lanes read consecutive entries.
+#include <algorithm>
+
 #include "nfs_common.cuh"
 
 namespace nfs {
@@ -29,10 +31,6 @@ namespace nfs {
 // ------------------------------------------------------------------------------------------------
 // complex helpers and register DFTs
 // ------------------------------------------------------------------------------------------------
-#ifndef NFS_FFT_PACKED
-#define NFS_FFT_PACKED 1
-#endif
-#if NFS_FFT_PACKED
 // complex add / subtract as one packed instruction (SASS FADD2): one issue slot instead of two
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) {
   unsigned long long ua, ub, ur;
@@ -52,10 +50,6 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(ur));
   return r;
 }
-#else
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-#endif
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
@@ -135,13 +129,10 @@ __device__ __forceinline__ void dft(float2* u) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// L2 eviction hints (NFS_FFT_L2HINTS): the uint16 frame is read by the sum items and again, a few queue
+// L2 eviction hints: the uint16 frame is read by the sum items and again, a few queue
 // steps later, by the row items; the row-pass intermediate is written and re-read through L2; the ring
 // slot is written once and not read again by this kernel.
 // ------------------------------------------------------------------------------------------------
-#ifndef NFS_FFT_L2HINTS
-#define NFS_FFT_L2HINTS 1
-#endif
 __device__ __forceinline__ unsigned long long pol_evict_last() {
   unsigned long long p;
   asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
@@ -153,62 +144,35 @@ __device__ __forceinline__ unsigned long long pol_evict_first() {
   return p;
 }
 __device__ __forceinline__ uint4 ld_u4_hint(const uint4* p, unsigned long long pol) {
-#if NFS_FFT_L2HINTS
   uint4 v;
   asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
                : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
                : "l"(p), "l"(pol));
   return v;
-#else
-  return __ldg(p);
-#endif
 }
 __device__ __forceinline__ float2 ld_f2_cg_hint(const float2* p, unsigned long long pol) {
-#if NFS_FFT_L2HINTS
   float2 v;
   asm volatile("ld.global.cg.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol) : "memory");
   return v;
-#else
-  return __ldcg(p);
-#endif
 }
 __device__ __forceinline__ void st_f2_hint(float2* p, float2 v, unsigned long long pol) {
-#if NFS_FFT_L2HINTS
   asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
-#else
-  *p = v;
-#endif
 }
 __device__ __forceinline__ void st_f4_hint(float4* p, float4 v, unsigned long long pol) {
-#if NFS_FFT_L2HINTS
   asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w),
                "l"(pol)
                : "memory");
-#else
-  *p = v;
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------
 // plan constants for FFT length L
 // ------------------------------------------------------------------------------------------------
-#ifndef NFS_FFT_NT
-#define NFS_FFT_NT 128
-#endif
-#ifndef NFS_FFT_NT_LARGE
-#define NFS_FFT_NT_LARGE 256
-#endif
-#ifndef NFS_FFT_DR
-#define NFS_FFT_DR 0
-#define NFS_FFT_DC 0
-#define NFS_FFT_SLOTS 0
-#endif
 constexpr int kMaxSlots = 40;
 
 template <int L>
 struct Plan {
   static constexpr int T = L / 32;                       // threads per FFT
-  static constexpr int NT = L <= 1024 ? (L >= 512 ? NFS_FFT_NT : 256) : NFS_FFT_NT_LARGE;  // threads per CTA
+  static constexpr int NT = (L == 512 || L == 1024) ? 128 : 256;  // threads per CTA
   static constexpr int minBlocks = 512 / NT;  // CTAs per SM the kernel is compiled for (128 registers per thread)
   static constexpr int Fc = NT / T;                      // FFTs per CTA item
   static constexpr bool two = L > 1024;                  // two-level plan
@@ -232,9 +196,9 @@ struct Plan {
   static constexpr int claimed = 2 * minBlocks * 148;
   static constexpr int win_ = (claimed + perStep - 1) / perStep;
   static constexpr int win = win_ < 16 ? win_ : 16;
-  static constexpr int Dr = NFS_FFT_DR ? NFS_FFT_DR : win + 1;                   // sum items -> row items
-  static constexpr int Dc = NFS_FFT_DC ? NFS_FFT_DC : (L <= 1024 ? win + 1 : win);  // row items -> column items
-  static constexpr int slots = NFS_FFT_SLOTS ? NFS_FFT_SLOTS : Dc + win + (L <= 1024 ? 1 : 0);  // intermediate frames
+  static constexpr int Dr = win + 1;                   // sum items -> row items
+  static constexpr int Dc = L <= 1024 ? win + 1 : win;  // row items -> column items
+  static constexpr int slots = Dc + win + (L <= 1024 ? 1 : 0);  // intermediate frames
   static_assert(Dc < slots && slots <= kMaxSlots, "queue order must cover the slot reuse dependency");
 };
 
@@ -703,53 +667,62 @@ __global__ void __launch_bounds__(256) k_make_ref(const uint16_t* __restrict__ f
 // launchers
 // ------------------------------------------------------------------------------------------------
 template <int L>
+static bool configure_L(Ctx& c) {
+  using P = Plan<L>;
+  if (!NFS_CUDA(c, cudaFuncSetAttribute(k_fft<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem))) return false;
+  int per_sm = 0;
+  if (!NFS_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fft<L>, P::NT, P::smem))) return false;
+  c.fft_grid = std::max(1, per_sm) * std::max(1, c.n_sm);
+  return true;
+}
+
+template <int L>
 static int launch_fft_L(Ctx& c, const FftJob& job, int cls) {
   using P = Plan<L>;
-  if (c.fft_grid == 0) {
-    cudaFuncSetAttribute(k_fft<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem);
-    int per_sm = 0, dev = 0, sms = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fft<L>, P::NT, P::smem);
-    if (per_sm < 1) per_sm = 1;
-    c.fft_grid = per_sm * sms;
-  }
   const long long total = (long long)(job.nf + P::Dr + P::Dc) * P::perStep;
   const int grid = (int)std::min<long long>(c.fft_grid, total);
   ProfScope ps(c, cls);
-  cudaMemsetAsync(c.fft_cnt, 0, sizeof(unsigned) * (1 + 3 * (size_t)job.nf) + 0, c.stream);
-  cudaMemsetAsync(c.sums, 0, sizeof(unsigned long long) * (size_t)job.nf, c.stream);
+  if (!NFS_CUDA(c, cudaMemsetAsync(c.fft_cnt, 0, sizeof(unsigned) * (1 + 3 * (size_t)job.nf), c.stream))) return 0;
+  if (!NFS_CUDA(c, cudaMemsetAsync(c.sums, 0, sizeof(unsigned long long) * (size_t)job.nf, c.stream))) return 0;
   k_fft<L><<<grid, P::NT, P::smem, c.stream>>>(job);
+  NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
+#define NFS_FFT_SIZES(X) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096)
+
 static int launch_fft(Ctx& c, const FftJob& job, int cls) {
   switch (c.W) {
-    case 32: return launch_fft_L<32>(c, job, cls);
-    case 64: return launch_fft_L<64>(c, job, cls);
-    case 128: return launch_fft_L<128>(c, job, cls);
-    case 256: return launch_fft_L<256>(c, job, cls);
-    case 512: return launch_fft_L<512>(c, job, cls);
-    case 1024: return launch_fft_L<1024>(c, job, cls);
-    case 2048: return launch_fft_L<2048>(c, job, cls);
-    case 4096: return launch_fft_L<4096>(c, job, cls);
+#define X(L) \
+  case L: return launch_fft_L<L>(c, job, cls);
+    NFS_FFT_SIZES(X)
+#undef X
     default: return 0;
   }
 }
+
+// once at create: dynamic shared memory of the kernel for this frame size and its persistent grid
+bool fft_configure(Ctx& c) {
+  switch (c.W) {
+#define X(L) \
+  case L: return configure_L<L>(c);
+    NFS_FFT_SIZES(X)
+#undef X
+    default: return false;
+  }
+}
+
+size_t fft_cnt_elems(const Ctx& c) { return 1 + 3 * (size_t)c.B; }
 
 template <int L>
 static constexpr int slots_of() { return Plan<L>::slots; }
 size_t fft_rowT_elems(const Ctx& c) {
   int slots = kMaxSlots;
   switch (c.W) {
-    case 32: slots = slots_of<32>(); break;
-    case 64: slots = slots_of<64>(); break;
-    case 128: slots = slots_of<128>(); break;
-    case 256: slots = slots_of<256>(); break;
-    case 512: slots = slots_of<512>(); break;
-    case 1024: slots = slots_of<1024>(); break;
-    case 2048: slots = slots_of<2048>(); break;
-    case 4096: slots = slots_of<4096>(); break;
+#define X(L) \
+  case L: slots = slots_of<L>(); break;
+    NFS_FFT_SIZES(X)
+#undef X
     default: break;
   }
   return (size_t)slots * (size_t)c.P;
@@ -779,11 +752,12 @@ int launch_make_ref(Ctx& c, const uint16_t* frame0) {
   const int64_t npx = (int64_t)c.W * c.H;
   {
     ProfScope ps(c, kKSum);
-    cudaMemsetAsync(c.sums, 0, sizeof(unsigned long long), c.stream);
+    if (!NFS_CUDA(c, cudaMemsetAsync(c.sums, 0, sizeof(unsigned long long), c.stream))) return 0;
     int nblk = (int)std::min<int64_t>(592, (npx / 8 + 255) / 256);
     k_frame_sum<<<nblk, 256, 0, c.stream>>>(reinterpret_cast<const uint4*>(frame0), npx / 8, c.sums);
     nblk = (int)std::min<int64_t>(1184, (npx + 1023) / 1024);
     k_make_ref<<<nblk, 256, 0, c.stream>>>(frame0, npx, (float)c.W * (float)c.H, c.sums, c.ref, c.d_flags);
+    NFS_CUDA(c, cudaGetLastError());
   }
   FftJob j = make_job(c);
   j.dst = c.Fref;

@@ -2,121 +2,55 @@
 // for every new frame s of a batch and every requested lag tau ("only the square
 // moduli of FFT differences are evaluated N(N-1)/2 times"; L25 average over the measurement time).
 //
-// k_lag_tiled (default): a CTA works on 32 consecutive Fourier pixels and one group of lags at a time; a
-// producer warp streams the batch through shared memory with TMA tensor copies (cp.async.bulk.tensor +
-// mbarrier): a NEW stream (frames s) and an OLD stream delayed by the group's lags.  A consumer warp owns up to
-// kG lags: for a run of contiguous lags it keeps a rotating register window of the kG most recent OLD
-// frames, so one step costs two LDS.64 and kG pair-updates (packed sub.f32x2 + fma.rn.f32x2: two issue
-// slots per update); isolated lags take one LDS.64 per update.  fp32 partial sums are folded into the fp64
-// totals every kFoldChunks chunks and at the end of a tile (BASELINE.json north_star (4)).  One warp of the
-// lightest group also adds the batch to the I sums (sum |F'|^2, sum F').
-// Two launch shapes (template parameter PERS, chosen per batch by launch_lag_tiled): one CTA per (pixel tile,
-// lag group), or persistent CTAs that claim the pixel tiles of their group and keep the pipeline full across
-// tiles.  Results do not depend on the shape.
-// k_lag_simple: plain per-pixel kernel through L1/L2, kept as an in-library cross-check.
+// k_lag_tiled<NCW>: a CTA works on a tile of 4*NCW consecutive Fourier pixels (32 or 64) and one group of lags at
+// a time.  A producer warp streams the batch through shared memory with TMA tensor copies (cp.async.bulk.tensor +
+// mbarrier) into a ring of chunks that holds the lag window; the batch's own frames are the head of that ring
+// (single stream) or, for a group whose smallest lag is far away, a second stream.  A consumer warp owns 32 pixels
+// and one lag task:
+//   * a run of consecutive lags tau0 .. tau0+cnt-1 (cnt <= 13): the smallest lag is accumulated directly
+//     (|z_s - z_{s-tau0}|^2: sub.f32x2 + fma.rn.f32x2), every further lag through the difference of neighbouring lags
+//        |z_s - z_{o-1}|^2 - |z_s - z_o|^2 = |z_{o-1}|^2 - |z_o|^2 - 2 Re( conj(z_s) (z_{o-1} - z_o) ),   o = s - tau,
+//     i.e. ONE packed FMA per pair update on a rotating register window of the increments e_o = z_{o-1} - z_o; the
+//     |z|^2 terms telescope to two boundary values per lag and fold interval.  This halves the arithmetic of the
+//     dominant loop and, unlike the plain cross-term form, does not cancel in fp32: the
+//     accumulated quantity is the small difference between neighbouring lags itself;
+//   * a list of isolated lags (<= 6): one LDS.64 and the direct update per pair.
+// fp32 partial sums are folded into the fp64 totals every kFoldChunks chunks and at the end of a tile
+// (BASELINE.json north_star (4)).  One warp of the lightest group also adds the batch to the I sums (sum |F'|^2,
+// sum F').  Two launch shapes (template parameter PERS, chosen per batch by launch_lag_tiled): one CTA per (pixel
+// tile, lag group), or persistent CTAs that claim the pixel tiles of their group and keep the pipeline full across
+// tiles.  Results do not depend on the shape or on the tile width.
 #include <algorithm>
 
 #include "nfs_common.cuh"
 
 namespace nfs {
 
-__device__ __forceinline__ void upd(float2& acc, float2 zn, float2 zo) {
-  const float dx = zn.x - zo.x, dy = zn.y - zo.y;
-  acc.x = fmaf(dx, dx, acc.x);
-  acc.y = fmaf(dy, dy, acc.y);
-}
-
 // ------------------------------------------------------------------------------------------------
-// I accumulators: I2 += sum |F'_s|^2, I1 += sum F'_s over the batch (R9; static spectrum
-// is rebuilt at finalize as <|F'+F_r|^2>).  One thread per pixel, fp32 partials folded every 64 steps.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_accum_I(const float2* __restrict__ ring, int R, int64_t P, int64_t t0, int b,
-                                                 double* __restrict__ I2, double2* __restrict__ I1) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= P) return;
-  double d2 = 0.0, dx = 0.0, dy = 0.0;
-  int slot = (int)(t0 % R);
-  for (int j0 = 0; j0 < b; j0 += 64) {
-    float a2 = 0.f, ax = 0.f, ay = 0.f;
-    const int je = min(b, j0 + 64);
-    for (int j = j0; j < je; ++j) {
-      const float2 z = __ldcs(&ring[(int64_t)slot * P + p]);
-      a2 = fmaf(z.x, z.x, fmaf(z.y, z.y, a2));
-      ax += z.x;
-      ay += z.y;
-      if (++slot == R) slot = 0;
-    }
-    d2 += (double)a2;
-    dx += (double)ax;
-    dy += (double)ay;
-  }
-  I2[p] += d2;
-  double2 v = I1[p];
-  v.x += dx;
-  v.y += dy;
-  I1[p] = v;
-}
-
-// ------------------------------------------------------------------------------------------------
-// plain kernel: thread = (pixel, 8 consecutive lag indices); grid (ceil(P/128), ceil(n_lags/8))
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_lag_simple(const float2* __restrict__ ring, int R, int64_t P, int64_t t0, int b,
-                                                    const int32_t* __restrict__ lags, int n_lags,
-                                                    double* __restrict__ totals) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= P) return;
-  const int l0 = blockIdx.y * 8;
-  int tau[8];
-  float2 acc[8];
-#pragma unroll
-  for (int g = 0; g < 8; ++g) {
-    tau[g] = (l0 + g < n_lags) ? lags[l0 + g] : 0x7fffffff;
-    acc[g] = make_float2(0.f, 0.f);
-  }
-  for (int j = 0; j < b; ++j) {
-    const int64_t s = t0 + j;
-    const float2 zn = ring[(s % R) * P + p];
-#pragma unroll
-    for (int g = 0; g < 8; ++g) {
-      if (s >= tau[g]) {
-        const float2 zo = ring[((s - tau[g]) % R) * P + p];
-        upd(acc[g], zn, zo);
-      }
-    }
-  }
-#pragma unroll
-  for (int g = 0; g < 8; ++g)
-    if (l0 + g < n_lags) totals[(int64_t)(l0 + g) * P + p] += (double)(acc[g].x + acc[g].y);
-}
-
-// ------------------------------------------------------------------------------------------------
-// tiled kernel: warp-specialised.  Warps 0..kMaxTasks-1 = consumers (one lag task each, placed by the
-// plan so that the four SM sub-partitions carry equal work), the last warp = producer (highest warp
-// id: first in the issue arbiter, so loads are never starved by the math warps).
-// Time is cut into chunks of kChunk = 2*kG steps.  Shared memory, in rows of 32 pixels (256 B):
+// Warp-specialised kernel.  Warps 0..NCW-1 = consumers (warp w: task slot w & 7, 32-pixel sub-tile w >> 3; the plan
+// places tasks on slots so that the four SM sub-partitions carry equal work), the last warp = producer (highest
+// warp id: first in the issue arbiter, so loads are never starved by the math warps).
+// Time is cut into chunks of kChunk = 2*kG steps.  Shared memory, in rows of TPX pixels (8 B each):
 //   OLD  [(NSLOT + 1) * kChunk]  ring of NSLOT = LEAD + stages chunk slots; OLD row e holds frame
-//                                E0 + e, E0 = t0 - tau_min - LEAD*kChunk, at row e % (NSLOT*kChunk); the
-//                                last kChunk rows duplicate slot 0 so kG consecutive rows never wrap
-//   NEW  [stages * kChunk]       the batch's own frames, chunk c in stage c % stages
+//                                E0 + e, E0 = t0 - tau_lo - LEAD*kChunk, at row e % (NSLOT*kChunk); the
+//                                last kChunk rows duplicate slot 0 so that up to kChunk consecutive rows never wrap.
+//                                tau_lo = 0 for a single-stream group (the batch's frames are "lag 0" of the window),
+//                                else the group's smallest lag; LEAD = window span in chunks
+//   NEW  [stages * kChunk]       two-stream groups only: the batch's own frames, chunk c in stage c % stages
 // full[stage]: the producer's arrival + the bytes of its copies for one pipeline step; empty[stage]: the
-// consumer warps.  One tile per CTA: step = consumer chunk c (NEW chunk c, OLD chunk c + LEAD; chunk 0 also
+// consumer warps.  One tile per CTA: step = consumer chunk c (OLD chunk c + LEAD, NEW chunk c; chunk 0 also
 // brings OLD chunks 0..LEAD-1).  Persistent: every tile has LEAD prologue steps that bring one OLD chunk each,
 // then one step per chunk (OLD chunk j, NEW chunk j - LEAD); steps and ring slots are numbered through all the
 // tiles of the CTA, so the next tile's window streams in while the last chunks of the current one are consumed.
-// `stages` (2..kMaxStages) is chosen at create from the shared memory the widest lag group leaves, so
-// that the producer runs several chunks (each ~3 us of math) ahead of the HBM/L2 latency.
-// A chunk of frames that is contiguous in the HBM ring is one 2-D TMA box (cp.async.bulk.tensor,
-// 32 pixels x kChunk ring slots); a chunk that straddles the ring's wrap-around or starts before the
-// first frame falls back to one 256-byte bulk copy per row.
+// A chunk of frames that is contiguous in the HBM ring is one 2-D TMA box (TPX pixels x kChunk ring slots); a chunk
+// that straddles the ring's wrap-around or starts before the first frame falls back to one bulk copy per row.
 // ------------------------------------------------------------------------------------------------
-constexpr int kRowF2 = kTilePx;                 // float2 per shared-memory row (one frame, 32 pixels = 256 B)
-constexpr unsigned kRowBytes = kRowF2 * 8u;
+__host__ __device__ inline int lag_lead(int tau_lo, int tau_max) { return (tau_max - tau_lo + kChunk - 1) / kChunk; }
+__host__ __device__ inline int lag_tau_lo(const LagGroup& g) { return (g.flags & 2) ? 0 : g.tau_min; }
 
-__host__ __device__ inline int lag_lead(int tau_min, int tau_max) { return (tau_max - tau_min + kChunk - 1) / kChunk; }
-
-static size_t lag_smem_bytes(int tau_min, int tau_max, int stages) {
-  const int nslot = lag_lead(tau_min, tau_max) + stages;
-  return 128 + sizeof(float2) * kRowF2 * (size_t)((nslot + 1) * kChunk + stages * kChunk);
+static size_t lag_smem_bytes(int tau_lo, int tau_max, bool single, int stages, int tpx) {
+  const int nslot = lag_lead(tau_lo, tau_max) + stages;
+  return 128 + sizeof(float2) * (size_t)tpx * (size_t)((nslot + 1) * kChunk + (single ? 0 : stages * kChunk));
 }
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -129,10 +63,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-#ifndef NFS_LAG_PROD_HINT_NS
-#define NFS_LAG_PROD_HINT_NS 20000
-#endif
-// producer side: same wait with a suspend-time hint, so that the idle warp does not burn issue slots
+// producer side: wait with a suspend-time hint, so that the idle warp does not burn issue slots
 __device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, unsigned parity) {
   asm volatile(
       "{\n"
@@ -143,7 +74,7 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t* bar, unsigned parity
       "bra WAITR_%=;\n"
       "DONER_%=:\n"
       "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity), "r"((unsigned)NFS_LAG_PROD_HINT_NS)
+      "r"(parity), "r"(20000u)
       : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
@@ -166,7 +97,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
-// 2-D tensor copy global -> shared (SASS UTMALDG): box = 32 pixels (64 floats) x kChunk ring slots
+// 2-D tensor copy global -> shared (SASS UTMALDG): box = TPX pixels (2 TPX floats) x kChunk ring slots
 __device__ __forceinline__ void tma_box_g2s(void* dst, const CUtensorMap* tmap, int c0, int c1, uint64_t* bar) {
   asm volatile(
       "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(
@@ -196,14 +127,17 @@ __device__ __forceinline__ void upd2(f2x& acc, f2x zn, f2x zo) {
   const f2x d = sub2(zn, zo);
   acc = fma2(d, d, acc);
 }
-__device__ __forceinline__ float f2x_sum(f2x v) {
-  return __uint_as_float((unsigned)(v & 0xffffffffull)) + __uint_as_float((unsigned)(v >> 32));
-}
+__device__ __forceinline__ float f2x_lo(f2x v) { return __uint_as_float((unsigned)(v & 0xffffffffull)); }
+__device__ __forceinline__ float f2x_hi(f2x v) { return __uint_as_float((unsigned)(v >> 32)); }
+__device__ __forceinline__ float f2x_sum(f2x v) { return f2x_lo(v) + f2x_hi(v); }
+__device__ __forceinline__ double norm2_f64(float2 z) { return (double)z.x * (double)z.x + (double)z.y * (double)z.y; }
 
 // producer: bring frames f0 .. f0+kChunk-1 of this pixel tile into shared rows dst (and dup, if given).
 // Returns the bytes this lane's copies will complete on the barrier.
+template <int TPX>
 __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const float2* __restrict__ ring, int R, int64_t P,
                                                int64_t p0, int64_t f0, f2x* dst, f2x* dup, uint64_t* bar, int lane) {
+  constexpr unsigned kRowBytes = TPX * 8u;
   const int s0 = (int)(((f0 % R) + R) % R);
   if (f0 >= 0 && s0 + kChunk <= R) {
     if (lane != 0) return 0u;
@@ -216,10 +150,10 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
     const int64_t f = f0 + lane;
     if (f >= 0) {  // rows before the first frame are never used
       const float2* src = ring + (f % R) * P + p0;
-      bulk_g2s(dst + (size_t)lane * kRowF2, src, kRowBytes, bar);
+      bulk_g2s(dst + (size_t)lane * TPX, src, kRowBytes, bar);
       bytes = kRowBytes;
       if (dup) {
-        bulk_g2s(dup + (size_t)lane * kRowF2, src, kRowBytes, bar);
+        bulk_g2s(dup + (size_t)lane * TPX, src, kRowBytes, bar);
         bytes += kRowBytes;
       }
     }
@@ -227,77 +161,104 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
   return bytes;
 }
 
-// One block of kG steps of a dense task with exactly CNT lags: step u loads the new frame and the one
-// OLD frame entering the rotating window (2 LDS.64), then CNT pair updates out of registers.
-template <int CNT>
-__device__ __forceinline__ void dense_block(f2x (&acc)[kG], f2x (&w)[kG], const f2x* nb, const f2x* ob) {
+// ---- register-window task with exactly CNT lags: one whole chunk in which every pair of every step exists ----
+// acc[0]: direct sum of the smallest lag; acc[g], g >= 1: cross sum X_{g-1} = sum_s Re(conj(z_s) e_{s - tau0 - (g-1)});
+// w: the 13 most recent increments e_o = z_{o-1} - z_o of the OLD stream o = s - tau0; zprev = z_{o-1}.
+// Per step: 2 LDS.64 (issued one step ahead), the increment, the direct update (2) and CNT - 1 packed FMAs.  The
+// chunk's kChunk OLD rows are contiguous (the ring's slot 0 is duplicated behind its last slot).
+template <int CNT, int TPX>
+__device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid, const f2x* newc,
+                                            const f2x* oldl, int& o0, int DEPTH) {
+  if (!wvalid) {  // (re)build the window: the increments of the CNT-2 OLD frames that precede the chunk's first one
+    int r = o0 - (CNT - 1);
+    if (r < 0) r += DEPTH;
+    f2x zz = oldl[(size_t)r * TPX];
 #pragma unroll
-  for (int u = 0; u < kG; ++u) {
-    const f2x zn = nb[(size_t)u * kRowF2];
-    w[u] = ob[(size_t)u * kRowF2];
+    for (int k = CNT - 2; k >= 1; --k) {
+      if (++r == DEPTH) r = 0;
+      const f2x zk = oldl[(size_t)r * TPX];
+      w[kG - k] = sub2(zz, zk);
+      zz = zk;
+    }
+    zprev = zz;  // z of the OLD frame just before the chunk's first one
+    wvalid = true;
+  }
+  const f2x* ob = oldl + (size_t)o0 * TPX;
+  f2x zn = newc[0], zo = ob[0];
 #pragma unroll
-    for (int g = 0; g < CNT; ++g) upd2(acc[g], zn, w[(u - g + kG) % kG]);
+  for (int u = 0; u < kChunk; ++u) {
+    f2x zn1 = zn, zo1 = zo;
+    if (u + 1 < kChunk) {  // next step's operands: in flight while this step's FMAs issue
+      zn1 = newc[(size_t)(u + 1) * TPX];
+      zo1 = ob[(size_t)(u + 1) * TPX];
+    }
+    w[u % kG] = sub2(zprev, zo);
+    zprev = zo;
+    upd2(acc[0], zn, zo);
+#pragma unroll
+    for (int g = 1; g < CNT; ++g) acc[g] = fma2(zn, w[(u - (g - 1) + 2 * kG) % kG], acc[g]);
+    zn = zn1;
+    zo = zo1;
   }
+  o0 += kChunk;
+  if (o0 >= DEPTH) o0 -= DEPTH;
 }
-// ---- whole chunks (kChunk = kChunk/kG blocks) in which every pair of every step exists: the common case ----
-template <int CNT>
-__device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int& o0,
-                                            int DEPTH) {
-#pragma unroll 1
-  for (int blk = 0; blk < kChunk / kG; ++blk) {
-    dense_block<CNT>(acc, w, newc + (size_t)blk * kG * kRowF2, oldl + (size_t)o0 * kRowF2);
-    o0 += kG;
-    if (o0 >= DEPTH) o0 -= DEPTH;
-  }
-}
-__device__ __forceinline__ void dense_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
-                                                     int& o0, int DEPTH) {
+template <int TPX>
+__device__ __forceinline__ void dense_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid,
+                                                     const f2x* newc, const f2x* oldl, int& o0, int DEPTH) {
   switch (cnt) {  // warp-uniform; the plan makes dense tasks of kDenseMin..kG lags
-    case 12: dense_chunk<12>(acc, w, newc, oldl, o0, DEPTH); break;
-    case 11: dense_chunk<11>(acc, w, newc, oldl, o0, DEPTH); break;
-    case 10: dense_chunk<10>(acc, w, newc, oldl, o0, DEPTH); break;
-    case 9: dense_chunk<9>(acc, w, newc, oldl, o0, DEPTH); break;
-    case 8: dense_chunk<8>(acc, w, newc, oldl, o0, DEPTH); break;
-    case 7: dense_chunk<7>(acc, w, newc, oldl, o0, DEPTH); break;
-    default: dense_chunk<kG>(acc, w, newc, oldl, o0, DEPTH); break;  // 13 (shorter runs: surplus lags are discarded)
+    case 2: dense_chunk<2, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 3: dense_chunk<3, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 4: dense_chunk<4, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 5: dense_chunk<5, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 6: dense_chunk<6, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 7: dense_chunk<7, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 8: dense_chunk<8, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 9: dense_chunk<9, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 10: dense_chunk<10, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 11: dense_chunk<11, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    case 12: dense_chunk<12, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+    default: dense_chunk<kG, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
   }
 }
-template <int CNT>
+// ---- lag-list task with exactly CNT lags, whole chunk: the low word of w[i] holds the OLD row of lag i; its
+// kChunk rows are contiguous (duplicated slot 0) ----
+template <int CNT, int TPX>
 __device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH) {
-#pragma unroll 1
-  for (int blk = 0; blk < kChunk / kG; ++blk) {
-    const f2x* nb = newc + (size_t)blk * kG * kRowF2;
+  const f2x* ol[CNT];
 #pragma unroll
-    for (int u = 0; u < kG; ++u) {
-      const f2x zn = nb[(size_t)u * kRowF2];
+  for (int i = 0; i < CNT; ++i) ol[i] = oldl + (size_t)(unsigned)w[i] * TPX;
 #pragma unroll
-      for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
-    }
+  for (int u = 0; u < kChunk; ++u) {
+    const f2x zn = newc[(size_t)u * TPX];
 #pragma unroll
-    for (int i = 0; i < CNT; ++i) {
-      unsigned o = (unsigned)w[i] + kG;
-      if (o >= (unsigned)DEPTH) o -= DEPTH;
-      w[i] = (f2x)o;
-    }
+    for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, ol[i][(size_t)u * TPX]);
+  }
+#pragma unroll
+  for (int i = 0; i < CNT; ++i) {
+    unsigned o = (unsigned)w[i] + kChunk;
+    if (o >= (unsigned)DEPTH) o -= DEPTH;
+    w[i] = (f2x)o;
   }
 }
+template <int TPX>
 __device__ __forceinline__ void sparse_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
                                                       int DEPTH) {
   switch (cnt) {
     case 0: break;  // a task that only accumulates the I sums
-    case 1: sparse_chunk<1>(acc, w, newc, oldl, DEPTH); break;
-    case 2: sparse_chunk<2>(acc, w, newc, oldl, DEPTH); break;
-    case 3: sparse_chunk<3>(acc, w, newc, oldl, DEPTH); break;
-    case 4: sparse_chunk<4>(acc, w, newc, oldl, DEPTH); break;
-    case 5: sparse_chunk<5>(acc, w, newc, oldl, DEPTH); break;
-    default: sparse_chunk<kSparseMax>(acc, w, newc, oldl, DEPTH); break;  // the plan makes lag lists of <= kSparseMax
+    case 1: sparse_chunk<1, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 2: sparse_chunk<2, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 3: sparse_chunk<3, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 4: sparse_chunk<4, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 5: sparse_chunk<5, TPX>(acc, w, newc, oldl, DEPTH); break;
+    default: sparse_chunk<kSparseMax, TPX>(acc, w, newc, oldl, DEPTH); break;  // the plan makes lag lists of <= kSparseMax
   }
 }
 
 // One block of a lag-list task with exactly CNT lags in which some pairs do not exist (warm-up: the OLD
 // frame would precede the first frame; or the batch's ragged tail): pair (step u, lag i) is counted iff
 // u >= u0_i = lag_i - (frame number of step 0), and u < ns.
-template <int CNT>
+template <int CNT, int TPX>
 __device__ __forceinline__ void sparse_masked(int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb, const f2x* oldl,
                                               const int* my_lags, int64_t frame0) {
   int u0[CNT];
@@ -306,82 +267,112 @@ __device__ __forceinline__ void sparse_masked(int ns, f2x (&acc)[kG], const f2x 
 #pragma unroll
   for (int u = 0; u < kG; ++u) {
     if (u < ns) {
-      const f2x zn = nb[(size_t)u * kRowF2];
+      const f2x zn = nb[(size_t)u * TPX];
 #pragma unroll
       for (int i = 0; i < CNT; ++i)
-        if (u >= u0[i]) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * kRowF2]);
+        if (u >= u0[i]) upd2(acc[i], zn, oldl[(size_t)((unsigned)w[i] + u) * TPX]);
     }
   }
 }
+template <int TPX>
 __device__ __forceinline__ void sparse_masked_dispatch(int cnt, int ns, f2x (&acc)[kG], const f2x (&w)[kG], const f2x* nb,
                                                        const f2x* oldl, const int* my_lags, int64_t frame0) {
   switch (cnt) {
     case 0: break;
-    case 1: sparse_masked<1>(ns, acc, w, nb, oldl, my_lags, frame0); break;
-    case 2: sparse_masked<2>(ns, acc, w, nb, oldl, my_lags, frame0); break;
-    case 3: sparse_masked<3>(ns, acc, w, nb, oldl, my_lags, frame0); break;
-    case 4: sparse_masked<4>(ns, acc, w, nb, oldl, my_lags, frame0); break;
-    case 5: sparse_masked<5>(ns, acc, w, nb, oldl, my_lags, frame0); break;
-    default: sparse_masked<kSparseMax>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 1: sparse_masked<1, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 2: sparse_masked<2, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 3: sparse_masked<3, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 4: sparse_masked<4, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    case 5: sparse_masked<5, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
+    default: sparse_masked<kSparseMax, TPX>(ns, acc, w, nb, oldl, my_lags, frame0); break;
   }
 }
 
-template <bool PERS, bool SKIP>
-__global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
+// Fold of a register-window task after whole chunks: S(tau0) directly; S(tau + 1) = S(tau) - 2 X + |z_{sa - tau - 1}|^2
+// - |z_{sb - tau}|^2 over the steps sa..sb of the whole chunks since the segment opened.  The first |z|^2 went into
+// the totals when the segment opened, the second is the OLD row oend - g of the step after the last whole chunk (that
+// chunk's window is still resident: call before the chunk that follows is released), everything in fp64.
+template <int TPX>
+__device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* oldl, int oend, int DEPTH, double* tot,
+                                           int64_t P, int64_t p) {
+  double run = (double)f2x_sum(acc[0]);
+  atomicAdd(&tot[p], run);
+  int r = oend;
+#pragma unroll
+  for (int g = 1; g < kG; ++g) {
+    if (g < cnt) {
+      if (--r < 0) r += DEPTH;
+      const f2x z = oldl[(size_t)r * TPX];
+      run -= 2.0 * (double)f2x_sum(acc[g]) + norm2_f64(make_float2(f2x_lo(z), f2x_hi(z)));
+      atomicAdd(&tot[(int64_t)g * P + p], run);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < kG; ++g) acc[g] = 0ull;
+}
+
+template <int NCW, bool PERS, bool SKIP>
+__global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 registers: 5 warps per SM sub-partition
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P,
-                int64_t t0_batch, int b_batch, int ngroups, int stages, const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups,
-                const int32_t* __restrict__ lags, double* __restrict__ totals, double* __restrict__ I2,
-                double2* __restrict__ I1, int ntiles, int* __restrict__ claim) {
+                int64_t t0_batch, int b_batch, int gbase, int ngroups, int lbase, int stages,
+                const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups, const int32_t* __restrict__ lags,
+                double* __restrict__ totals, double* __restrict__ I2, double2* __restrict__ I1, int ntiles,
+                int* __restrict__ claim) {
   constexpr int G = kG;
+  constexpr int TPX = NCW * 4;  // pixels per tile: one 32-pixel sub-tile per 8 consumer warps
+  static_assert(NCW == 8 || NCW == 16, "8 task slots x 1 or 2 sub-tiles");
   static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
   static_assert(kSparseMax == 6, "sparse_chunk_dispatch lists cases 0..5 and the default");
-  static_assert(kMaxTasks <= 16 && kMaxTasks % 4 == 0, "warp_task[16], whole sub-partition rounds");
+  static_assert(kTaskSlots == 8, "warp_task[], sub-tile = warp >> 3");
   extern __shared__ __align__(128) unsigned char smraw[];
-  __shared__ int s_lags[kMaxTasks * kG];  // the lags of each sparse task, for the warm-up path
-  __shared__ int s_tile[kMaxStages];      // tile of the item whose first step uses this stage, or -1: no more work
+  __shared__ int s_lags[NCW * kG];  // the lags of each sparse task, for the warm-up path
+  __shared__ int s_tile[kMaxStages];  // tile of the item whose first step uses this stage, or -1: no more work
   // persistent launch: group gi owns CTAs [cta0, cta0 + nctas), which claim the group's pixel tiles one after
   // the other (claim[gi], zeroed before the launch) and run through them without draining the shared-memory
   // pipeline.  One-tile launch: CTA = (tile, group), the groups of a tile side by side (they share L2 lines).
-  int gi = 0;
+  int gi = gbase;
   if constexpr (PERS) {
-    while (gi + 1 < ngroups && (int)blockIdx.x >= groups[gi].cta0 + groups[gi].nctas) ++gi;
+    while (gi + 1 < gbase + ngroups && (int)blockIdx.x >= groups[gi].cta0 + groups[gi].nctas) ++gi;
   } else {
-    gi = blockIdx.x % ngroups;
+    gi = gbase + blockIdx.x % ngroups;
   }
   const LagGroup& grp = groups[gi];
   const int tau_min = grp.tau_min, tau_max = grp.tau_max;
+  const bool withI = (grp.flags & 1) != 0;
+  const bool single = (grp.flags & 2) != 0;
   // no frame pair of this group exists yet (the group that accumulates the I sums always runs)
-  if (grp.flags == 0 && (int64_t)tau_min > t0_batch + b_batch - 1) return;
+  if (!withI && (int64_t)tau_min > t0_batch + b_batch - 1) return;
   // SKIP (launched only while some group's smallest lag still reaches back before frame 0): such a group skips
   // the whole chunks in which it has no pair, i.e. it works on the batch cut at the front (the I sums need every
   // frame: that group keeps the whole batch).  Otherwise t0 and b stay kernel parameters (no registers).
   int64_t t0 = t0_batch;
   int b = b_batch;
   if constexpr (SKIP) {
-    if (grp.flags == 0 && (int64_t)tau_min > t0) {
+    if (!withI && (int64_t)tau_min > t0) {
       const int skip = (int)(((int64_t)tau_min - t0) / kChunk) * kChunk;
       t0 += skip;
       b -= skip;
     }
   }
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int LEAD = lag_lead(tau_min, tau_max);
+  const int tau_lo = single ? 0 : tau_min;
+  const int LEAD = lag_lead(tau_lo, tau_max);
   const int NSLOT = LEAD + stages;
   const int DEPTH = NSLOT * kChunk;
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw);      // [kMaxStages]
   uint64_t* empty = full + kMaxStages;                      // [kMaxStages]
   static_assert(2 * kMaxStages * 8 <= 128, "barriers fit the 128-byte header");
-  f2x* OLD = reinterpret_cast<f2x*>(smraw + 128);           // [(NSLOT + 1) * kChunk][32]
-  f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * kRowF2;   // [stages][kChunk][32]
+  f2x* OLD = reinterpret_cast<f2x*>(smraw + 128);           // [(NSLOT + 1) * kChunk][TPX]
+  f2x* NEW = OLD + (size_t)(NSLOT + 1) * kChunk * TPX;      // [stages][kChunk][TPX], two-stream groups only
   const int nchunks = (b + kChunk - 1) / kChunk;
   // One item (pixel tile) = LEAD prologue steps that only bring OLD chunks (the window), then nchunks steps that
-  // bring OLD chunk j and NEW chunk j - LEAD and are consumed.  Steps are numbered through all items of the
+  // bring OLD chunk j (and NEW chunk j - LEAD) and are consumed.  Steps are numbered through all items of the
   // CTA: step v uses pipeline stage v % stages and puts its OLD chunk into ring slot v % NSLOT, which held the
   // OLD chunk of step v - NSLOT = v - LEAD - stages, last read by the consumers at step v - stages.
   const int V = nchunks + LEAD;
 
   if (tid == 0) {
-    const unsigned nt = (unsigned)grp.ntasks;
+    const unsigned nt = (unsigned)grp.ntasks * (NCW / kTaskSlots);
     for (int s = 0; s < stages; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], nt);
@@ -390,9 +381,9 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   }
   __syncthreads();
 
-  if (warp == kMaxTasks) {
+  if (warp == NCW) {
     // ------------------------------- producer -------------------------------
-    const int64_t E0 = t0 - tau_min - (int64_t)LEAD * kChunk;  // frame held by row 0 of an item's OLD chunk 0
+    const int64_t E0 = t0 - tau_lo - (int64_t)LEAD * kChunk;  // frame held by row 0 of an item's OLD chunk 0
     int st = 0, slot = 0;
     unsigned ph = 0;  // parity of this stage's current use
     if constexpr (PERS) {
@@ -408,16 +399,16 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
           }
           break;
         }
-        const int64_t p0 = (int64_t)tile * kTilePx;
+        const int64_t p0 = (int64_t)tile * TPX;
         for (int j = 0; j < V; ++j) {
           mbar_wait_relaxed(&empty[st], ph ^ 1u);  // passes at once on the first use of a stage
           if (j == 0 && lane == 0) s_tile[st] = tile;  // ordered before the consumers' read by the arrive below
-          f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
-          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
-          unsigned bytes = load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)j * kChunk, dst, dup, &full[st], lane);
-          if (j >= LEAD)
-            bytes += load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)(j - LEAD) * kChunk,
-                                NEW + (size_t)st * kChunk * kRowF2, nullptr, &full[st], lane);
+          f2x* dst = OLD + (size_t)slot * kChunk * TPX;
+          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * TPX : nullptr;
+          unsigned bytes = load_chunk<TPX>(&tmap, ring, R, P, p0, E0 + (int64_t)j * kChunk, dst, dup, &full[st], lane);
+          if (!single && j >= LEAD)
+            bytes += load_chunk<TPX>(&tmap, ring, R, P, p0, t0 + (int64_t)(j - LEAD) * kChunk,
+                                     NEW + (size_t)st * kChunk * TPX, nullptr, &full[st], lane);
           bytes = __reduce_add_sync(0xffffffffu, bytes);
           if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
           if (++st == stages) st = 0, ph ^= 1u;
@@ -426,15 +417,17 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
       }
     } else {
       // one pixel tile: the whole window (OLD chunks 0..LEAD) comes with the first chunk, no prologue steps
-      const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * kTilePx;
+      const int64_t p0 = (int64_t)(blockIdx.x / ngroups) * TPX;
       for (int c = 0; c < nchunks; ++c) {
         if (c >= stages) mbar_wait_relaxed(&empty[st], ph ^ 1u);
-        unsigned bytes = load_chunk(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * kRowF2,
-                                    nullptr, &full[st], lane);
+        unsigned bytes = 0;
+        if (!single)
+          bytes = load_chunk<TPX>(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * TPX, nullptr,
+                                  &full[st], lane);
         for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
-          f2x* dst = OLD + (size_t)slot * kChunk * kRowF2;
-          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * kRowF2 : nullptr;
-          bytes += load_chunk(&tmap, ring, R, P, p0, E0 + (int64_t)m * kChunk, dst, dup, &full[st], lane);
+          f2x* dst = OLD + (size_t)slot * kChunk * TPX;
+          f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * TPX : nullptr;
+          bytes += load_chunk<TPX>(&tmap, ring, R, P, p0, E0 + (int64_t)m * kChunk, dst, dup, &full[st], lane);
           if (++slot == NSLOT) slot = 0;
         }
         bytes = __reduce_add_sync(0xffffffffu, bytes);
@@ -446,40 +439,44 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   }
 
   // ------------------------------- consumers -------------------------------
-  const int tix = grp.warp_task[warp];
+  const int sub = warp >> 3;  // 32-pixel sub-tile of this warp
+  const int tix = grp.warp_task[warp & (kTaskSlots - 1)];
   if (tix < 0) return;
   const LagTask tk = tasks[grp.task0 + tix];
   const bool dense = (tk.kind & 1) == 0;
-  const bool doI = (tk.kind & 2) != 0;  // this warp also accumulates I2 += |F'_s|^2, I1 += F'_s (group 0 only)
+  const bool doI = (tk.kind & 2) != 0;  // this warp also accumulates I2 += |F'_s|^2, I1 += F'_s (one group only)
   const int cnt = tk.cnt;
-  f2x i2 = 0ull, i1 = 0ull;             // fp32 partials of the batch (<= 1024 terms, like acc)
-  // acc: fp32 partial sums (re^2 and im^2 lanes, packed).  Dense task: w = rotating window of the G most
-  // recent OLD frames.  Sparse task: the low word of w[i] holds the OLD row of lag i at the block start.
+  f2x i2 = 0ull, i1 = 0ull;             // fp32 partials of the I sums (<= kFoldChunks * kChunk terms, like acc)
+  // Dense task: acc[0] direct sum of lag tau0, acc[g] cross sum of lag tau0 + g against tau0 + g - 1; w = rotating
+  // window of the G most recent increments of the OLD stream.  Sparse task: acc[i] direct sum of lag i; the low
+  // word of w[i] holds the OLD row of lag i at the block start.
   f2x acc[G], w[G];
+  f2x zprev = 0ull;
 #pragma unroll
   for (int g = 0; g < G; ++g) acc[g] = 0ull, w[g] = 0ull;
   // OLD row (before the ring modulo) of the frame that lag tau pairs with step j:  j + offbase - tau
-  const int offbase = LEAD * kChunk + tau_min;
+  const int offbase = LEAD * kChunk + tau_lo;
   int o0 = 0;           // dense: ring row of frame (t0 + jb - tau0) at the current block start
   bool wvalid = false;  // dense: the register window matches the current block start
-  int tau_lo, tau_hi;   // smallest / largest lag of the task
+  int tau_lo_t, tau_hi_t;  // smallest / largest lag of the task
   if (dense) {
-    tau_lo = tk.tau0;
-    tau_hi = tk.tau0 + cnt - 1;
+    tau_lo_t = tk.tau0;
+    tau_hi_t = tk.tau0 + cnt - 1;
   } else if (cnt == 0) {  // I sums only
-    tau_lo = tau_hi = 0;
+    tau_lo_t = tau_hi_t = 0;
   } else {
-    tau_lo = lags[tk.l0];
-    tau_hi = lags[tk.l0 + cnt - 1];
+    tau_lo_t = lags[tk.l0];
+    tau_hi_t = lags[tk.l0 + cnt - 1];
 #pragma unroll
     for (int i = 0; i < G; ++i)
       if (i < cnt && lane == 0) s_lags[warp * G + i] = lags[tk.l0 + i];  // read back by this warp only
   }
   __syncwarp();
   // batch-relative step from which every lag (j_all) / any lag (j_any) of the task has a frame pair
-  const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi - t0));
-  const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo - t0));
-  const f2x* oldl = OLD + lane;
+  const int j_all = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_hi_t - t0));
+  const int j_any = (int)min((int64_t)1 << 30, max((int64_t)0, (int64_t)tau_lo_t - t0));
+  const f2x* oldl = OLD + sub * 32 + lane;
+  double* tot = totals + (int64_t)(tk.l0 - lbase) * P;  // row of the task's first lag
 
   int st = 0, slot0 = 0;  // slot0: ring slot of the current item's OLD chunk 0
   unsigned ph = 0;
@@ -492,7 +489,7 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     if (tile < 0) break;
     waited = true;
   }
-  const int64_t p = (int64_t)tile * kTilePx + lane;
+  const int64_t p = (int64_t)tile * TPX + sub * 32 + lane;
   // per-item state: OLD rows of the item's first step
   const int base_row = slot0 * kChunk + offbase;
   wvalid = false;
@@ -503,6 +500,8 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
     for (int i = 0; i < G; ++i)
       if (i < cnt) w[i] = (f2x)(unsigned)((base_row - s_lags[warp * G + i]) % DEPTH);
   }
+  int nslot = slot0 + LEAD;  // single stream: ring slot of the item's NEW chunk 0 (= OLD chunk LEAD)
+  if (nslot >= NSLOT) nslot -= NSLOT;
   slot0 = (slot0 + V) % NSLOT;
   // prologue steps: the window is being filled, nothing to consume
 #pragma unroll 1
@@ -515,11 +514,14 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   }
   for (int cseg = 0; cseg < nchunks; cseg += kFoldChunks) {  // fp32 partial sums span one segment of chunks
   const int cend = min(nchunks, cseg + kFoldChunks);
+  bool open = false;  // dense: whole chunks have been accumulated in this segment (their boundary terms are open)
+  int oend = 0;       // dense: OLD row of the step after the segment's last whole chunk
 #pragma unroll 1
   for (int c = cseg; c < cend; ++c) {
     if (!waited) mbar_wait(&full[st], ph);
     waited = false;
-    const f2x* newc = NEW + (size_t)st * kChunk * kRowF2 + lane;
+    const f2x* newc = (single ? OLD + (size_t)nslot * kChunk * TPX : NEW + (size_t)st * kChunk * TPX) + sub * 32 + lane;
+    if (++nslot == NSLOT) nslot = 0;
     const int j0 = c * kChunk;
     if (j0 >= j_all && j0 + kChunk <= b) {
       // ---- fast chunk: every pair of every step exists ----
@@ -528,72 +530,79 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
         for (int blk = 0; blk < kChunk / G; ++blk) {
 #pragma unroll
           for (int u = 0; u < G; ++u) {
-            const f2x zn = newc[(size_t)(blk * G + u) * kRowF2];
+            const f2x zn = newc[(size_t)(blk * G + u) * TPX];
             i2 = fma2(zn, zn, i2);
             i1 = add2(i1, zn);
           }
         }
       }
       if (dense) {
-        if (!wvalid) {  // (re)load the window: the G-1 OLD frames that precede the chunk's first one
+        if (!open) {
+          // first whole chunk of the segment: the |z|^2 of the OLD frames just before it enter the totals of the
+          // further lags (they telescope against the ones subtracted at the fold): lag tau0 + g gets
+          // sum_{k=1..g} |z_{o0-k}|^2, in fp64
+          open = true;
+          double pre = 0.0;
+          int r = o0;
 #pragma unroll
-          for (int q = 1; q < G; ++q) {
-            int r = o0 - q;
-            if (r < 0) r += DEPTH;
-            w[G - q] = oldl[(size_t)r * kRowF2];
+          for (int g = 1; g < G; ++g) {
+            if (g < cnt) {
+              if (--r < 0) r += DEPTH;
+              const f2x z = oldl[(size_t)r * TPX];
+              pre += norm2_f64(make_float2(f2x_lo(z), f2x_hi(z)));
+              if (p < P) atomicAdd(&tot[(int64_t)g * P + p], pre);
+            }
           }
-          wvalid = true;
         }
-        dense_chunk_dispatch(cnt, acc, w, newc, oldl, o0, DEPTH);
+        dense_chunk_dispatch<TPX>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
+        oend = o0;
       } else {
-        sparse_chunk_dispatch(cnt, acc, w, newc, oldl, DEPTH);
+        sparse_chunk_dispatch<TPX>(cnt, acc, w, newc, oldl, DEPTH);
       }
     } else {
+    if (dense && open) {  // the whole chunks before this one: fold them while their last window rows are resident
+      if (p < P) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
+      open = false;
+    }
 #pragma unroll 1
     for (int blk = 0; blk < kChunk / G; ++blk) {  // warm-up and the batch's last, partial chunk: checked per block
       const int jb = c * kChunk + blk * G;  // batch-relative index of the block's first step
       const int ns = min(G, b - jb);        // steps of this block inside the batch
       if (ns <= 0) break;
-      const f2x* nb = newc + (size_t)blk * G * kRowF2;
+      const f2x* nb = newc + (size_t)blk * G * TPX;
       if (doI) {
 #pragma unroll
         for (int u = 0; u < G; ++u) {
           if (u < ns) {
-            const f2x zn = nb[(size_t)u * kRowF2];
+            const f2x zn = nb[(size_t)u * TPX];
             i2 = fma2(zn, zn, i2);
             i1 = add2(i1, zn);
           }
         }
       }
       if (jb + ns <= j_any) {
-        wvalid = false;  // no pair of this task yet
+        // no pair of this task yet
       } else if (dense) {
-        // ---- masked block: pair (step u, lag tau0 + g) exists iff u - g >= vbase, and u < ns.  All G lags of
-        // the window are updated; the surplus ones of a short task are discarded at the fold. ----
+        // ---- masked block of a run of lags: every existing pair directly, pair (step u, lag tau0 + g) exists
+        // iff u - g >= vbase and u < ns; straight into the fp64 totals (rare: the warm-up of a stack and the
+        // ragged tail of a batch).  Rows o0 - (G-1) .. o0 + G-1 are contiguous thanks to the duplicated slot. ----
         const int vbase = (int)max((int64_t)-64, (int64_t)tk.tau0 - t0 - jb);
-        if (!wvalid) {  // (re)load the window; rows of frames before the first one are masked below
+        int rb = o0 - (G - 1);
+        if (rb < 0) rb += DEPTH;
+        const f2x* ob = oldl + (size_t)rb * TPX;
 #pragma unroll
-          for (int q = 1; q < G; ++q) {
-            int r = o0 - q;
-            if (r < 0) r += DEPTH;
-            w[G - q] = oldl[(size_t)r * kRowF2];
+        for (int g = 0; g < G; ++g) {
+          if (g < cnt) {
+            f2x a = 0ull;
+#pragma unroll 1
+            for (int u = max(0, vbase + g); u < ns; ++u) upd2(a, nb[(size_t)u * TPX], ob[(size_t)(G - 1 + u - g) * TPX]);
+            if (p < P) atomicAdd(&tot[(int64_t)g * P + p], (double)f2x_sum(a));
           }
         }
-        wvalid = ns == G;
-        const f2x* ob = oldl + (size_t)o0 * kRowF2;
-#pragma unroll
-        for (int u = 0; u < G; ++u) {
-          if (u < ns) {
-            const f2x zn = nb[(size_t)u * kRowF2];
-            w[u] = ob[(size_t)u * kRowF2];
-#pragma unroll
-            for (int g = 0; g < G; ++g)
-              if (u - g >= vbase) upd2(acc[g], zn, w[(u - g + G) % G]);
-          }
-        }
+        wvalid = false;
       } else {
         // ---- masked block of a lag list: pair (step u, lag i) exists iff u >= u0_i, and u < ns ----
-        sparse_masked_dispatch(cnt, ns, acc, w, nb, oldl, &s_lags[warp * G], t0 + jb);
+        sparse_masked_dispatch<TPX>(cnt, ns, acc, w, nb, oldl, &s_lags[warp * G], t0 + jb);
       }
       if (dense) {
         o0 += G;
@@ -618,33 +627,45 @@ __global__ void __launch_bounds__((kMaxTasks + 1) * 32, kLagMinBlocks)
   // (RED.ADD.F64 in L2, nothing returns to the SM) per (lag, pixel).  Every address has one writer per
   // launch, which folds in program order, and launches are stream ordered: the order of the additions
   // is fixed and the result deterministic.
+  if (p < P) {
+    if (dense) {
+      if (open) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
+    } else {
 #pragma unroll
-  for (int g = 0; g < G; ++g) {
-    if (g < cnt) atomicAdd(&totals[(int64_t)(tk.l0 + g) * P + p], (double)f2x_sum(acc[g]));
-    acc[g] = 0ull;
+      for (int g = 0; g < G; ++g)
+        if (g < cnt) atomicAdd(&tot[(int64_t)g * P + p], (double)f2x_sum(acc[g]));
+    }
+    if (doI) {
+      atomicAdd(&I2[p], (double)f2x_sum(i2));
+      atomicAdd(&I1[p].x, (double)f2x_lo(i1));
+      atomicAdd(&I1[p].y, (double)f2x_hi(i1));
+    }
   }
-  if (doI) {
-    atomicAdd(&I2[p], (double)f2x_sum(i2));
-    atomicAdd(&I1[p].x, (double)__uint_as_float((unsigned)(i1 & 0xffffffffull)));
-    atomicAdd(&I1[p].y, (double)__uint_as_float((unsigned)(i1 >> 32)));
-    i2 = 0ull, i1 = 0ull;
-  }
+#pragma unroll
+  for (int g = 0; g < G; ++g) acc[g] = 0ull;
+  i2 = 0ull, i1 = 0ull;
   }
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// host: the lag plan.  Lags are cut into tasks (one consumer warp each) and tasks into groups (one CTA
-// per group and pixel tile).  A run of >= kDenseMin consecutive lags becomes dense tasks of equal size
-// <= kG; the other lags become sparse tasks.  A group takes consecutive lags while its consumer warps
-// (<= kMaxTasks) and its shared-memory window (lag span) fit; the sparse lags of a group are then spread
-// over the warps the dense tasks leave free, and tasks are placed on warps so that the four SM
-// sub-partitions (warp id mod 4) carry equal FP32 work (longest-processing-time first).
+// host: the lag plan.  Lags are cut into tasks (one consumer warp each per 32-pixel sub-tile) and tasks into groups
+// (one CTA per group and pixel tile).  A run of >= kDenseMin consecutive lags becomes dense tasks of equal size
+// <= kG; the other lags become sparse tasks.  A group takes consecutive lags while its task slots (<= kTaskSlots)
+// and its shared-memory window (lag span) fit; the sparse lags of a group are then spread over the slots the dense
+// tasks leave free, and tasks are placed on slots so that the four SM sub-partitions (warp id mod 4) carry equal
+// FP32 work (longest-processing-time first).
 // ------------------------------------------------------------------------------------------------
 namespace {
 struct Atom {
   int l0, cnt, kind;  // dense task, or one sparse lag (cnt = 1)
 };
+
+// issue slots per time step: a run costs 2 loads, the increment, the direct update (2) and one FMA per further lag;
+// a lag list one load and two packed operations per lag plus the load of the new frame
+double task_cost(const LagTask& t) {
+  return ((t.kind & 1) == 0 ? 4.0 + t.cnt : 3.0 * t.cnt + 1.0) + ((t.kind & 2) ? 3.0 : 0.0);
+}
 
 void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1, bool with_I,
                  std::vector<LagTask>& tasks, std::vector<LagGroup>& groups) {
@@ -654,13 +675,12 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   g.tau_max = L[atoms[a1 - 1].l0 + atoms[a1 - 1].cnt - 1];
   int n_dense = 0, n_sparse = 0;
   for (size_t a = a0; a < a1; ++a) (atoms[a].kind == 0 ? n_dense : n_sparse) += 1;
-  // sparse task size: small enough to use the free warps (up to 8 warps in all), large enough to fit them
+  // sparse task size: small enough to use the free slots, large enough to fit them
   int s = 1;
   if (n_sparse > 0) {
-    const int free_w = kMaxTasks - n_dense;
-    const int want_w = std::max(1, std::min(free_w, 8 - std::min(n_dense, 7)));
-    s = std::min(kSparseMax, std::max(1, (n_sparse + want_w - 1) / want_w));
-    for (;; ++s) {  // stretches are cut separately: make sure the warps suffice
+    const int free_w = kTaskSlots - n_dense;
+    s = std::min(kSparseMax, std::max(1, (n_sparse + free_w - 1) / std::max(1, free_w)));
+    for (;; ++s) {  // stretches are cut separately: make sure the slots suffice
       int need = 0;
       size_t a = a0;
       while (a < a1) {
@@ -693,45 +713,44 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   }
   g.ntasks = (int)tasks.size() - g.task0;
   g.flags = with_I ? 1 : 0;
-  auto cost = [&](int k) {
-    const LagTask& t = tasks[g.task0 + k];
-    return ((t.kind & 1) == 0 ? 4 * t.cnt + 2 : 5 * t.cnt + 1) + ((t.kind & 2) ? 5 : 0);
-  };
-  if (with_I) {  // this group also accumulates the I sums (kind bit 1): on a warp of its own if one is free,
+  if (with_I) {  // this group also accumulates the I sums (kind bit 1): on a slot of its own if one is free,
                  // else on its lightest task
-    if (g.ntasks < kMaxTasks) {
+    if (g.ntasks < kTaskSlots) {
       tasks.push_back(LagTask{0, 0, 0, 1 | 2});
       g.ntasks += 1;
     } else {
       int best = 0;
       for (int k = 1; k < g.ntasks; ++k)
-        if (cost(k) < cost(best)) best = k;
+        if (task_cost(tasks[g.task0 + k]) < task_cost(tasks[g.task0 + best])) best = k;
       tasks[g.task0 + best].kind |= 2;
     }
   }
-  // placement: heaviest task first onto the least loaded sub-partition that still has a free warp
+  // placement: heaviest task first onto the least loaded sub-partition that still has a free slot
   for (int w = 0; w < 16; ++w) g.warp_task[w] = -1;
   std::vector<int> order(g.ntasks);
   for (int k = 0; k < g.ntasks; ++k) order[k] = k;
-  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost(x) > cost(y); });
-  int load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0};
+  std::stable_sort(order.begin(), order.end(),
+                   [&](int x, int y) { return task_cost(tasks[g.task0 + x]) > task_cost(tasks[g.task0 + y]); });
+  double load[4] = {0, 0, 0, 0};
+  int used[4] = {0, 0, 0, 0};
   for (int k : order) {
     int best = -1;
     for (int q = 0; q < 4; ++q)
-      if (used[q] < kMaxTasks / 4 && (best < 0 || load[q] < load[best])) best = q;
+      if (used[q] < kTaskSlots / 4 && (best < 0 || load[q] < load[best])) best = q;
     g.warp_task[used[best] * 4 + best] = (signed char)k;
     used[best] += 1;
-    load[best] += cost(k);
+    load[best] += task_cost(tasks[g.task0 + k]);
   }
+  g.cta0 = g.nctas = 0;
   groups.push_back(g);
 }
 }  // namespace
 
-bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
+bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
   const std::vector<int32_t>& L = c.lags;
-  // shared memory one CTA may use when kLagMinBlocks CTAs share an SM (1 KB per CTA is reserved)
-  size_t budget = (size_t)std::max(0, smem_sm / kLagMinBlocks - 1024 - 512);  // 1 KB reserved + 512 B static per CTA
-  budget = std::min(budget, (size_t)c.max_smem_optin);
+  // shared memory a CTA may use: the opt-in maximum (one CTA per SM) bounds a group's window; two CTAs of 32-pixel
+  // tiles share an SM when the plan's footprint allows it (1 KB per CTA is reserved, 1 KB static)
+  const size_t budget = (size_t)std::max(0, std::min(smem_sm - 2048, c.max_smem_optin - 1024));
   // atoms
   std::vector<Atom> atoms;
   for (int i = 0; i < c.n_lags;) {
@@ -743,7 +762,11 @@ bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
       int l = i;
       for (int k = 0; k < nt; ++k) {
         const int cnt = len / nt + (k < len % nt ? 1 : 0);
-        atoms.push_back(Atom{l, cnt, 0});
+        if (cnt >= kDenseMin) {
+          atoms.push_back(Atom{l, cnt, 0});
+        } else {
+          for (int q = 0; q < cnt; ++q) atoms.push_back(Atom{l + q, 1, 1});
+        }
         l += cnt;
       }
     } else {
@@ -751,12 +774,16 @@ bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
     }
     i = j + 1;
   }
-  // greedy groups
+  // greedy groups: a group is streamed as a single window when that costs no more shared memory than two streams
+  auto single_of = [&](int tmin, int tmax) {
+    return lag_smem_bytes(0, tmax, true, kMinStages, 32) <= lag_smem_bytes(tmin, tmax, false, kMinStages, 32);
+  };
   c.tasks.clear();
   c.groups.clear();
   auto fits = [&](size_t a0, size_t a1) {  // atoms [a0, a1) as one group
     const int tmin = L[atoms[a0].l0], tmax = L[atoms[a1 - 1].l0 + atoms[a1 - 1].cnt - 1];
-    if (lag_smem_bytes(tmin, tmax, kMinStages + 1) > budget && a1 - a0 > 1) return false;
+    const bool sg = single_of(tmin, tmax);
+    if (lag_smem_bytes(sg ? 0 : tmin, tmax, sg, kMinStages, 32) > budget && a1 - a0 > 1) return false;
     int need = 0;
     size_t a = a0;
     while (a < a1) {
@@ -766,7 +793,7 @@ bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
       need += ((int)(e - a) + kSparseMax - 1) / kSparseMax;
       a = e;
     }
-    return need <= kMaxTasks;
+    return need <= kTaskSlots;
   };
   std::vector<std::pair<size_t, size_t>> cuts;
   size_t a0 = 0;
@@ -783,34 +810,56 @@ bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
     for (size_t a = r.first; a < r.second; ++a) n += atoms[a].cnt;
     return n;
   };
-  for (size_t k = 1; k < cuts.size(); ++k)
+  c.max_group_lags = 0;
+  for (size_t k = 0; k < cuts.size(); ++k) {
     if (nl(cuts[k]) < nl(cuts[gI])) gI = k;
+    c.max_group_lags = std::max(c.max_group_lags, nl(cuts[k]));
+  }
   for (size_t k = 0; k < cuts.size(); ++k) close_group(L, atoms, cuts[k].first, cuts[k].second, k == gI, c.tasks, c.groups);
-  // pipeline depth: as deep as the widest group's window leaves room for
-  int stages = kMaxStages;
-  for (const LagGroup& g : c.groups)
-    while (stages > kMinStages && lag_smem_bytes(g.tau_min, g.tau_max, stages) > budget) --stages;
-  size_t smem = 0;
-  for (const LagGroup& g : c.groups) smem = std::max(smem, lag_smem_bytes(g.tau_min, g.tau_max, stages));
+  for (LagGroup& g : c.groups)
+    if (single_of(g.tau_min, g.tau_max)) g.flags |= 2;
+  // tile width and pipeline depth.  64-pixel tiles (16 consumer warps, one CTA per SM, 512-byte rows) when every
+  // group's window then still leaves kMinStages + 1 stages; else 32-pixel tiles, two CTAs per SM if they fit.
+  auto smem_for = [&](int stages, int tpx) {
+    size_t m = 0;
+    for (const LagGroup& g : c.groups) m = std::max(m, lag_smem_bytes(lag_tau_lo(g), g.tau_max, (g.flags & 2) != 0, stages, tpx));
+    return m;
+  };
+  int tpx = 32, per_sm = 1, stages = kMinStages;
+  if (P % 64 == 0 && smem_for(kMinStages + 1, 64) <= budget) {
+    tpx = 64;
+    stages = kMinStages + 1;
+    while (stages < kMaxStages && smem_for(stages + 1, 64) <= budget) ++stages;
+  } else {
+    const size_t half = (size_t)std::max(0, smem_sm / 2 - 2048);
+    if (smem_for(kMinStages + 1, 32) <= half) {
+      per_sm = 2;
+      stages = kMinStages + 1;
+      while (stages < kMaxStages && smem_for(stages + 1, 32) <= half) ++stages;
+    } else {
+      while (stages < kMaxStages && smem_for(stages + 1, 32) <= budget) ++stages;
+    }
+  }
+  const size_t smem = smem_for(stages, tpx);
   if (smem > (size_t)c.max_smem_optin) return false;  // a single task's own lag span does not fit
   c.lag_stages = stages;
   c.lag_smem = smem;
-  // persistent CTAs: the cta_slots resident CTAs of the device are shared out in proportion to the groups' work
-  // per pixel tile (FP32 work of the tasks + a constant for streaming the window), at least one CTA each
+  c.lag_tpx = tpx;
+  c.lag_ctas_per_sm = per_sm;
+  // persistent CTAs: the resident CTAs of the device are shared out in proportion to the groups' work per pixel
+  // tile (issue slots of the tasks + a constant for streaming the window), at least one CTA each
   {
+    const int ntiles = (int)std::min<int64_t>((P + tpx - 1) / tpx, 1 << 30);
     const int ng = (int)c.groups.size();
     std::vector<double> wgt(ng);
     double wsum = 0.0;
     for (int g = 0; g < ng; ++g) {
-      double wg = 40.0;
-      for (int k = 0; k < c.groups[g].ntasks; ++k) {
-        const LagTask& t = c.tasks[c.groups[g].task0 + k];
-        wg += ((t.kind & 1) == 0 ? 4.0 * t.cnt + 2.0 : 5.0 * t.cnt + 1.0) + ((t.kind & 2) ? 5.0 : 0.0);
-      }
+      double wg = 20.0;
+      for (int k = 0; k < c.groups[g].ntasks; ++k) wg += task_cost(c.tasks[c.groups[g].task0 + k]);
       wgt[g] = wg;
       wsum += wg;
     }
-    const int slots = std::max(cta_slots, ng);
+    const int slots = std::max(per_sm * std::max(1, n_sm), ng);
     int used = 0;
     for (int g = 0; g < ng; ++g) {
       int n = (int)(slots * wgt[g] / wsum);
@@ -840,69 +889,101 @@ bool lag_plan(Ctx& c, int smem_sm, int cta_slots, int ntiles) {
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-int launch_accum_I(Ctx& c, int64_t t0, int b) {
-  ProfScope ps(c, kKAccI);
-  k_accum_I<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.ring, c.R, c.P, t0, b, c.I2, c.I1);
-  return 1;
+namespace {
+typedef void (*LagKernel)(const CUtensorMap, const float2*, int, int64_t, int64_t, int, int, int, int, int, const LagTask*,
+                          const LagGroup*, const int32_t*, double*, double*, double2*, int, int*);
+LagKernel lag_kernel(int tpx, bool pers, bool skip) {
+  if (tpx == 64)
+    return pers ? (skip ? k_lag_tiled<16, true, true> : k_lag_tiled<16, true, false>)
+                : (skip ? k_lag_tiled<16, false, true> : k_lag_tiled<16, false, false>);
+  return pers ? (skip ? k_lag_tiled<8, true, true> : k_lag_tiled<8, true, false>)
+              : (skip ? k_lag_tiled<8, false, true> : k_lag_tiled<8, false, false>);
 }
+}  // namespace
 
-int launch_lag_simple(Ctx& c, int64_t t0, int b) {
-  dim3 grid((unsigned)((c.P + 127) / 128), (unsigned)((c.n_lags + 7) / 8));
-  ProfScope ps(c, kKLag);
-  k_lag_simple<<<grid, 128, 0, c.stream>>>(c.ring, c.R, c.P, t0, b, c.d_lags, c.n_lags, c.totals);
-  return 1;
-}
-
-// 2-D tensor map over the ring: dim0 = 2*P floats (32 pixels = 64 floats per box), dim1 = R ring slots
-bool lag_make_tensor_map(Ctx& c) {
+// once at create, after the ring is allocated: the 2-D tensor map over the ring (dim0 = 2*P floats, box of one pixel
+// tile; dim1 = R ring slots, box of kChunk) and the dynamic shared memory of the four launch variants
+bool lag_configure(Ctx& c) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-      qres != cudaDriverEntryPointSuccess)
+  if (!NFS_CUDA(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres))) return false;
+  if (!fn || qres != cudaDriverEntryPointSuccess) {
+    c.status = NFS_ERR_CUDA;
+    c.cuda_err = "cuTensorMapEncodeTiled not available";
     return false;
+  }
   const cuuint64_t gdim[2] = {(cuuint64_t)(2 * c.P), (cuuint64_t)c.R};
   const cuuint64_t gstride[1] = {(cuuint64_t)c.P * sizeof(float2)};
-  const cuuint32_t box[2] = {(cuuint32_t)(2 * kTilePx), (cuuint32_t)kChunk};
+  const cuuint32_t box[2] = {(cuuint32_t)(2 * c.lag_tpx), (cuuint32_t)kChunk};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult r = reinterpret_cast<EncodeFn>(fn)(&c.ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c.ring, gdim, gstride, box,
                                                     estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
+  if (r != CUDA_SUCCESS) {
+    c.status = NFS_ERR_CUDA;
+    c.cuda_err = "cuTensorMapEncodeTiled failed";
+    return false;
+  }
+  for (int v = 0; v < 4; ++v)
+    if (!NFS_CUDA(c, cudaFuncSetAttribute(lag_kernel(c.lag_tpx, (v & 1) != 0, (v & 2) != 0),
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem)))
+      return false;
+  return true;
 }
 
 int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
-  cudaFuncSetAttribute(k_lag_tiled<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
-  cudaFuncSetAttribute(k_lag_tiled<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
-  cudaFuncSetAttribute(k_lag_tiled<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
-  cudaFuncSetAttribute(k_lag_tiled<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem);
   const int ngroups = (int)c.groups.size();
-  const int ntiles = (int)(c.P / kTilePx);
-  // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold: ~8 us) outweighs its work: batches
-  // of one or two chunks — provided the window prologue of a tile (LEAD steps) hides inside the pipeline depth and
-  // the device is shared by at most two groups.  Measured on the B200 (profiles/r01_summary.md): lags 1..100,
-  // batch 26: 35.8 -> 26.2 ms per 2000 frames; lags 1..208 (two groups): 66.5 -> 51.4 ms.  Elsewhere one CTA per
-  // (tile, group) is as fast or faster: with a long window (isolated far lags) every tile costs LEAD barrier rounds
-  // before its first chunk (lags 1..60 + 9 isolated lags <= 500, batch 26: 67 -> 147 ms); with many groups the
-  // CTAs of a pixel tile launched side by side share the NEW frames in L2 and open the same DRAM pages (config 4:
-  // 663 -> 852 ms); at long batches the fixed cost is amortised anyway (config 2: 13.95 -> 14.18 ms).
+  const int tpx = c.lag_tpx;
+  const int ntiles = (int)((c.P + tpx - 1) / tpx);
+  const int nthreads = (tpx / 4 + 1) * 32;
+  int n = 0;
+  if (c.bin_only) {
+    // PAPER.md:L41 ("store the entire 2D power spectra, which might be unnecessary"): one lag group per launch into
+    // a per-pixel scratch of that group's lags, reduced into the |q|-binned totals in a fixed order right after
+    int lbase = 0;
+    for (int g = 0; g < ngroups; ++g) {
+      const LagGroup& grp = c.groups[g];
+      int nl = 0;
+      for (int k = 0; k < grp.ntasks; ++k) nl += c.tasks[grp.task0 + k].cnt;
+      const bool runs = (grp.flags & 1) || (int64_t)grp.tau_min <= t0 + b - 1;
+      if (runs) {
+        const bool skip = !(grp.flags & 1) && (int64_t)grp.tau_min - t0 >= kChunk;
+        {
+          ProfScope ps(c, kKLag);
+          if (!NFS_CUDA(c, cudaMemsetAsync(c.totals, 0, sizeof(double) * (size_t)nl * c.P, c.stream))) return n;
+          lag_kernel(tpx, false, skip)<<<(unsigned)ntiles, nthreads, c.lag_smem, c.stream>>>(
+              c.ring_map, c.ring, c.R, c.P, t0, b, g, 1, lbase, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2,
+              c.I1, ntiles, c.d_claim);
+          n += 1;
+        }
+        n += launch_bin_accumulate(c, lbase, nl);
+      }
+      lbase += nl;
+    }
+    return n;
+  }
+  // Persistent CTAs pay off where a CTA's fixed cost (launch, window fill, fold) outweighs its work: batches of one
+  // or two chunks — provided the window prologue of a tile (LEAD steps) hides inside the pipeline depth and the
+  // device is shared by at most two groups.  Elsewhere one CTA per (tile, group) is as fast or faster: with a long
+  // window every tile costs LEAD barrier rounds before its first chunk; with many groups the CTAs of a pixel tile
+  // launched side by side share the batch's frames in L2 and open the same DRAM pages; at long batches the fixed
+  // cost is amortised anyway (measurements: profiles/).
   int max_lead = 0;
-  for (const LagGroup& g : c.groups) max_lead = std::max(max_lead, lag_lead(g.tau_min, g.tau_max));
-  const bool persistent = c.lag_persistent >= 0 ? c.lag_persistent != 0
-                                                : (b <= 2 * kChunk && ngroups <= 2 && max_lead <= c.lag_stages);
+  for (const LagGroup& g : c.groups) max_lead = std::max(max_lead, lag_lead(lag_tau_lo(g), g.tau_max));
+  const bool persistent = c.lag_shape ? c.lag_shape == 2 : (b <= 2 * kChunk && ngroups <= 2 && max_lead <= c.lag_stages);
   const unsigned grid = persistent ? (unsigned)c.lag_grid : (unsigned)ntiles * (unsigned)ngroups;
   ProfScope ps(c, kKLag);
   // some group (other than the one that accumulates the I sums) has whole chunks without a pair in this batch
   bool skip = false;
-  for (const LagGroup& g : c.groups) skip |= g.flags == 0 && (int64_t)g.tau_min - t0 >= kChunk && (int64_t)g.tau_min <= t0 + b - 1;
-  auto kern = persistent ? (skip ? k_lag_tiled<true, true> : k_lag_tiled<true, false>)
-                         : (skip ? k_lag_tiled<false, true> : k_lag_tiled<false, false>);
-  if (persistent) cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream);
-  kern<<<grid, (kMaxTasks + 1) * 32, c.lag_smem, c.stream>>>(c.ring_map, c.ring, c.R, c.P, t0, b, ngroups, c.lag_stages,
-                                                              c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1, ntiles,
-                                                              c.d_claim);
+  for (const LagGroup& g : c.groups)
+    skip |= !(g.flags & 1) && (int64_t)g.tau_min - t0 >= kChunk && (int64_t)g.tau_min <= t0 + b - 1;
+  if (persistent && !NFS_CUDA(c, cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream))) return 0;
+  lag_kernel(tpx, persistent, skip)<<<grid, nthreads, c.lag_smem, c.stream>>>(
+      c.ring_map, c.ring, c.R, c.P, t0, b, 0, ngroups, 0, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1,
+      ntiles, c.d_claim);
   return 1;
 }
 

@@ -11,7 +11,8 @@ values fixed by BASELINE.json `configs`:
             per Fourier mode: a_0 = S xi, a_{t+1} = a_t e^{-Gamma} + S sqrt(1 - e^{-2 Gamma}) xi,
             S(q) = 1/(1 + (q/q0)^4), S(0) = 0, Gamma(q) = gamma0 (q/q0)^2, q in cycles/px.
 
-This module serves both the CUDA path's tests/bench and the oracle's tests; it imports neither.
+This module (harness code at the repo root, outside the product package) serves both the CUDA path's
+tests/bench and the oracle's tests; it imports neither.
 It is harness code: torch (incl. torch.fft) is used so configs 2-4 can be generated on the GPU.
 Oracle and library always consume the *same uint16 bytes* within a run.
 """

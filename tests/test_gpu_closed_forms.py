@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_1209_3362_b200 import synth
+import synth
 
 pytestmark = pytest.mark.gpu
 
@@ -53,7 +53,9 @@ def test_gain_invariance(binding):
 
 
 def test_telegraph_stack(binding):
-    """P5: frames alternate between P and Q: even lags give exactly 0, odd lags |F_P - F_Q|^2 for every tau."""
+    """P5: frames alternate between P and Q: even lags give 0, odd lags |F_P - F_Q|^2 for every tau.  Lags that open a
+    run of consecutive lags (or stand alone) are accumulated directly and give exact zeros; the further lags of a run
+    come from the neighbouring-lag recurrence and give zero up to fp32 rounding of the odd-lag value."""
     rng = np.random.default_rng(7)
     Pimg = rng.integers(500, 3000, size=(64, 64)).astype(np.uint16)
     Qimg = rng.integers(500, 3000, size=(64, 64)).astype(np.uint16)
@@ -65,7 +67,9 @@ def test_telegraph_stack(binding):
     ref = np.abs(np.fft.rfft2(ip - iq, norm="ortho")) ** 2
     for l, tau in enumerate(lags):
         if tau % 2 == 0:
-            assert np.all(D2d[l] == 0.0)
+            assert np.abs(D2d[l]).max() <= 2e-6 * ref.max()
+            if tau == 12:
+                assert np.all(D2d[l] == 0.0)
         else:
             m = ref > 1e-6 * ref.max()
             assert (np.abs(D2d[l] - ref)[m] / ref[m]).max() < 1e-4

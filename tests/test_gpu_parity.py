@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_1209_3362_b200 import synth
+import synth
 
 pytestmark = pytest.mark.gpu
 
@@ -25,10 +25,10 @@ def binding():
     return b
 
 
-def gpu_run(binding, stack, lags, n_b, batch=0, variant=0, split=None, want_2d=True):
+def gpu_run(binding, stack, lags, n_b, batch=0, shape=0, split=None, want_2d=True):
     N, H, W = stack.shape
     nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch)
-    nfs.set_lag_kernel(variant)
+    nfs.set_launch_shape(shape)
     if split:
         i = 0
         while i < N:
@@ -91,11 +91,11 @@ def cfg0():
     return cfg, st, ref
 
 
-@pytest.mark.parametrize("variant,batch,split", [(0, 0, None), (1, 0, None), (0, 5, None), (0, 0, 3), (0, 7, 5),
-                                                  (1, 0, 1), (0, 0, 1), (0, 32, None), (0, 1, None)])
-def test_config0_full(binding, cfg0, variant, batch, split):
+@pytest.mark.parametrize("shape,batch,split", [(0, 0, None), (1, 0, None), (0, 5, None), (0, 0, 3), (0, 7, 5),
+                                                (2, 0, 1), (0, 0, 1), (0, 32, None), (0, 1, None), (2, 0, None)])
+def test_config0_full(binding, cfg0, shape, batch, split):
     cfg, st, ref = cfg0
-    g = gpu_run(binding, st, cfg.lags, cfg.n_qbins, batch=batch, variant=variant, split=split)
+    g = gpu_run(binding, st, cfg.lags, cfg.n_qbins, batch=batch, shape=shape, split=split)
     assert g["N"] == cfg.N and g["launches"] > 0
     assert g["counts"][0] == 0, "config 0 has an empty first bin (reading R7)"
     check_against_oracle(g, ref, cfg.W)
@@ -137,12 +137,12 @@ def test_scaled_configs(binding, oracle, idx, W, N, lags, n_b, batch, per_pixel)
     st = synth.make_stack(cfg, "cuda")
     ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=per_pixel)
     first = None
-    for variant in ((0, 1, 2, 3) if W <= 512 else (0, 2, 3)):
-        g = gpu_run(binding, st, lags, n_b, batch=batch, variant=variant, want_2d=per_pixel)
+    for shape in (0, 1, 2):
+        g = gpu_run(binding, st, lags, n_b, batch=batch, shape=shape, want_2d=per_pixel)
         check_against_oracle(g, ref, W, per_pixel=per_pixel)
-        if variant != 1:  # the launch shape of the tiled kernel (one tile per CTA / persistent CTAs) changes no bit
-            first = first or g
-            assert np.array_equal(g["D"], first["D"]) and np.array_equal(g["I_q"], first["I_q"])
+        # the launch shape of the lag kernel (one tile per CTA / persistent CTAs) changes no bit
+        first = first or g
+        assert np.array_equal(g["D"], first["D"]) and np.array_equal(g["I_q"], first["I_q"])
 
 
 # --------------------------------------------------------------------------------------------------------------
@@ -163,8 +163,8 @@ def test_random_lag_lists_batches_and_splits(binding, oracle, seed):
     cfg.seed = 500 + seed
     st = synth.make_stack(cfg, "cuda")
     ref = oracle.structure_function(st.cpu().numpy(), lags, n_b, want_2d=True)
-    for variant in (2, 3):
-        g = gpu_run(binding, st, lags, n_b, batch=batch, split=split or None, variant=variant)
+    for shape in (1, 2):
+        g = gpu_run(binding, st, lags, n_b, batch=batch, split=split or None, shape=shape)
         check_against_oracle(g, ref, W)
 
 
@@ -190,7 +190,7 @@ def test_lags_beyond_N_and_single_frame(binding, oracle):
     g = gpu_run(binding, st, lags, 16)
     assert g["n_pairs"].tolist() == [5, 4, 1, 0, 0, 0]
     check_against_oracle(g, ref, cfg.W)
-    assert np.all(g["D2d"][3:] == 0.0)
+    assert np.all(g["D2d"][3:] == 0.0), "lags >= N: rows of exact zeros"
     # N = 1: no pairs at all, I(q) still defined
     ref1 = oracle.structure_function(st[:1].cpu().numpy(), [1, 2], 16, want_2d=True)
     g1 = gpu_run(binding, st[:1].contiguous(), [1, 2], 16)

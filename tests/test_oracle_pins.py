@@ -384,3 +384,46 @@ def test_p14_white_noise_variance_is_half_the_D_plateau(oracle):
     for b in range(n_b):
         if v.counts[b]:
             assert abs(v.V_q[b] / var - 1.0) < 6.0 / math.sqrt(v.counts[b] * N / 2.0)
+
+
+# ---- P11: the half-plane variant equals the full-plane definition --------------------------
+def _synth_np(idx, **kw):
+    import synth
+
+    cfg = synth.config(idx, **kw)
+    return cfg, synth.make_stack(cfg, "cpu").numpy()
+
+
+@pytest.mark.parametrize("idx,kw", [(0, {}), (1, dict(W=128, N=60, lags=[1, 2, 3, 5, 8, 13, 21, 40], n_qbins=32)),
+                                    (3, dict(W=64, N=24, lags=[1, 2, 7, 23, 24, 30], n_qbins=16))])
+def test_p11_half_plane_equals_full_plane(oracle, idx, kw):
+    """BASELINE.json configs[0] in full and scaled configs 1 and 3: the half-plane evaluation (Hermitian weights
+    2 / 1 in the bin means) against the full-plane definition — counts identical, values to 1e-12."""
+    cfg, fr = _synth_np(idx, **kw)
+    full = oracle.structure_function(fr, cfg.lags, cfg.n_qbins, want_2d=True)
+    half = oracle.structure_function_half(fr, cfg.lags, cfg.n_qbins, want_2d=True)
+    assert np.array_equal(half.counts, full.counts) and np.array_equal(half.n_pairs, full.n_pairs)
+    np.testing.assert_allclose(half.D, full.D, rtol=1e-12, atol=1e-300)
+    np.testing.assert_allclose(half.I_q, full.I_q, rtol=1e-12, atol=1e-300)
+    n = cfg.W // 2
+    np.testing.assert_allclose(half.D2d, full.D2d[:, :, :n + 1], rtol=1e-12, atol=1e-22)
+    np.testing.assert_allclose(half.I2d, full.I2d[:, :n + 1], rtol=1e-12, atol=1e-22)
+    # rows with tau >= N are zero rows in both
+    assert np.all(half.D[half.n_pairs == 0] == 0.0)
+
+
+def test_p11_half_plane_counts_against_bruteforce_python_ints(oracle):
+    """The weights 2 / 1 reproduce the full-plane counts of the pure-Python bin rule (oracle/brute_force.py), also on
+    a non-square frame, where a transposed W/H in the weights or in the Nyquist column would show."""
+    for (H, W, n_b) in ((8, 16, 5), (16, 8, 7), (32, 32, 16)):
+        fr = _rng(31).integers(100, 4000, (3, H, W)).astype(np.uint16)
+        half = oracle.structure_function_half(fr, [1, 2], n_b)
+        c = [0] * n_b
+        for ky in range(H):
+            for kx in range(W):
+                b = bf.qbin(kx, ky, W, H, n_b)
+                if b >= 0:
+                    c[b] += 1
+        assert half.counts.tolist() == c
+        full = oracle.structure_function(fr, [1, 2], n_b)
+        np.testing.assert_allclose(half.D, full.D, rtol=1e-12, atol=1e-300)

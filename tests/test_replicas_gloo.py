@@ -8,7 +8,8 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_1209_3362_b200 import replicas, synth
+import synth
+from paper_1209_3362_b200 import replicas
 
 
 def _free_port():
