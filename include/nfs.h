@@ -154,13 +154,15 @@ NFS_API int nfs_set_launch_shape(nfs_ctx* ctx, int shape);
  * nfs_create would build for `lags` (HOST, strictly increasing, >= 1) and frames of n_px Fourier pixels on a
  * device with n_sm SMs, `smem_per_sm` bytes of shared memory per SM and `smem_optin` bytes per CTA, and writes it
  * to out (HOST, cap int32):
- *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA, pixels per tile (32 | 64), CTAs per SM]
+ *   [n_groups, n_tasks, pipeline stages, dynamic shared memory bytes per CTA, pixels per tile (32 | 64), CTAs per SM,
+ *    task slots per group (8 | 16)]
  *   per group (23 values): first task, number of tasks, tau_min, tau_max, flags (bit 0: one task of the
  *     group accumulates the I sums; bit 1: single stream, the batch's frames are the head of the window),
  *     then for task slots 0..15 the task (relative) a consumer warp of that slot runs or -1, then the
  *     first persistent CTA of the group and their number
  *   per task (4 values): smallest lag, number of lags, index of its first lag in `lags`, kind (bit 0:
- *     0 = run of consecutive lags on the register-window path, 1 = lag list; bit 1: also accumulates I)
+ *     0 = run of consecutive lags on the register-window path, 1 = lag list; bit 1: also accumulates sum |F'|^2,
+ *     bit 2: also accumulates sum F' — the two sums of the static spectrum I)
  * Returns the number of int32 written (> 0), or NFS_ERR_INVALID_ARG (bad list, cap too small, a single
  * task's lag span exceeding shared memory). */
 NFS_API int nfs_plan_lags(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,

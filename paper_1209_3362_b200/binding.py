@@ -116,14 +116,14 @@ def nfs_plan_lags(lags, n_px=1024 * 513, smem_per_sm=233472, smem_optin=232448, 
     """Host-only lag plan (no CUDA call): dict(stages, smem, tile_px, ctas_per_sm, groups=[...], tasks=[...]); see
     include/nfs.h."""
     lags = np.ascontiguousarray(lags, dtype=np.int32)
-    cap = 6 + 27 * (len(lags) + 1)
+    cap = 7 + 27 * (len(lags) + 1)
     out = np.zeros(cap, dtype=np.int32)
     n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(n_px), int(smem_per_sm), int(smem_optin), int(n_sm),
                                      _dp(out, C.c_int32), cap)
     if n < 0:
         raise NFSError(n)
-    ng, nt, stages, smem, tile_px, per_sm = (int(v) for v in out[:6])
-    o = 6
+    ng, nt, stages, smem, tile_px, per_sm, slots = (int(v) for v in out[:7])
+    o = 7
     groups, tasks = [], []
     for _ in range(ng):
         g = out[o:o + 23]
@@ -134,7 +134,7 @@ def nfs_plan_lags(lags, n_px=1024 * 513, smem_per_sm=233472, smem_optin=232448, 
         t = out[o:o + 4]
         tasks.append(dict(tau0=int(t[0]), cnt=int(t[1]), l0=int(t[2]), kind=int(t[3])))
         o += 4
-    return dict(stages=stages, smem=smem, tile_px=tile_px, ctas_per_sm=per_sm, groups=groups, tasks=tasks)
+    return dict(stages=stages, smem=smem, tile_px=tile_px, ctas_per_sm=per_sm, slots=slots, groups=groups, tasks=tasks)
 
 
 def nfs_destroy(handle):

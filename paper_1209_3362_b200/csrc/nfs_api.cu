@@ -452,14 +452,14 @@ int nfs_set_launch_shape(nfs_ctx* h, int shape) {
 
 static int plan_impl(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,
                      int cap) {
-  if (!lags_ok(lags, n_lags) || !out || cap < 6 || n_px < 32 || n_sm < 1) return NFS_ERR_INVALID_ARG;
+  if (!lags_ok(lags, n_lags) || !out || cap < 7 || n_px < 32 || n_sm < 1) return NFS_ERR_INVALID_ARG;
   Ctx c;
   c.lags.assign(lags, lags + n_lags);
   c.n_lags = n_lags;
   c.Lmax = lags[n_lags - 1];
   c.max_smem_optin = smem_optin;
   if (!lag_plan(c, smem_per_sm, n_sm, (int64_t)n_px)) return NFS_ERR_INVALID_ARG;
-  const size_t need = 6 + c.groups.size() * 23 + c.tasks.size() * 4;
+  const size_t need = 7 + c.groups.size() * 23 + c.tasks.size() * 4;
   if (need > (size_t)cap) return NFS_ERR_INVALID_ARG;
   int32_t* o = out;
   *o++ = (int32_t)c.groups.size();
@@ -468,6 +468,7 @@ static int plan_impl(const int32_t* lags, int n_lags, int n_px, int smem_per_sm,
   *o++ = (int32_t)c.lag_smem;
   *o++ = c.lag_tpx;
   *o++ = c.lag_ctas_per_sm;
+  *o++ = c.lag_slots;
   for (const LagGroup& g : c.groups) {
     *o++ = g.task0, *o++ = g.ntasks, *o++ = g.tau_min, *o++ = g.tau_max, *o++ = g.flags;
     for (int w = 0; w < 16; ++w) *o++ = g.warp_task[w];

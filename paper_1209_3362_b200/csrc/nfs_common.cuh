@@ -21,7 +21,7 @@ namespace nfs {
 
 // ---- lag-accumulation plan (built on the host at create, nfs_lag.cu: lag_plan) ---------------------
 constexpr int kG = 13;            // lags per register-window task (window depth)
-constexpr int kTaskSlots = 8;     // lag tasks per group: one consumer warp each per 32-pixel sub-tile
+constexpr int kTaskSlots = 8;     // lag tasks per group (16 for long-window plans): one consumer warp each per 32-pixel sub-tile
 constexpr int kChunk = 2 * kG;    // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
 constexpr int kMinStages = 2;
 constexpr int kMaxStages = 8;     // pipeline depth is chosen at create from the shared memory left
@@ -33,7 +33,8 @@ struct LagTask {
   int tau0;  // smallest lag of the task
   int cnt;   // number of lags handled (<= kG)
   int l0;    // index of the first lag in the sorted lag list
-  int kind;  // bit 0: 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt); bit 1: also accumulates I2, I1
+  int kind;  // bit 0: 0 = dense run tau0..tau0+cnt-1, 1 = sparse list lags[l0..l0+cnt); bit 1: also accumulates I2
+             // (sum |F'|^2); bit 2: also accumulates I1 (sum F')
 };
 struct LagGroup {
   int task0, ntasks;
@@ -94,7 +95,8 @@ struct Ctx {
   LagGroup* d_groups = nullptr;
   int* d_claim = nullptr;        // [n_groups] next pixel tile of each group, zeroed before every persistent launch
   int lag_stages = kMinStages;   // pipeline stages of k_lag_tiled (chosen by lag_plan)
-  int lag_tpx = 32;              // Fourier pixels per CTA tile: 32 (8 consumer warps) or 64 (16 consumer warps)
+  int lag_tpx = 32;              // Fourier pixels per CTA tile: 32 or 64
+  int lag_slots = kTaskSlots;    // task slots per group: 8, or 16 (one 32-pixel CTA of 16 consumer warps per SM)
   int lag_ctas_per_sm = 1;       // resident CTAs per SM the plan counts on
   int lag_grid = 0;              // persistent CTAs of k_lag_tiled (sum of the groups' shares)
   int lag_shape = 0;             // 0: chosen per launch (launch_lag_tiled); 1 / 2: forced one-tile / persistent

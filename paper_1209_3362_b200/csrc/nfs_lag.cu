@@ -168,7 +168,7 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
 // chunk's kChunk OLD rows are contiguous (the ring's slot 0 is duplicated behind its last slot).
 template <int CNT, int TPX>
 __device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid, const f2x* newc,
-                                            const f2x* oldl, int& o0, int DEPTH) {
+                                            const f2x* oldl, int& o0, int DEPTH, int doI, f2x& i2, f2x& i1) {
   if (!wvalid) {  // (re)build the window: the increments of the CNT-2 OLD frames that precede the chunk's first one
     int r = o0 - (CNT - 1);
     if (r < 0) r += DEPTH;
@@ -196,35 +196,79 @@ __device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], f2x& z
     zprev = zo;
     upd2(acc[0], zn, zo);
 #pragma unroll
-    for (int g = 1; g < CNT; ++g) acc[g] = fma2(zn, w[(u - (g - 1) + 2 * kG) % kG], acc[g]);
+    for (int g = 1; g < CNT; ++g) acc[g] = fma2(zn, w[(u - (g - 1) + kChunk) % kG], acc[g]);
+    if (doI & 1) i2 = fma2(zn, zn, i2);  // the I sums ride on the frame already in registers (warp-uniform flags)
+    if (doI & 2) i1 = add2(i1, zn);
     zn = zn1;
     zo = zo1;
   }
   o0 += kChunk;
   if (o0 >= DEPTH) o0 -= DEPTH;
 }
-template <int TPX>
+// One block of <= kG steps of a register-window task in which every pair of every step exists, but the batch may
+// end inside it (ns <= kG steps): the same arithmetic as dense_chunk, one predicate per step.
+template <int CNT, int TPX>
+__device__ __forceinline__ void dense_block_partial(int ns, f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid,
+                                                    const f2x* nb, const f2x* oldl, int o0, int DEPTH) {
+  if (!wvalid) {
+    int r = o0 - (CNT - 1);
+    if (r < 0) r += DEPTH;
+    f2x zz = oldl[(size_t)r * TPX];
+#pragma unroll
+    for (int k = CNT - 2; k >= 1; --k) {
+      if (++r == DEPTH) r = 0;
+      const f2x zk = oldl[(size_t)r * TPX];
+      w[kG - k] = sub2(zz, zk);
+      zz = zk;
+    }
+    zprev = zz;
+  }
+  const f2x* ob = oldl + (size_t)o0 * TPX;
+#pragma unroll
+  for (int u = 0; u < kG; ++u) {
+    if (u < ns) {
+      const f2x zn = nb[(size_t)u * TPX], zo = ob[(size_t)u * TPX];
+      w[u] = sub2(zprev, zo);
+      zprev = zo;
+      upd2(acc[0], zn, zo);
+#pragma unroll
+      for (int g = 1; g < CNT; ++g) acc[g] = fma2(zn, w[(u - (g - 1) + kG) % kG], acc[g]);
+    }
+  }
+  wvalid = ns == kG;  // a shorter block ends the batch
+}
+
+// warp-uniform dispatch on the number of lags: the plan makes runs of kDenseMin..kG lags, mostly of kG and kG - 1
+template <int TPX, int CNT = kG>
 __device__ __forceinline__ void dense_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid,
-                                                     const f2x* newc, const f2x* oldl, int& o0, int DEPTH) {
-  switch (cnt) {  // warp-uniform; the plan makes dense tasks of kDenseMin..kG lags
-    case 2: dense_chunk<2, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 3: dense_chunk<3, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 4: dense_chunk<4, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 5: dense_chunk<5, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 6: dense_chunk<6, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 7: dense_chunk<7, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 8: dense_chunk<8, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 9: dense_chunk<9, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 10: dense_chunk<10, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 11: dense_chunk<11, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    case 12: dense_chunk<12, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
-    default: dense_chunk<kG, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH); break;
+                                                     const f2x* newc, const f2x* oldl, int& o0, int DEPTH, int doI, f2x& i2,
+                                                     f2x& i1) {
+  if constexpr (CNT <= kDenseMin) {
+    dense_chunk<kDenseMin, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+  } else {
+    if (cnt == CNT)
+      dense_chunk<CNT, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+    else
+      dense_chunk_dispatch<TPX, CNT - 1>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+  }
+}
+template <int TPX, int CNT = kG>
+__device__ __forceinline__ void dense_partial_dispatch(int cnt, int ns, f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev,
+                                                       bool& wvalid, const f2x* nb, const f2x* oldl, int o0, int DEPTH) {
+  if constexpr (CNT <= kDenseMin) {
+    dense_block_partial<kDenseMin, TPX>(ns, acc, w, zprev, wvalid, nb, oldl, o0, DEPTH);
+  } else {
+    if (cnt == CNT)
+      dense_block_partial<CNT, TPX>(ns, acc, w, zprev, wvalid, nb, oldl, o0, DEPTH);
+    else
+      dense_partial_dispatch<TPX, CNT - 1>(cnt, ns, acc, w, zprev, wvalid, nb, oldl, o0, DEPTH);
   }
 }
 // ---- lag-list task with exactly CNT lags, whole chunk: the low word of w[i] holds the OLD row of lag i; its
 // kChunk rows are contiguous (duplicated slot 0) ----
 template <int CNT, int TPX>
-__device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH) {
+__device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH,
+                                             int doI, f2x& i2, f2x& i1) {
   const f2x* ol[CNT];
 #pragma unroll
   for (int i = 0; i < CNT; ++i) ol[i] = oldl + (size_t)(unsigned)w[i] * TPX;
@@ -233,6 +277,8 @@ __device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const
     const f2x zn = newc[(size_t)u * TPX];
 #pragma unroll
     for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, ol[i][(size_t)u * TPX]);
+    if (doI & 1) i2 = fma2(zn, zn, i2);
+    if (doI & 2) i1 = add2(i1, zn);
   }
 #pragma unroll
   for (int i = 0; i < CNT; ++i) {
@@ -243,15 +289,22 @@ __device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const
 }
 template <int TPX>
 __device__ __forceinline__ void sparse_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
-                                                      int DEPTH) {
+                                                      int DEPTH, int doI, f2x& i2, f2x& i1) {
   switch (cnt) {
-    case 0: break;  // a task that only accumulates the I sums
-    case 1: sparse_chunk<1, TPX>(acc, w, newc, oldl, DEPTH); break;
-    case 2: sparse_chunk<2, TPX>(acc, w, newc, oldl, DEPTH); break;
-    case 3: sparse_chunk<3, TPX>(acc, w, newc, oldl, DEPTH); break;
-    case 4: sparse_chunk<4, TPX>(acc, w, newc, oldl, DEPTH); break;
-    case 5: sparse_chunk<5, TPX>(acc, w, newc, oldl, DEPTH); break;
-    default: sparse_chunk<kSparseMax, TPX>(acc, w, newc, oldl, DEPTH); break;  // the plan makes lag lists of <= kSparseMax
+    case 0:  // a task that only accumulates the I sums
+#pragma unroll
+      for (int u = 0; u < kChunk; ++u) {
+        const f2x zn = newc[(size_t)u * TPX];
+        i2 = fma2(zn, zn, i2);
+        i1 = add2(i1, zn);
+      }
+      break;
+    case 1: sparse_chunk<1, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
+    case 2: sparse_chunk<2, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
+    case 3: sparse_chunk<3, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
+    case 4: sparse_chunk<4, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
+    case 5: sparse_chunk<5, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
+    default: sparse_chunk<kSparseMax, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;  // lag lists of <= kSparseMax
   }
 }
 
@@ -311,19 +364,20 @@ __device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* o
   for (int g = 0; g < kG; ++g) acc[g] = 0ull;
 }
 
-template <int NCW, bool PERS, bool SKIP>
-__global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 registers: 5 warps per SM sub-partition
+template <int NCW, int SLOTS, bool PERS, bool SKIP>
+__global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P,
                 int64_t t0_batch, int b_batch, int gbase, int ngroups, int lbase, int stages,
                 const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups, const int32_t* __restrict__ lags,
                 double* __restrict__ totals, double* __restrict__ I2, double2* __restrict__ I1, int ntiles,
                 int* __restrict__ claim) {
   constexpr int G = kG;
-  constexpr int TPX = NCW * 4;  // pixels per tile: one 32-pixel sub-tile per 8 consumer warps
-  static_assert(NCW == 8 || NCW == 16, "8 task slots x 1 or 2 sub-tiles");
-  static_assert(kChunk % G == 0 && kChunk <= 32, "a chunk is a whole number of G-step blocks, one lane per row");
-  static_assert(kSparseMax == 6, "sparse_chunk_dispatch lists cases 0..5 and the default");
-  static_assert(kTaskSlots == 8, "warp_task[], sub-tile = warp >> 3");
+  constexpr int TPX = 32 * (NCW / SLOTS);  // pixels per tile: one 32-pixel sub-tile per SLOTS consumer warps
+  static_assert(NCW == SLOTS || NCW == 2 * SLOTS, "SLOTS task slots x 1 or 2 sub-tiles");
+  static_assert(NCW + 1 <= 32, "at most 1024 threads");
+  static_assert(kChunk % G == 0 && kChunk <= 32 && 2 * G - 1 <= kChunk, "a chunk is a whole number of G-step blocks, one lane per row");
+  static_assert(kSparseMax == 6 && kSparseMax <= G, "sparse_chunk_dispatch lists cases 0..5 and the default");
+  static_assert(SLOTS <= 16 && SLOTS % 4 == 0, "warp_task[16], whole sub-partition rounds");
   extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ int s_lags[NCW * kG];  // the lags of each sparse task, for the warm-up path
   __shared__ int s_tile[kMaxStages];  // tile of the item whose first step uses this stage, or -1: no more work
@@ -372,7 +426,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
   const int V = nchunks + LEAD;
 
   if (tid == 0) {
-    const unsigned nt = (unsigned)grp.ntasks * (NCW / kTaskSlots);
+    const unsigned nt = (unsigned)grp.ntasks * (NCW / SLOTS);
     for (int s = 0; s < stages; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], nt);
@@ -439,12 +493,12 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
   }
 
   // ------------------------------- consumers -------------------------------
-  const int sub = warp >> 3;  // 32-pixel sub-tile of this warp
-  const int tix = grp.warp_task[warp & (kTaskSlots - 1)];
+  const int sub = warp / SLOTS;  // 32-pixel sub-tile of this warp
+  const int tix = grp.warp_task[warp % SLOTS];
   if (tix < 0) return;
   const LagTask tk = tasks[grp.task0 + tix];
   const bool dense = (tk.kind & 1) == 0;
-  const bool doI = (tk.kind & 2) != 0;  // this warp also accumulates I2 += |F'_s|^2, I1 += F'_s (one group only)
+  const int doI = (tk.kind >> 1) & 3;  // bit 0: this warp also accumulates I2 += |F'_s|^2; bit 1: I1 += F'_s
   const int cnt = tk.cnt;
   f2x i2 = 0ull, i1 = 0ull;             // fp32 partials of the I sums (<= kFoldChunks * kChunk terms, like acc)
   // Dense task: acc[0] direct sum of lag tau0, acc[g] cross sum of lag tau0 + g against tau0 + g - 1; w = rotating
@@ -525,17 +579,6 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
     const int j0 = c * kChunk;
     if (j0 >= j_all && j0 + kChunk <= b) {
       // ---- fast chunk: every pair of every step exists ----
-      if (doI) {
-#pragma unroll 1
-        for (int blk = 0; blk < kChunk / G; ++blk) {
-#pragma unroll
-          for (int u = 0; u < G; ++u) {
-            const f2x zn = newc[(size_t)(blk * G + u) * TPX];
-            i2 = fma2(zn, zn, i2);
-            i1 = add2(i1, zn);
-          }
-        }
-      }
       if (dense) {
         if (!open) {
           // first whole chunk of the segment: the |z|^2 of the OLD frames just before it enter the totals of the
@@ -554,16 +597,12 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
             }
           }
         }
-        dense_chunk_dispatch<TPX>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
+        dense_chunk_dispatch<TPX>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
         oend = o0;
       } else {
-        sparse_chunk_dispatch<TPX>(cnt, acc, w, newc, oldl, DEPTH);
+        sparse_chunk_dispatch<TPX>(cnt, acc, w, newc, oldl, DEPTH, doI, i2, i1);
       }
     } else {
-    if (dense && open) {  // the whole chunks before this one: fold them while their last window rows are resident
-      if (p < P) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
-      open = false;
-    }
 #pragma unroll 1
     for (int blk = 0; blk < kChunk / G; ++blk) {  // warm-up and the batch's last, partial chunk: checked per block
       const int jb = c * kChunk + blk * G;  // batch-relative index of the block's first step
@@ -575,17 +614,40 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
         for (int u = 0; u < G; ++u) {
           if (u < ns) {
             const f2x zn = nb[(size_t)u * TPX];
-            i2 = fma2(zn, zn, i2);
-            i1 = add2(i1, zn);
+            if (doI & 1) i2 = fma2(zn, zn, i2);
+            if (doI & 2) i1 = add2(i1, zn);
           }
         }
       }
       if (jb + ns <= j_any) {
         // no pair of this task yet
+      } else if (dense && jb >= j_all) {
+        // ---- the batch's last chunk: every pair of the block's ns steps exists: same recurrence, predicated steps ----
+        if (!open) {
+          open = true;
+          double pre = 0.0;
+          int r = o0;
+#pragma unroll
+          for (int g = 1; g < G; ++g) {
+            if (g < cnt) {
+              if (--r < 0) r += DEPTH;
+              const f2x z = oldl[(size_t)r * TPX];
+              pre += norm2_f64(make_float2(f2x_lo(z), f2x_hi(z)));
+              if (p < P) atomicAdd(&tot[(int64_t)g * P + p], pre);
+            }
+          }
+        }
+        dense_partial_dispatch<TPX>(cnt, ns, acc, w, zprev, wvalid, nb, oldl, o0, DEPTH);
+        oend = o0 + ns;
+        if (oend >= DEPTH) oend -= DEPTH;
       } else if (dense) {
         // ---- masked block of a run of lags: every existing pair directly, pair (step u, lag tau0 + g) exists
         // iff u - g >= vbase and u < ns; straight into the fp64 totals (rare: the warm-up of a stack and the
         // ragged tail of a batch).  Rows o0 - (G-1) .. o0 + G-1 are contiguous thanks to the duplicated slot. ----
+        if (open) {  // (not reached in practice: warm-up blocks precede the whole chunks) fold what is open first
+          if (p < P) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
+          open = false;
+        }
         const int vbase = (int)max((int64_t)-64, (int64_t)tk.tau0 - t0 - jb);
         int rb = o0 - (G - 1);
         if (rb < 0) rb += DEPTH;
@@ -619,11 +681,12 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
       }
     }
     }
+    if (c == cend - 1) break;  // the segment's last chunk is released after the fold below, which reads its window rows
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[st]);
     if (++st == stages) st = 0, ph ^= 1u;
   }
-  // fold the fp32 partial sums (<= kFoldChunks * kChunk terms) into the fp64 totals: one reduction
+// fold the fp32 partial sums (<= kFoldChunks * kChunk terms) into the fp64 totals: one reduction
   // (RED.ADD.F64 in L2, nothing returns to the SM) per (lag, pixel).  Every address has one writer per
   // launch, which folds in program order, and launches are stream ordered: the order of the additions
   // is fixed and the result deterministic.
@@ -635,8 +698,8 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
       for (int g = 0; g < G; ++g)
         if (g < cnt) atomicAdd(&tot[(int64_t)g * P + p], (double)f2x_sum(acc[g]));
     }
-    if (doI) {
-      atomicAdd(&I2[p], (double)f2x_sum(i2));
+    if (doI & 1) atomicAdd(&I2[p], (double)f2x_sum(i2));
+    if (doI & 2) {
       atomicAdd(&I1[p].x, (double)f2x_lo(i1));
       atomicAdd(&I1[p].y, (double)f2x_hi(i1));
     }
@@ -644,6 +707,9 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW == 8 ? 2 : 1)  // 96 regis
 #pragma unroll
   for (int g = 0; g < G; ++g) acc[g] = 0ull;
   i2 = 0ull, i1 = 0ull;
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&empty[st]);
+  if (++st == stages) st = 0, ph ^= 1u;
   }
   }
 }
@@ -664,10 +730,10 @@ struct Atom {
 // issue slots per time step: a run costs 2 loads, the increment, the direct update (2) and one FMA per further lag;
 // a lag list one load and two packed operations per lag plus the load of the new frame
 double task_cost(const LagTask& t) {
-  return ((t.kind & 1) == 0 ? 4.0 + t.cnt : 3.0 * t.cnt + 1.0) + ((t.kind & 2) ? 3.0 : 0.0);
+  return ((t.kind & 1) == 0 ? 4.0 + t.cnt : 3.0 * t.cnt + 1.0) + ((t.kind & 2) ? 1.0 : 0.0) + ((t.kind & 4) ? 1.0 : 0.0);
 }
 
-void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1, bool with_I,
+void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1, bool with_I, int slots,
                  std::vector<LagTask>& tasks, std::vector<LagGroup>& groups) {
   LagGroup g;
   g.task0 = (int)tasks.size();
@@ -678,7 +744,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   // sparse task size: small enough to use the free slots, large enough to fit them
   int s = 1;
   if (n_sparse > 0) {
-    const int free_w = kTaskSlots - n_dense;
+    const int free_w = slots - n_dense;
     s = std::min(kSparseMax, std::max(1, (n_sparse + free_w - 1) / std::max(1, free_w)));
     for (;; ++s) {  // stretches are cut separately: make sure the slots suffice
       int need = 0;
@@ -713,16 +779,18 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   }
   g.ntasks = (int)tasks.size() - g.task0;
   g.flags = with_I ? 1 : 0;
-  if (with_I) {  // this group also accumulates the I sums (kind bit 1): on a slot of its own if one is free,
-                 // else on its lightest task
-    if (g.ntasks < kTaskSlots) {
-      tasks.push_back(LagTask{0, 0, 0, 1 | 2});
+  if (with_I) {  // this group also accumulates the I sums (kind bits 1, 2): on a slot of its own if one is free,
+                 // else on its lightest tasks
+    if (g.ntasks < slots) {
+      tasks.push_back(LagTask{0, 0, 0, 1 | 2 | 4});
       g.ntasks += 1;
-    } else {
-      int best = 0;
-      for (int k = 1; k < g.ntasks; ++k)
-        if (task_cost(tasks[g.task0 + k]) < task_cost(tasks[g.task0 + best])) best = k;
-      tasks[g.task0 + best].kind |= 2;
+    } else {  // sum |F'|^2 (bit 1) and sum F' (bit 2) ride on the two lightest tasks: one packed operation per step each
+      for (int bit = 2; bit <= 4; bit *= 2) {
+        int best = 0;
+        for (int k = 1; k < g.ntasks; ++k)
+          if (task_cost(tasks[g.task0 + k]) < task_cost(tasks[g.task0 + best])) best = k;
+        tasks[g.task0 + best].kind |= bit;
+      }
     }
   }
   // placement: heaviest task first onto the least loaded sub-partition that still has a free slot
@@ -736,7 +804,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
   for (int k : order) {
     int best = -1;
     for (int q = 0; q < 4; ++q)
-      if (used[q] < kTaskSlots / 4 && (best < 0 || load[q] < load[best])) best = q;
+      if (used[q] < slots / 4 && (best < 0 || load[q] < load[best])) best = q;
     g.warp_task[used[best] * 4 + best] = (signed char)k;
     used[best] += 1;
     load[best] += task_cost(tasks[g.task0 + k]);
@@ -746,7 +814,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 }
 }  // namespace
 
-bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
+static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
   const std::vector<int32_t>& L = c.lags;
   // shared memory a CTA may use: the opt-in maximum (one CTA per SM) bounds a group's window; two CTAs of 32-pixel
   // tiles share an SM when the plan's footprint allows it (1 KB per CTA is reserved, 1 KB static)
@@ -793,7 +861,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
       need += ((int)(e - a) + kSparseMax - 1) / kSparseMax;
       a = e;
     }
-    return need <= kTaskSlots;
+    return need <= slots;
   };
   std::vector<std::pair<size_t, size_t>> cuts;
   size_t a0 = 0;
@@ -815,7 +883,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
     if (nl(cuts[k]) < nl(cuts[gI])) gI = k;
     c.max_group_lags = std::max(c.max_group_lags, nl(cuts[k]));
   }
-  for (size_t k = 0; k < cuts.size(); ++k) close_group(L, atoms, cuts[k].first, cuts[k].second, k == gI, c.tasks, c.groups);
+  for (size_t k = 0; k < cuts.size(); ++k) close_group(L, atoms, cuts[k].first, cuts[k].second, k == gI, slots, c.tasks, c.groups);
   for (LagGroup& g : c.groups)
     if (single_of(g.tau_min, g.tau_max)) g.flags |= 2;
   // tile width and pipeline depth.  64-pixel tiles (16 consumer warps, one CTA per SM, 512-byte rows) when every
@@ -826,13 +894,13 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
     return m;
   };
   int tpx = 32, per_sm = 1, stages = kMinStages;
-  if (P % 64 == 0 && smem_for(kMinStages + 1, 64) <= budget) {
+  if (slots == kTaskSlots && P % 64 == 0 && smem_for(kMinStages + 1, 64) <= budget) {
     tpx = 64;
     stages = kMinStages + 1;
     while (stages < kMaxStages && smem_for(stages + 1, 64) <= budget) ++stages;
   } else {
     const size_t half = (size_t)std::max(0, smem_sm / 2 - 2048);
-    if (smem_for(kMinStages + 1, 32) <= half) {
+    if (slots == kTaskSlots && smem_for(kMinStages + 1, 32) <= half) {
       per_sm = 2;
       stages = kMinStages + 1;
       while (stages < kMaxStages && smem_for(stages + 1, 32) <= half) ++stages;
@@ -845,6 +913,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
   c.lag_stages = stages;
   c.lag_smem = smem;
   c.lag_tpx = tpx;
+  c.lag_slots = slots;
   c.lag_ctas_per_sm = per_sm;
   // persistent CTAs: the resident CTAs of the device are shared out in proportion to the groups' work per pixel
   // tile (issue slots of the tasks + a constant for streaming the window), at least one CTA each
@@ -886,18 +955,39 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
   return true;
 }
 
+// The plan nfs_create uses.  Eight task slots per group with 64-pixel tiles (16 consumer warps) or two CTAs of
+// 32-pixel tiles per SM; a plan whose window leaves room for one 32-pixel CTA per SM only (long lag spans: isolated
+// lags) is redone with sixteen task slots, so that sixteen consumer warps share the SM there too.
+bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
+  if (!plan_with(c, kTaskSlots, smem_sm, n_sm, P)) return false;
+  if (c.lag_tpx == 32 && c.lag_ctas_per_sm == 1) {
+    Ctx alt = c;
+    if (plan_with(alt, 2 * kTaskSlots, smem_sm, n_sm, P)) {
+      c.tasks = alt.tasks, c.groups = alt.groups;
+      c.lag_stages = alt.lag_stages, c.lag_smem = alt.lag_smem, c.lag_tpx = alt.lag_tpx, c.lag_slots = alt.lag_slots;
+      c.lag_ctas_per_sm = alt.lag_ctas_per_sm, c.lag_grid = alt.lag_grid, c.max_group_lags = alt.max_group_lags;
+    }
+  }
+  return true;
+}
+
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
 namespace {
 typedef void (*LagKernel)(const CUtensorMap, const float2*, int, int64_t, int64_t, int, int, int, int, int, const LagTask*,
                           const LagGroup*, const int32_t*, double*, double*, double2*, int, int*);
-LagKernel lag_kernel(int tpx, bool pers, bool skip) {
-  if (tpx == 64)
-    return pers ? (skip ? k_lag_tiled<16, true, true> : k_lag_tiled<16, true, false>)
-                : (skip ? k_lag_tiled<16, false, true> : k_lag_tiled<16, false, false>);
-  return pers ? (skip ? k_lag_tiled<8, true, true> : k_lag_tiled<8, true, false>)
-              : (skip ? k_lag_tiled<8, false, true> : k_lag_tiled<8, false, false>);
+template <int NCW, int SLOTS>
+LagKernel lag_kernel_of(bool pers, bool skip) {
+  return pers ? (skip ? k_lag_tiled<NCW, SLOTS, true, true> : k_lag_tiled<NCW, SLOTS, true, false>)
+              : (skip ? k_lag_tiled<NCW, SLOTS, false, true> : k_lag_tiled<NCW, SLOTS, false, false>);
+}
+// (tile pixels, task slots): (64, 8) 16 consumer warps on two sub-tiles; (32, 8) 8 consumer warps, two CTAs per SM
+// where they fit; (32, 16) 16 consumer warps on sixteen tasks
+LagKernel lag_kernel(int tpx, int slots, bool pers, bool skip) {
+  if (slots == 2 * kTaskSlots) return lag_kernel_of<2 * kTaskSlots, 2 * kTaskSlots>(pers, skip);
+  if (tpx == 64) return lag_kernel_of<2 * kTaskSlots, kTaskSlots>(pers, skip);
+  return lag_kernel_of<kTaskSlots, kTaskSlots>(pers, skip);
 }
 }  // namespace
 
@@ -928,7 +1018,7 @@ bool lag_configure(Ctx& c) {
     return false;
   }
   for (int v = 0; v < 4; ++v)
-    if (!NFS_CUDA(c, cudaFuncSetAttribute(lag_kernel(c.lag_tpx, (v & 1) != 0, (v & 2) != 0),
+    if (!NFS_CUDA(c, cudaFuncSetAttribute(lag_kernel(c.lag_tpx, c.lag_slots, (v & 1) != 0, (v & 2) != 0),
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.lag_smem)))
       return false;
   return true;
@@ -938,7 +1028,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   const int ngroups = (int)c.groups.size();
   const int tpx = c.lag_tpx;
   const int ntiles = (int)((c.P + tpx - 1) / tpx);
-  const int nthreads = (tpx / 4 + 1) * 32;
+  const int nthreads = (c.lag_slots * (tpx / 32) + 1) * 32;
   int n = 0;
   if (c.bin_only) {
     // PAPER.md:L41 ("store the entire 2D power spectra, which might be unnecessary"): one lag group per launch into
@@ -954,7 +1044,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
         {
           ProfScope ps(c, kKLag);
           if (!NFS_CUDA(c, cudaMemsetAsync(c.totals, 0, sizeof(double) * (size_t)nl * c.P, c.stream))) return n;
-          lag_kernel(tpx, false, skip)<<<(unsigned)ntiles, nthreads, c.lag_smem, c.stream>>>(
+          lag_kernel(tpx, c.lag_slots, false, skip)<<<(unsigned)ntiles, nthreads, c.lag_smem, c.stream>>>(
               c.ring_map, c.ring, c.R, c.P, t0, b, g, 1, lbase, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2,
               c.I1, ntiles, c.d_claim);
           n += 1;
@@ -981,7 +1071,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   for (const LagGroup& g : c.groups)
     skip |= !(g.flags & 1) && (int64_t)g.tau_min - t0 >= kChunk && (int64_t)g.tau_min <= t0 + b - 1;
   if (persistent && !NFS_CUDA(c, cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream))) return 0;
-  lag_kernel(tpx, persistent, skip)<<<grid, nthreads, c.lag_smem, c.stream>>>(
+  lag_kernel(tpx, c.lag_slots, persistent, skip)<<<grid, nthreads, c.lag_smem, c.stream>>>(
       c.ring_map, c.ring, c.R, c.P, t0, b, 0, ngroups, 0, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1,
       ntiles, c.d_claim);
   return 1;

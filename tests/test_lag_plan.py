@@ -14,7 +14,6 @@ from paper_1209_3362_b200 import binding
 
 KG = 13          # lags per register-window task (nfs_common.cuh: kG)
 KS = 6           # lags per lag-list task (kSparseMax)
-MAX_TASKS = 8    # task slots per group (kTaskSlots)
 N_SM = 148
 P_1024 = 1024 * 513   # Fourier pixels of a 1024 x 1024 frame
 SMEM_SM = 233472   # B200: shared memory per SM
@@ -29,16 +28,18 @@ def check_plan(lags, plan, n_px=P_1024):
     lags = list(lags)
     groups, tasks = plan["groups"], plan["tasks"]
     covered = np.zeros(len(lags), dtype=int)
-    n_I = 0
+    n_I2 = n_I1 = 0
     seen_tasks = set()
     assert sum(g["flags"] & 1 for g in groups) == 1, "exactly one group accumulates the I sums"
+    MAX_TASKS = plan["slots"]   # task slots per group: 8, or 16 for one 32-pixel CTA of 16 consumer warps per SM
+    assert MAX_TASKS in (8, 16) and (MAX_TASKS == 8 or (plan["tile_px"], plan["ctas_per_sm"]) == (32, 1))
     for g in groups:
         assert 1 <= g["ntasks"] <= MAX_TASKS
         placed = [w for w in g["warp_task"] if w >= 0]
         assert sorted(placed) == list(range(g["ntasks"])), "every task of a group runs on exactly one warp"
         assert all(w < 0 for w in g["warp_task"][MAX_TASKS:])
         lo, hi = 1 << 30, 0
-        has_I = 0
+        has_I2 = has_I1 = 0
         for k in range(g["ntasks"]):
             ti = g["task0"] + k
             assert ti not in seen_tasks
@@ -47,9 +48,10 @@ def check_plan(lags, plan, n_px=P_1024):
             assert 0 <= t["cnt"] <= (KG if (t["kind"] & 1) == 0 else KS)
             if (t["kind"] & 1) == 0:
                 assert t["cnt"] >= 2, "a register-window task has a direct lag and at least one neighbour"
-            has_I += (t["kind"] >> 1) & 1
+            has_I2 += (t["kind"] >> 1) & 1
+            has_I1 += (t["kind"] >> 2) & 1
             if t["cnt"] == 0:
-                assert t["kind"] == 3, "a task without lags only accumulates I"
+                assert t["kind"] == 7, "a task without lags only accumulates I"
                 continue
             own = lags[t["l0"]:t["l0"] + t["cnt"]]
             assert len(own) == t["cnt"] and own[0] == t["tau0"]
@@ -57,10 +59,11 @@ def check_plan(lags, plan, n_px=P_1024):
                 assert own == list(range(t["tau0"], t["tau0"] + t["cnt"])), "a dense task is a run of consecutive lags"
             covered[t["l0"]:t["l0"] + t["cnt"]] += 1
             lo, hi = min(lo, own[0]), max(hi, own[-1])
-        assert has_I == (g["flags"] & 1)
-        n_I += has_I
+        assert has_I2 == has_I1 == (g["flags"] & 1), "sum |F'|^2 and sum F' each ride on exactly one task"
+        n_I2 += has_I2
+        n_I1 += has_I1
         assert (g["tau_min"], g["tau_max"]) == (lo, hi)
-    assert n_I == 1
+    assert n_I2 == 1 and n_I1 == 1
     # persistent CTAs: contiguous shares, at least one per group, all resident slots handed out
     at = 0
     for g in groups:
@@ -90,6 +93,7 @@ def test_plan_of_baseline_configs(ci):
         assert plan["groups"][0]["flags"] == 3 and plan["tile_px"] == 64
     if ci == 3:       # 40 log-spaced lags <= 500: one pass over the tile (one group, the whole window in shared memory)
         assert len(plan["groups"]) == 1 and plan["groups"][0]["flags"] == 3 and plan["tile_px"] == 32
+        assert plan["slots"] == 16 and len(plan["tasks"]) > 8
     if ci == 4:       # lags 1..1000: ten groups of ~104 lags, only the first streams the batch as the head of its window
         assert len(plan["groups"]) == 10
         assert [g["flags"] & 2 for g in plan["groups"]] == [2] + [0] * 9
