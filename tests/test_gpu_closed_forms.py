@@ -1,6 +1,6 @@
 """The CUDA path against what the mathematics fixes directly (the same closed forms that pin the oracle, SURVEY.md
-§8(c) P3-P6, P9), and — at BASELINE.json's full sizes, in the launch configuration bench.py times — against the
-oracle on sampled Fourier pixels plus properties that hold at any size."""
+§8(c) P3-P6, P9) and the variance form of the fluctuation spectrum against oracle step 7.  The full-size comparisons
+with the oracle are in tests/test_gpu_full_size.py."""
 import numpy as np
 import pytest
 import torch
@@ -130,101 +130,6 @@ def test_parseval_and_dc(binding):
         four = (D2d[l] * wgt[None, :]).sum()
         assert four == pytest.approx(real, rel=1e-5)
         assert D2d[l, 0, 0] < 1e-9 * D2d[l].max()
-
-
-# --------------------------------------------------------------------------------------------------------------
-# full sizes, bench.py's launch configuration (default internal batch, one push of the whole stack)
-# --------------------------------------------------------------------------------------------------------------
-def _sample_pixels(W, H, n_rand, seed):
-    n = W // 2
-    rng = np.random.default_rng(seed)
-    ky = [0, 1, 0, 1, H // 2, H - 1, 3, H // 4, 0, H // 2, 7]
-    kx = [1, 0, 2, 1, 0, 1, n, n, n - 1, n, 0]
-    # low-|q| region where the signal lives, plus uniform samples of the whole half plane
-    ky += list(rng.integers(0, 24, n_rand)) + list(rng.integers(0, H, n_rand))
-    kx += list(rng.integers(0, 24, n_rand)) + list(rng.integers(0, n + 1, n_rand))
-    return np.array(ky, dtype=np.int32), np.array(kx, dtype=np.int32)
-
-
-@pytest.mark.parametrize("idx", [1, 2, 3])
-def test_full_size_sampled_pixels_and_invariants(binding, oracle, idx):
-    cfg = synth.config(idx)            # 512^2 x 1000 / 1024^2 x 2000, lags 1..100 / 2048^2 x 1000, 40 log-spaced lags
-    st = synth.make_stack(cfg, "cuda")
-    nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins)
-    nfs.push(st)
-    D, I_q, cnt = nfs.finalize()
-    sel = [0, 1, 9, 10, 49, 98, 99] if idx != 3 else [0, 9, 10, 18, 19, 21, 34, 35, 39]
-    D2d = {l: nfs.D2d(l) for l in sel}
-    I2d = nfs.I2d()
-    npairs = nfs.pair_counts()
-    nfs.close()
-    assert npairs.tolist() == [cfg.N - t for t in cfg.lags]
-    # exact, data-independent bin counts
-    assert cnt[:8].tolist() == [8, 36, 64, 84, 112, 132, 172, 184]
-    assert int(cnt.sum()) == {1: 205856, 2: 823468, 3: 3294092}[idx]
-    # sampled pixels against the oracle (full fp64 transform of every frame, explicit pair loop)
-    ky, kx = _sample_pixels(cfg.W, cfg.H, 24, seed=idx)
-    ref = oracle.structure_function_sampled(st.cpu().numpy(), cfg.lags, ky, kx)
-    dmax = max(D2d[l].max() for l in sel)
-    worst = 0.0
-    for l in sel:
-        g = D2d[l][ky, kx]
-        r = ref.D2d[l]
-        m = r > 1e-6 * dmax
-        assert m.sum() >= 8
-        worst = max(worst, float((np.abs(g - r)[m] / r[m]).max()))
-    assert worst < 1e-3, worst
-    gI = I2d[ky, kx]
-    assert (np.abs(gI - ref.I2d) / ref.I2d).max() < 1e-2
-    # invariants that hold at any size: conservation of the azimuthal mean, D2d(DC) = 0, symmetry of the ky axis
-    n = cfg.W // 2
-    wgt = np.full(n + 1, 2.0)
-    wgt[0] = wgt[n] = 1.0
-    kyy = np.arange(cfg.H)
-    sy = np.where(kyy < cfg.H // 2, kyy, kyy - cfg.H)[:, None].astype(np.float64)
-    sx = np.arange(n + 1)[None, :].astype(np.float64)
-    q2 = 4.0 * ((sx / cfg.W) ** 2 + (sy / cfg.H) ** 2)
-    inc = (q2 < 1.0) & ~((sx == 0) & (sy == 0))
-    for l in sel:
-        lhs = float((cnt * D[l]).sum())
-        rhs = float((D2d[l] * wgt[None, :])[inc].sum())
-        assert lhs == pytest.approx(rhs, rel=1e-9)
-        assert D2d[l][0, 0] < 1e-9 * D2d[l].max()
-        # kx = 0 column is Hermitian in ky: D2d(ky, 0) = D2d(-ky, 0)
-        col = D2d[l][:, 0]
-        assert np.abs(col[1:cfg.H // 2] - col[:cfg.H // 2:-1]).max() <= 1e-4 * col.max()
-
-
-def test_config4_shape_streamed_sampled_pixels(binding, oracle):
-    """BASELINE.json configs[4] at reduced length: 1024^2 frames pushed in chunks of 256 (as from pinned host
-    memory), all lags 1..1000 (ten lag groups), 2600 frames so that the Fourier ring (1000 + 1024 slots) wraps;
-    sampled pixels against the oracle's explicit pair loop."""
-    cfg = synth.config(4, N=2600)
-    assert cfg.lags == list(range(1, 1001)) and cfg.chunk == 256
-    st = synth.make_stack(cfg, "cuda")
-    nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins)
-    assert nfs.ring_capacity == 2024
-    for i in range(0, cfg.N, cfg.chunk):
-        nfs.push(st[i:i + cfg.chunk])
-    D, I_q, cnt = nfs.finalize()
-    sel = [0, 12, 13, 103, 104, 500, 998, 999]
-    D2d = {l: nfs.D2d(l) for l in sel}
-    npairs = nfs.pair_counts()
-    nfs.close()
-    assert npairs.tolist() == [cfg.N - t for t in cfg.lags]
-    assert int(cnt.sum()) == 823468
-    ky, kx = _sample_pixels(cfg.W, cfg.H, 16, seed=4)
-    ref = oracle.structure_function_sampled(st.cpu().numpy(), cfg.lags, ky, kx)
-    dmax = max(D2d[l].max() for l in sel)
-    worst = 0.0
-    for l in sel:
-        g = D2d[l][ky, kx]
-        r = ref.D2d[l]
-        m = r > 1e-6 * dmax
-        assert m.sum() >= 8
-        worst = max(worst, float((np.abs(g - r)[m] / r[m]).max()))
-    assert worst < 1e-3, worst
-    assert np.all(np.isfinite(D)) and np.all(D[:, cnt > 0] > 0)
 
 
 # --------------------------------------------------------------------------------------------------------------
