@@ -26,9 +26,38 @@ import numpy as np  # noqa: E402
 
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128
-# DRAM bytes (read + write) of one k_lag_tiled launch from the committed `ncu --set full` capture
-# (profiles/r01_lag_ncu.md), keyed by (workload, internal batch, frames); other workloads report null.
-NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH = {("config2", 1024, 2000): 0.5 * (5.272e9 + 5.497e9)}  # profiles/r01_lag_ncu.md
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "lag_traffic.csv")
+LAG_SOURCES = ["paper_1209_3362_b200/csrc/nfs_lag.cu", "paper_1209_3362_b200/csrc/nfs_common.cuh"]
+
+
+def lag_source_sha():
+    """SHA-256 (16 hex digits) of the lag kernel's sources: the key under which an ncu traffic figure is valid."""
+    import hashlib
+
+    h = hashlib.sha256()
+    for f in LAG_SOURCES:
+        h.update(open(os.path.join(ROOT, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_lag_traffic(workload, batch, frames):
+    """DRAM bytes (read + write) per k_lag_tiled launch from the committed `ncu --set full` capture
+    (profiles/lag_traffic.csv: workload,batch,frames,source_sha16,bytes_per_launch,capture).  Returned only if the
+    capture was taken from the kernel sources of this tree; otherwise null with the reason."""
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, "no profiles/lag_traffic.csv"
+    sha = lag_source_sha()
+    stale = False
+    for line in open(TRAFFIC_CSV):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) < 6 or f[0] == "workload":
+            continue
+        if (f[0], f[1], f[2]) == (workload, str(batch), str(frames)):
+            if f[3] == sha:
+                return float(f[4]), "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/" + f[5]
+            stale = True
+    return None, ("the ncu capture in profiles/lag_traffic.csv is of other kernel sources (sha16 now %s)" % sha) if stale else \
+        "no ncu capture of this workload"
 
 
 def load_peaks():
@@ -133,6 +162,36 @@ def workload_counts(cfg):
     return P, pairs
 
 
+def lag_algorithmic_work(cfg, binding):
+    """FP32 work of the lag accumulation per Fourier pixel and time step (all pairs present), from the lag plan
+    (DESIGN.md 7.2): a run of c consecutive lags costs one complex increment (2 lane-instructions, 2 flops), the direct
+    update of its smallest lag (2 SUB + 2 FMA = 4 lane-instructions, 6 flops) and one complex FMA per further lag
+    (2 lane-instructions, 4 flops); an isolated lag costs the direct update.  -> (lane-instructions, flops)."""
+    plan = binding.nfs_plan_lags(cfg.lags, cfg.H * (cfg.W // 2 + 1))
+    inst = flop = 0
+    for t in plan["tasks"]:
+        c = t["cnt"]
+        if c == 0:
+            continue
+        if (t["kind"] & 1) == 0:
+            inst += 2 + 4 + 2 * (c - 1)
+            flop += 2 + 6 + 4 * (c - 1)
+        else:
+            inst += 4 * c
+            flop += 6 * c
+    return inst, flop, plan
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def oracle_sample_frames(cfg):
     """Frames of the bounded oracle sample: about 10-30 s of CPU work on the box's host cores."""
     return min(cfg.N, 128 if cfg.W >= 2048 else (400 if cfg.W >= 1024 else (1000 if cfg.W >= 512 else cfg.N)))
@@ -149,9 +208,13 @@ def oracle_sample(cfg, stack_np_fn):
     dt = time.time() - t
     pairs_s = sum(max(0, n_s - t) for t in cfg.lags)
     pairs_full = sum(max(0, cfg.N - t) for t in cfg.lags)
-    desc = ("first %d frames of the %dx%d stack, all %d lags, full-plane fp64 oracle (oracle/nfs_oracle.c); the sample has "
-            "%.1f frame pairs per frame, the full stack %.1f" % (n_s, cfg.W, cfg.H, len(cfg.lags), pairs_s / n_s, pairs_full / cfg.N))
-    return n_s / dt, dt, desc, orc.num_threads()
+    desc = ("first %d frames of the %dx%d stack, all %d lags, full-plane fp64 oracle (oracle/nfs_oracle.c: it evaluates "
+            "both halves of the Hermitian plane, twice the pixels the kernels touch); the sample has %.1f frame pairs per "
+            "frame, the full stack %.1f" % (n_s, cfg.W, cfg.H, len(cfg.lags), pairs_s / n_s, pairs_full / cfg.N))
+    fft_s, pair_s = orc.last_stage_seconds()
+    extra = dict(cpu_model=cpu_model(), fft_stage_seconds=fft_s, pair_stage_seconds=pair_s,
+                 frame_pairs_per_s=pairs_s / dt, pixel_pair_updates_per_s=pairs_s * cfg.W * cfg.H / dt)
+    return n_s / dt, dt, desc, orc.num_threads(), extra
 
 
 def run_reference(args, cfg):
@@ -164,9 +227,9 @@ def run_reference(args, cfg):
     n_s = oracle_sample_frames(cfg)
     frames = gen.next_frames(n_s).numpy()
     times = []
-    desc, cores = "", 0
+    desc, cores, extra = "", 0, {}
     for i in range(args.warmup + args.steps):
-        v, dt, desc, cores = oracle_sample(cfg, lambda n: frames[:n])
+        v, dt, desc, cores, extra = oracle_sample(cfg, lambda n: frames[:n])
         if i >= args.warmup:
             times.append(dt)
     T = sum(times) / len(times)
@@ -176,7 +239,7 @@ def run_reference(args, cfg):
                impl="reference",
                config=dict(workload="%s: %dx%d uint16, %d lags, %d |q| bins (bounded sample: %d of %d frames)" % (
                    cfg.name, cfg.W, cfg.H, len(cfg.lags), cfg.n_qbins, n_s, cfg.N)),
-               cpu_baseline=dict(value=val, unit="frames/s", cores=cores, kind="oracle", sample=desc),
+               cpu_baseline=dict(value=val, unit="frames/s", cores=cores, kind="oracle", sample=desc, **extra),
                e2e=dict(value=val, unit="frames/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(out), flush=True)
 
@@ -219,7 +282,7 @@ def run_ours(args, cfg):
         raise RuntimeError("bench.py --impl ours needs a CUDA device: the hot path has no CPU fallback")
     torch.cuda.set_device(local)
     dist = None
-    if world > 1 or os.environ.get("NFS_BENCH_FORCE_DIST"):  # the env switch exercises the N > 1 code path on one GPU
+    if world > 1:
         import torch.distributed as dist_mod
 
         dist = dist_mod
@@ -229,12 +292,12 @@ def run_ours(args, cfg):
     P, pairs = workload_counts(cfg)
     updates = pairs * P
 
+    from paper_1209_3362_b200 import replicas
+
     # every rank analyses its own stack (replicas; seed differs per rank)
-    cfg_r = cfg if rank == 0 else synth.StackConfig(**{**cfg.__dict__, "seed": cfg.seed + 100 * rank, "fringes": []})
-    stack = synth.make_stack(cfg_r, dev)
+    stack = synth.make_stack(replicas.rank_config(cfg, rank), dev)
     stream = torch.cuda.Stream(device=dev)
     nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch)
-    nfs.set_profiling(True)
     torch.cuda.synchronize()
 
     def step():
@@ -244,8 +307,6 @@ def run_ours(args, cfg):
 
     for _ in range(max(args.warmup, 1) if args.warmup else 0):
         step()
-    nfs.kernel_times()
-    launches0 = 0
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
@@ -265,13 +326,21 @@ def run_ours(args, cfg):
         dist.barrier()
     t_wall = time.time() - t_wall
     clocks = sampler.stop() if rank == 0 else None
-    ms_total = e0.elapsed_time(e1)
-    ktimes = nfs.kernel_times()
-    if dist is not None:
-        tt = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = replicas.max_over_ranks(e0.elapsed_time(e1), dist, dev)
     ms_step = ms_total / args.steps
+    # per-kernel durations: the same K steps once more with a CUDA event pair around every launch on the library's
+    # stream (kept out of the headline region: the event records cost a little host and device time)
+    nfs.set_profiling(True)
+    nfs.kernel_times()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record(stream)
+    for _ in range(args.steps):
+        step()
+    e3.record(stream)
+    torch.cuda.synchronize()
+    ktimes = nfs.kernel_times()
+    nfs.set_profiling(False)
+    ms_step_profiled = e2.elapsed_time(e3) / args.steps
     value = world * cfg.N / (ms_step * 1e-3)
 
     # ---- end to end through the C-ABI with the stack in pinned HOST memory ----
@@ -285,50 +354,63 @@ def run_ours(args, cfg):
         return
 
     # ---- roofline of the dominant kernel (lag accumulation, k_lag_tiled) ----
-    # Algorithmic work per launch: one pair update = 2 FADD + 2 FFMA on fp32 = 4 lane-instructions
-    # = 6 flops; the kernel's average launch duration comes from CUDA events recorded around every launch on
-    # the library's stream (nfs_set_profiling) over the timed region.
+    # Algorithmic work per launch: FP32 lane-instructions of the neighbouring-lag recurrence for the
+    # lag plan of this workload x the frame pairs x pixels one launch processes; the kernel's average launch duration
+    # comes from CUDA events recorded around every launch on the library's stream (nfs_set_profiling).
     lag_ms, lag_n = ktimes["lag_accum"]
     lag_s_per_launch = lag_ms * 1e-3 / max(lag_n, 1)
     upd_per_launch = updates * args.steps / max(lag_n, 1)
-    flop_per_update = 6.0
-    inst_per_update = 4.0
-    peak_tflops = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * (flop_per_update / inst_per_update) / 1e12
+    inst_step, flop_step, plan = lag_algorithmic_work(cfg, binding)
+    n_l = len(cfg.lags)
+    inst_per_update, flop_per_update = inst_step / n_l, flop_step / n_l   # averaged over the lags of the plan
+    lane_rate_peak = SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
+    peak_tflops = lane_rate_peak * (flop_per_update / inst_per_update) / 1e12
     ach_tflops = upd_per_launch * flop_per_update / lag_s_per_launch / 1e12
     B = nfs.ring_capacity - cfg.lags[-1]  # the library's internal batch (frames)
     nb = (cfg.N + B - 1) // B
     # algorithmic HBM bytes of the accumulation: 8*U/B + 16*n_l/B per pixel and new frame
     lag_bytes = P * (8.0 * (cfg.N + nb * cfg.lags[-1]) + 16.0 * len(cfg.lags) * nb)
-    traffic = NCU_LAG_TRAFFIC_BYTES_PER_LAUNCH.get((cfg.name, B, cfg.N))
+    traffic, traffic_source = ncu_lag_traffic(cfg.name, B, cfg.N)
     roofline = dict(bound="alu", kernel="k_lag_tiled", achieved=ach_tflops, peak=peak_tflops, unit="TFLOP/s",
-                    frac=ach_tflops / peak_tflops, traffic=traffic,
-                    peak_source="derived (DESIGN.md §7.2): 148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) x 1.5 flop "
-                                "per lane-instruction (2 FADD + 2 FFMA = 6 flops per pair update)" % (peaks["sm_max_mhz"], peaks["source"]),
-                    traffic_source="ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the two batches), profiles/r01_lag_ncu.md",
+                    frac=ach_tflops / peak_tflops, traffic=traffic, traffic_source=traffic_source,
+                    peak_source="derived (DESIGN.md §7.2): 148 SM x 128 FP32 lanes x %.0f MHz (clocks.max.sm, %s) = %.3g "
+                                "lane-instructions/s x %.3f flop per lane-instruction of this lag plan (%.2f lane-instructions, "
+                                "%.2f flops per pair update: one direct update per run of lags, one complex FMA per further lag)"
+                                % (peaks["sm_max_mhz"], peaks["source"], lane_rate_peak, flop_per_update / inst_per_update,
+                                   inst_per_update, flop_per_update),
+                    lane_instructions_per_pair_update=inst_per_update, flops_per_pair_update=flop_per_update,
+                    direct_form=dict(note="the plain per-pair form |F_s - F_{s-tau}|^2 (4 lane-instructions, 6 flops per pair "
+                                          "update, round 1's kernel) would need this fraction of the same peak",
+                                     frac=upd_per_launch * 4.0 / lag_s_per_launch / lane_rate_peak),
                     pair_updates_per_s=upd_per_launch / lag_s_per_launch, ms_per_launch=lag_s_per_launch * 1e3,
                     ms_per_step=lag_ms / args.steps, launches_per_step=lag_n / args.steps,
+                    tile_px=plan["tile_px"], task_slots=plan["slots"], lag_groups=len(plan["groups"]),
                     hbm=dict(algorithmic_gb_per_step=lag_bytes / 1e9, achieved_gbs=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9,
                              peak_gbs=peaks["hbm_gbs"], frac=lag_bytes / (lag_ms * 1e-3 / args.steps) / 1e9 / peaks["hbm_gbs"],
                              note="of measured copy peak; HBM is not the binding roofline for dense lags (DESIGN.md §7.2)"))
     if world == 1 and not args.no_hbm_regime and not args.batch:
-        roofline["hbm_bound_regime"] = run_hbm_regime(torch, binding, stack, cfg, P, peaks)
+        roofline["hbm_bound_regime"] = run_hbm_regime(torch, binding, stack, cfg, P, peaks, inst_per_update)
     fft_ms = ktimes["fft"][0]
     fft_bytes = (2.0 * cfg.W * cfg.H + 24.0 * P) * cfg.N      # one round trip between the passes
     fft_bytes_min = (2.0 * cfg.W * cfg.H + 8.0 * P) * cfg.N   # intermediate kept in L2 (what k_fft does)
     fft_s = fft_ms / args.steps * 1e-3
-    fft = dict(bound="hbm", kernel="k_fft", ms_per_step=fft_ms / args.steps, algorithmic_gb_per_step=fft_bytes / 1e9,
-               achieved_gbs=fft_bytes / fft_s / 1e9, peak_gbs=peaks["hbm_gbs"], frac=fft_bytes / fft_s / 1e9 / peaks["hbm_gbs"],
-               l2_resident_gb_per_step=fft_bytes_min / 1e9, l2_resident_frac=fft_bytes_min / fft_s / 1e9 / peaks["hbm_gbs"],
+    fft = dict(bound="hbm", kernel="k_fft", ms_per_step=fft_ms / args.steps, algorithmic_gb_per_step=fft_bytes_min / 1e9,
+               achieved_gbs=fft_bytes_min / fft_s / 1e9, peak_gbs=peaks["hbm_gbs"], frac=fft_bytes_min / fft_s / 1e9 / peaks["hbm_gbs"],
+               bytes_note="2WH + 8P bytes per frame: the uint16 frame in, the Fourier frame out; the row-pass intermediate "
+                          "stays in L2",
+               round_trip_gb_per_step=fft_bytes / 1e9, round_trip_frac=fft_bytes / fft_s / 1e9 / peaks["hbm_gbs"],
+               round_trip_note="SURVEY.md 8(d)'s figure with one HBM round trip between the passes (2WH + 24P)",
                us_per_frame=fft_s / cfg.N * 1e6)
-    kernels = {k: dict(ms_per_step=v[0] / args.steps, launches_per_step=v[1] / args.steps) for k, v in ktimes.items()}
+    kernels = {k: dict(ms_per_step=v[0] / args.steps, launches_per_step=v[1] / args.steps) for k, v in ktimes.items()
+               if k != "unused"}
 
     # BASELINE.md holds a paper number only for the paper's own workload (512^2 x 2048, all lags): total time
     # "< 2 min" on a Tesla C2050, i.e. > 17.07 frames/s (another machine's: context, not the target)
     vs_baseline = value / (2048.0 / 120.0) if (cfg.name == "paper-fig3" and world == 1) else None
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        v, dt, desc, cores = oracle_sample(cfg, lambda n: stack[:n].cpu().numpy())
-        cpu = dict(value=v, unit="frames/s", cores=cores, kind="oracle", sample=desc, seconds=dt)
+        v, dt, desc, cores, extra = oracle_sample(cfg, lambda n: stack[:n].cpu().numpy())
+        cpu = dict(value=v, unit="frames/s", cores=cores, kind="oracle", sample=desc, seconds=dt, **extra)
 
     out = dict(metric="frames_per_s", value=value, unit="frames/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
                ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=vs_baseline, dtype="f32", data="synthetic",
@@ -337,14 +419,15 @@ def run_ours(args, cfg):
                    parallelism="replicas x%d" % world, internal_batch=B,
                    l2_policy="inputs larger than L2 (%.2f GB stack streamed from HBM every step)" % (stack.numel() * 2 / 1e9)),
                frame_pairs_per_s=world * pairs / (ms_step * 1e-3), pair_updates_per_s=world * updates / (ms_step * 1e-3),
-               wall_s_per_step=t_wall / args.steps, gpu_launches=n_launch, clocks=clocks, e2e=e2e, roofline=roofline,
+               wall_s_per_step=t_wall / args.steps, ms_per_step_with_kernel_events=ms_step_profiled, gpu_launches=n_launch,
+               clocks=clocks, e2e=e2e, roofline=roofline,
                fft=fft, kernels=kernels, cpu_baseline=cpu)
     print(json.dumps(out), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 
 
-def run_hbm_regime(torch, binding, stack, cfg, P, peaks):
+def run_hbm_regime(torch, binding, stack, cfg, P, peaks, inst_per_update):
     """The same lag kernel where HBM is its binding roofline (BASELINE.json metric: "lag-accumulation HBM GB/s"):
     batches of one 26-step chunk, so that every launch re-reads the whole lag window and touches the fp64 totals
     once per 26 frames.  Algorithmic bytes per launch = P (8 (b + Lmax) + 16 n_lags); time = CUDA
@@ -367,7 +450,7 @@ def run_hbm_regime(torch, binding, stack, cfg, P, peaks):
     ach = alg / (ms / steps * 1e-3) / 1e9
     return dict(internal_batch=B, launches_per_step=n / steps, ms_per_step=ms / steps, algorithmic_gb_per_step=alg / 1e9,
                 achieved_gbs=ach, peak_gbs=peaks["hbm_gbs"], frac=ach / peaks["hbm_gbs"],
-                alu_floor_ms=(sum(max(0, cfg.N - t) for t in cfg.lags) * P * 4.0) / (SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6) * 1e3,
+                alu_floor_ms=(sum(max(0, cfg.N - t) for t in cfg.lags) * P * inst_per_update) / (SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6) * 1e3,
                 note="same kernel and stack, batches of 26 frames: algorithmic HBM time exceeds the ALU floor, HBM is the bound")
 
 
@@ -415,10 +498,9 @@ def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
         D, I, cnt = step()
     torch.cuda.synchronize()
     dt = (time.time() - t) / steps
-    if dist is not None:
-        tt = torch.tensor([dt], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
+    from paper_1209_3362_b200 import replicas
+
+    dt = replicas.max_over_ranks(dt, dist, dev)
     del host
     return dict(value=world * cfg.N / dt, unit="frames/s", h2d_bytes_per_step=int(stack.numel() * 2),
                 d2h_bytes_per_step=int(D.nbytes + I.nbytes + 4), ms_per_step=dt * 1e3, chunk_frames=chunk,
