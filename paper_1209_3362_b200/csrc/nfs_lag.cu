@@ -168,7 +168,7 @@ __device__ __forceinline__ unsigned load_chunk(const CUtensorMap* tmap, const fl
 // chunk's kChunk OLD rows are contiguous (the ring's slot 0 is duplicated behind its last slot).
 template <int CNT, int TPX>
 __device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid, const f2x* newc,
-                                            const f2x* oldl, int& o0, int DEPTH, int doI, f2x& i2, f2x& i1) {
+                                            const f2x* oldl, int& o0, int DEPTH) {
   if (!wvalid) {  // (re)build the window: the increments of the CNT-2 OLD frames that precede the chunk's first one
     int r = o0 - (CNT - 1);
     if (r < 0) r += DEPTH;
@@ -197,8 +197,6 @@ __device__ __forceinline__ void dense_chunk(f2x (&acc)[kG], f2x (&w)[kG], f2x& z
     upd2(acc[0], zn, zo);
 #pragma unroll
     for (int g = 1; g < CNT; ++g) acc[g] = fma2(zn, w[(u - (g - 1) + kChunk) % kG], acc[g]);
-    if (doI & 1) i2 = fma2(zn, zn, i2);  // the I sums ride on the frame already in registers (warp-uniform flags)
-    if (doI & 2) i1 = add2(i1, zn);
     zn = zn1;
     zo = zo1;
   }
@@ -241,15 +239,14 @@ __device__ __forceinline__ void dense_block_partial(int ns, f2x (&acc)[kG], f2x 
 // warp-uniform dispatch on the number of lags: the plan makes runs of kDenseMin..kG lags, mostly of kG and kG - 1
 template <int TPX, int CNT = kG>
 __device__ __forceinline__ void dense_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], f2x& zprev, bool& wvalid,
-                                                     const f2x* newc, const f2x* oldl, int& o0, int DEPTH, int doI, f2x& i2,
-                                                     f2x& i1) {
+                                                     const f2x* newc, const f2x* oldl, int& o0, int DEPTH) {
   if constexpr (CNT <= kDenseMin) {
-    dense_chunk<kDenseMin, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+    dense_chunk<kDenseMin, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
   } else {
     if (cnt == CNT)
-      dense_chunk<CNT, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+      dense_chunk<CNT, TPX>(acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
     else
-      dense_chunk_dispatch<TPX, CNT - 1>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+      dense_chunk_dispatch<TPX, CNT - 1>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
   }
 }
 template <int TPX, int CNT = kG>
@@ -267,8 +264,7 @@ __device__ __forceinline__ void dense_partial_dispatch(int cnt, int ns, f2x (&ac
 // ---- lag-list task with exactly CNT lags, whole chunk: the low word of w[i] holds the OLD row of lag i; its
 // kChunk rows are contiguous (duplicated slot 0) ----
 template <int CNT, int TPX>
-__device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH,
-                                             int doI, f2x& i2, f2x& i1) {
+__device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl, int DEPTH) {
   const f2x* ol[CNT];
 #pragma unroll
   for (int i = 0; i < CNT; ++i) ol[i] = oldl + (size_t)(unsigned)w[i] * TPX;
@@ -277,8 +273,6 @@ __device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const
     const f2x zn = newc[(size_t)u * TPX];
 #pragma unroll
     for (int i = 0; i < CNT; ++i) upd2(acc[i], zn, ol[i][(size_t)u * TPX]);
-    if (doI & 1) i2 = fma2(zn, zn, i2);
-    if (doI & 2) i1 = add2(i1, zn);
   }
 #pragma unroll
   for (int i = 0; i < CNT; ++i) {
@@ -289,22 +283,36 @@ __device__ __forceinline__ void sparse_chunk(f2x (&acc)[kG], f2x (&w)[kG], const
 }
 template <int TPX>
 __device__ __forceinline__ void sparse_chunk_dispatch(int cnt, f2x (&acc)[kG], f2x (&w)[kG], const f2x* newc, const f2x* oldl,
-                                                      int DEPTH, int doI, f2x& i2, f2x& i1) {
+                                                      int DEPTH) {
   switch (cnt) {
-    case 0:  // a task that only accumulates the I sums
+    case 0: break;  // a task that only accumulates the I sums
+    case 1: sparse_chunk<1, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 2: sparse_chunk<2, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 3: sparse_chunk<3, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 4: sparse_chunk<4, TPX>(acc, w, newc, oldl, DEPTH); break;
+    case 5: sparse_chunk<5, TPX>(acc, w, newc, oldl, DEPTH); break;
+    default: sparse_chunk<kSparseMax, TPX>(acc, w, newc, oldl, DEPTH); break;  // lag lists of <= kSparseMax
+  }
+}
+
+// the I sums of one chunk (sum |F'_s|^2, sum F'_s over the batch's frames): ns <= kChunk steps of the NEW rows,
+// re-read from shared memory by the one warp of the group that carries them (outside the lag loops)
+template <int TPX>
+__device__ __forceinline__ void accumulate_I(const f2x* newc, int ns, int doI, f2x& i2, f2x& i1) {
+  if (ns == kChunk) {
 #pragma unroll
-      for (int u = 0; u < kChunk; ++u) {
-        const f2x zn = newc[(size_t)u * TPX];
-        i2 = fma2(zn, zn, i2);
-        i1 = add2(i1, zn);
-      }
-      break;
-    case 1: sparse_chunk<1, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
-    case 2: sparse_chunk<2, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
-    case 3: sparse_chunk<3, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
-    case 4: sparse_chunk<4, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
-    case 5: sparse_chunk<5, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;
-    default: sparse_chunk<kSparseMax, TPX>(acc, w, newc, oldl, DEPTH, doI, i2, i1); break;  // lag lists of <= kSparseMax
+    for (int u = 0; u < kChunk; ++u) {
+      const f2x zn = newc[(size_t)u * TPX];
+      if (doI & 1) i2 = fma2(zn, zn, i2);
+      if (doI & 2) i1 = add2(i1, zn);
+    }
+  } else {
+#pragma unroll 1
+    for (int u = 0; u < ns; ++u) {
+      const f2x zn = newc[(size_t)u * TPX];
+      if (doI & 1) i2 = fma2(zn, zn, i2);
+      if (doI & 2) i1 = add2(i1, zn);
+    }
   }
 }
 
@@ -577,6 +585,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
     const f2x* newc = (single ? OLD + (size_t)nslot * kChunk * TPX : NEW + (size_t)st * kChunk * TPX) + sub * 32 + lane;
     if (++nslot == NSLOT) nslot = 0;
     const int j0 = c * kChunk;
+    if (doI) accumulate_I<TPX>(newc, min(kChunk, b - j0), doI, i2, i1);
     if (j0 >= j_all && j0 + kChunk <= b) {
       // ---- fast chunk: every pair of every step exists ----
       if (dense) {
@@ -597,10 +606,10 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
             }
           }
         }
-        dense_chunk_dispatch<TPX>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH, doI, i2, i1);
+        dense_chunk_dispatch<TPX>(cnt, acc, w, zprev, wvalid, newc, oldl, o0, DEPTH);
         oend = o0;
       } else {
-        sparse_chunk_dispatch<TPX>(cnt, acc, w, newc, oldl, DEPTH, doI, i2, i1);
+        sparse_chunk_dispatch<TPX>(cnt, acc, w, newc, oldl, DEPTH);
       }
     } else {
 #pragma unroll 1
@@ -609,16 +618,6 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
       const int ns = min(G, b - jb);        // steps of this block inside the batch
       if (ns <= 0) break;
       const f2x* nb = newc + (size_t)blk * G * TPX;
-      if (doI) {
-#pragma unroll
-        for (int u = 0; u < G; ++u) {
-          if (u < ns) {
-            const f2x zn = nb[(size_t)u * TPX];
-            if (doI & 1) i2 = fma2(zn, zn, i2);
-            if (doI & 2) i1 = add2(i1, zn);
-          }
-        }
-      }
       if (jb + ns <= j_any) {
         // no pair of this task yet
       } else if (dense && jb >= j_all) {
@@ -730,7 +729,8 @@ struct Atom {
 // issue slots per time step: a run costs 2 loads, the increment, the direct update (2) and one FMA per further lag;
 // a lag list one load and two packed operations per lag plus the load of the new frame
 double task_cost(const LagTask& t) {
-  return ((t.kind & 1) == 0 ? 4.0 + t.cnt : 3.0 * t.cnt + 1.0) + ((t.kind & 2) ? 1.0 : 0.0) + ((t.kind & 4) ? 1.0 : 0.0);
+  const double lag_cost = t.cnt == 0 ? 0.0 : ((t.kind & 1) == 0 ? 4.0 + t.cnt : 3.0 * t.cnt + 1.0);
+  return lag_cost + ((t.kind & 6) ? 1.0 : 0.0) + ((t.kind & 2) ? 1.0 : 0.0) + ((t.kind & 4) ? 1.0 : 0.0);
 }
 
 void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, size_t a0, size_t a1, bool with_I, int slots,
@@ -784,12 +784,22 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
     if (g.ntasks < slots) {
       tasks.push_back(LagTask{0, 0, 0, 1 | 2 | 4});
       g.ntasks += 1;
-    } else {  // sum |F'|^2 (bit 1) and sum F' (bit 2) ride on the two lightest tasks: one packed operation per step each
-      for (int bit = 2; bit <= 4; bit *= 2) {
-        int best = 0;
-        for (int k = 1; k < g.ntasks; ++k)
-          if (task_cost(tasks[g.task0 + k]) < task_cost(tasks[g.task0 + best])) best = k;
-        tasks[g.task0 + best].kind |= bit;
+    } else {
+      // sum |F'|^2 (bit 1) and sum F' (bit 2) ride on the lightest task (the last one among equals): it re-reads the
+      // chunk's NEW rows, three issue slots per step.  If that task is part of a run of consecutive lags it hands up
+      // to three lags to the tasks before it in the run that have room, so that it stays no heavier than they are.
+      int best = 0;
+      for (int k = 1; k < g.ntasks; ++k)
+        if (task_cost(tasks[g.task0 + k]) <= task_cost(tasks[g.task0 + best])) best = k;
+      LagTask* T = &tasks[g.task0];
+      T[best].kind |= 6;
+      for (int moved = 0; moved < 3 && (T[best].kind & 1) == 0 && T[best].cnt > kDenseMin; ++moved) {
+        int k = best;  // nearest earlier task of the same run with room
+        while (k > 0 && (T[k - 1].kind & 1) == 0 && T[k - 1].tau0 + T[k - 1].cnt == T[k].tau0 && T[k - 1].cnt >= kG) --k;
+        if (k == 0 || (T[k - 1].kind & 1) != 0 || T[k - 1].tau0 + T[k - 1].cnt != T[k].tau0) break;
+        T[k - 1].cnt += 1;  // it takes the first lag of task k; every task from k to best - 1 shifts up by one lag
+        for (int q = k; q < best; ++q) T[q].tau0 += 1, T[q].l0 += 1;
+        T[best].tau0 += 1, T[best].l0 += 1, T[best].cnt -= 1;
       }
     }
   }
