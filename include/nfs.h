@@ -67,7 +67,7 @@ typedef enum nfs_status {
  * 128 while the ring would take more than a third of the free device memory): pushed frames are
  * transformed into the ring at once, their frame pairs are accumulated whenever `batch` frames are
  * pending (and at every finalize/getter).  Ring capacity is Lmax + batch frames of H*(W/2+1) complex64.
- * Whatever the batch, fp32 partial sums never span more than 520 frames before they are folded into
+ * Whatever the batch, fp32 partial sums never span more than 1040 frames before they are folded into
  * the fp64 totals.
  * nfs_create_opts additionally takes flags:
  *   NFS_FLAG_BIN_ONLY   keep only the |q|-binned sums of the difference spectra ("store the

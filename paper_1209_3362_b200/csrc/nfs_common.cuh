@@ -25,7 +25,7 @@ constexpr int kTaskSlots = 8;     // lag tasks per group (16 for long-window pla
 constexpr int kChunk = 2 * kG;    // time steps per shared-memory pipeline stage (multiple of kG, <= 32)
 constexpr int kMinStages = 2;
 constexpr int kMaxStages = 8;     // pipeline depth is chosen at create from the shared memory left
-constexpr int kFoldChunks = 20;   // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (520) steps
+constexpr int kFoldChunks = 40;   // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (1040) steps
 constexpr int kSparseMax = 6;     // lags per lag-list task (one LDS.64 per pair update, exact-count code paths)
 constexpr int kDenseMin = 2;      // runs of >= kDenseMin consecutive lags use the register-window path
 

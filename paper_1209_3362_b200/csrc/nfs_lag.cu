@@ -373,7 +373,7 @@ __device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* o
 }
 
 template <int NCW, int SLOTS, bool PERS, bool SKIP>
-__global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
+__global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
     k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P,
                 int64_t t0_batch, int b_batch, int gbase, int ngroups, int lbase, int stages,
                 const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups, const int32_t* __restrict__ lags,
@@ -382,7 +382,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
   constexpr int G = kG;
   constexpr int TPX = 32 * (NCW / SLOTS);  // pixels per tile: one 32-pixel sub-tile per SLOTS consumer warps
   static_assert(NCW == SLOTS || NCW == 2 * SLOTS, "SLOTS task slots x 1 or 2 sub-tiles");
-  static_assert(NCW + 1 <= 32, "at most 1024 threads");
+  static_assert(NCW + 4 <= 32, "at most 1024 threads");
   static_assert(kChunk % G == 0 && kChunk <= 32 && 2 * G - 1 <= kChunk, "a chunk is a whole number of G-step blocks, one lane per row");
   static_assert(kSparseMax == 6 && kSparseMax <= G, "sparse_chunk_dispatch lists cases 0..5 and the default");
   static_assert(SLOTS <= 16 && SLOTS % 4 == 0, "warp_task[16], whole sub-partition rounds");
@@ -443,7 +443,11 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
   }
   __syncthreads();
 
-  if (warp == NCW) {
+  // Registers: the CTA is launched with a whole warpgroup for the producer (warps NCW..NCW+3, of which only the
+  // first works), which gives its registers back (setmaxnreg.dec) so that the consumer warpgroups can grow theirs.
+  if (warp >= NCW) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 24;\n");
+    if (warp > NCW) return;
     // ------------------------------- producer -------------------------------
     const int64_t E0 = t0 - tau_lo - (int64_t)LEAD * kChunk;  // frame held by row 0 of an item's OLD chunk 0
     int st = 0, slot = 0;
@@ -499,6 +503,10 @@ __global__ void __launch_bounds__((NCW + 1) * 32, NCW <= 8 ? 2 : 1)
     }
     return;
   }
+  if constexpr (NCW <= 8)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;\n");
+  else
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 112;\n");
 
   // ------------------------------- consumers -------------------------------
   const int sub = warp / SLOTS;  // 32-pixel sub-tile of this warp
@@ -1038,7 +1046,7 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   const int ngroups = (int)c.groups.size();
   const int tpx = c.lag_tpx;
   const int ntiles = (int)((c.P + tpx - 1) / tpx);
-  const int nthreads = (c.lag_slots * (tpx / 32) + 1) * 32;
+  const int nthreads = (c.lag_slots * (tpx / 32) + 4) * 32;
   int n = 0;
   if (c.bin_only) {
     // PAPER.md:L41 ("store the entire 2D power spectra, which might be unnecessary"): one lag group per launch into
