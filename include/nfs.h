@@ -85,6 +85,37 @@ NFS_API int nfs_create_opts(nfs_ctx** out, int W, int H, const int32_t* lags, in
                             int batch_frames, unsigned flags);
 
 /*
+ * nfs_create_banded — the out-of-core schedule of PAPER.md:L33 and Fig. 2(b) (L37) for lag windows that exceed the
+ * device memory one is willing to spend: "if the number of images to be analyzed exceeds the G-RAM capacity then data
+ * has to be transferred multiple times ... data transfer can be optimized by organizing the memory as a First-In-
+ * First-Out (FIFO) queue ... N - 1 = alpha N* + beta".
+ *   ring_frames_cap   Fourier frames the device may hold (0 = no limit: identical to nfs_create_opts).  If it is
+ *                     smaller than Lmax + batch, the lags are cut into bands of N* = cap - 2 batch lags (batch =
+ *                     batch_frames, or min(1024, cap / 4) if 0).  Band 0 (lags <= N*) is accumulated while the frames
+ *                     stream through the ring, as in Fig. 2(a) ("the first triangle"); every Fourier frame is also
+ *                     copied once to pinned HOST memory owned by the library; the further bands ("diagonals") are
+ *                     swept at nfs_finalize / the getters: per band a FIFO window of N* + batch OLD frames and a
+ *                     "current image area" of `batch` NEW frames are uploaded again from that store, every frame at
+ *                     most twice per band (the paper's 2 alpha N transfers; its N_FFT = N (2 alpha - 3 + 2 / alpha)
+ *                     counts N - N* steps of two uploads for every further band, this schedule stops a band where its
+ *                     pairs end).  Frames are transformed once: what is uploaded again are Fourier frames.
+ *   max_frames        frames the host store is sized for (> 0 in band mode; pushing more returns NFS_ERR_INVALID_ARG).
+ * Requirements in band mode: the smallest requested lag <= N*; no NFS_FLAG_BIN_ONLY (NFS_ERR_UNSUPPORTED).  Results
+ * are those of nfs_create up to fp32 partial-sum rounding (other batch boundaries).  nfs_finalize stays a
+ * non-destructive snapshot: the bands are rebuilt from the store at each finalize that sees new frames, and the
+ * streaming ring is restored from the store at the next push.
+ * nfs_get_transfer_counts: out HOST [4] = {bands alpha, band width N* (0: not banded), Fourier frames uploaded
+ * host -> device so far, Fourier frames downloaded device -> host so far}.
+ * nfs_band_plan: host-only (no CUDA call), the same walk as the sweeps: out HOST [6] = {bands, N*, batch, OLD-window
+ * frames uploaded, NEW frames uploaded, kernel launches} for a stack of n_frames frames.
+ */
+NFS_API int nfs_create_banded(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                              int batch_frames, unsigned flags, int ring_frames_cap, int64_t max_frames);
+NFS_API int nfs_get_transfer_counts(const nfs_ctx* ctx, int64_t* out);
+NFS_API int nfs_band_plan(int64_t n_frames, const int32_t* lags, int n_lags, int ring_frames_cap, int batch_frames,
+                          int64_t* out);
+
+/*
  * nfs_push_frames — steps 1-4 for n more frames.
  *   d_frames  DEVICE [n][H][W] uint16, row-major, x fastest, pitch W, no padding, 16-byte aligned (the
  *             kernels read it with 128-bit loads; anything else returns NFS_ERR_INVALID_ARG).

@@ -26,6 +26,10 @@ SYMBOLS = [
     ("nfs_create", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P]),
     ("nfs_create_ex", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int]),
     ("nfs_create_opts", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int, C.c_uint]),
+    ("nfs_create_banded", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int, C.c_uint,
+                                    C.c_int, C.c_int64]),
+    ("nfs_get_transfer_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
+    ("nfs_band_plan", C.c_int, [C.c_int64, C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]),
     ("nfs_push_frames", C.c_int, [_P, _P, C.c_int]),
     ("nfs_finalize", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_get_pair_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
@@ -91,13 +95,28 @@ def _dp(a, t):
 
 
 # ---- functions with the C names -----------------------------------------------------------------------
-def nfs_create(W, H, lags, n_qbins, cuda_stream=None, batch_frames=0, flags=0):
+def nfs_create(W, H, lags, n_qbins, cuda_stream=None, batch_frames=0, flags=0, ring_frames_cap=0, max_frames=0):
     lg = np.ascontiguousarray(lags, dtype=np.int32)
     h = _P()
-    rc = load_library().nfs_create_opts(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins),
-                                        _P(cuda_stream) if cuda_stream else None, int(batch_frames), int(flags))
+    st = _P(cuda_stream) if cuda_stream else None
+    if ring_frames_cap:
+        rc = load_library().nfs_create_banded(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins), st,
+                                              int(batch_frames), int(flags), int(ring_frames_cap), int(max_frames))
+    else:
+        rc = load_library().nfs_create_opts(C.byref(h), int(W), int(H), _dp(lg, C.c_int32), int(lg.size), int(n_qbins), st,
+                                            int(batch_frames), int(flags))
     _check(rc)
     return h
+
+
+def nfs_band_plan(n_frames, lags, ring_frames_cap, batch_frames=0):
+    """Host-only walk of the out-of-core band schedule (include/nfs.h): dict(bands, band_width, batch, old_uploads,
+    new_uploads, launches)."""
+    lg = np.ascontiguousarray(lags, dtype=np.int32)
+    out = np.zeros(6, dtype=np.int64)
+    _check(load_library().nfs_band_plan(int(n_frames), _dp(lg, C.c_int32), int(lg.size), int(ring_frames_cap), int(batch_frames),
+                                        _dp(out, C.c_int64)))
+    return dict(zip(("bands", "band_width", "batch", "old_uploads", "new_uploads", "launches"), (int(v) for v in out)))
 
 
 def nfs_push_frames(handle, d_frames_ptr: int, n: int):
@@ -151,7 +170,7 @@ class NFS:
     temporary passed to push() is not recycled while the kernels still read it): include/nfs.h puts both duties on
     the caller of nfs_push_frames."""
 
-    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False):
+    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False, ring_frames_cap=0, max_frames=0):
         import torch
 
         self.lib = load_library()
@@ -162,7 +181,12 @@ class NFS:
             stream = torch.cuda.Stream()
         self._stream = stream  # without a device nfs_create itself reports NFS_ERR_CUDA: no fallback
         self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None, batch_frames,
-                                 NFS_FLAG_BIN_ONLY if bin_only else 0)
+                                 NFS_FLAG_BIN_ONLY if bin_only else 0, ring_frames_cap, max_frames)
+
+    def transfer_counts(self):
+        out = np.zeros(4, dtype=np.int64)
+        _check(self.lib.nfs_get_transfer_counts(self.handle, _dp(out, C.c_int64)), self.handle)
+        return dict(zip(("bands", "band_width", "h2d_frames", "d2h_frames"), (int(v) for v in out)))
 
     @property
     def stream(self):

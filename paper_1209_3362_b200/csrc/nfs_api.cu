@@ -146,6 +146,8 @@ void free_all(Ctx& c) {
                   c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim};
   for (void* p : ptrs)
     if (p) cudaFree(p);
+  if (c.h_store) cudaFreeHost(c.h_store);
+  c.h_store = nullptr;
   for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
   c.ev_pool.clear();
   if (c.own_stream && c.stream) cudaStreamDestroy(c.stream);
@@ -164,6 +166,9 @@ bool zero_state(Ctx& c) {
   c.n_frames = 0;
   c.n_acc = 0;
   c.n_launches = 0;
+  c.swept_frames = -1;
+  c.ring_dirty = false;
+  c.h2d_frames = c.d2h_frames = 0;
   return ok;
 }
 
@@ -193,6 +198,83 @@ void ring_to_plane(const Ctx& c, const double* src, double* out) {
     for (int x = 0; x <= n; ++x) out[(size_t)y * (n + 1) + x] = src[(size_t)x * H + y];
 }
 
+// ---- out-of-core band schedule (Fig. 2(b) L37) ----------------------------------------------------
+// Memory plan for a device that holds only `cap` Fourier frames: batch b, band width N* = cap - 2 b (a window of
+// N* + b OLD frames and b NEW frames).  Returns false if no band fits.
+bool band_memory_plan(int cap, int batch_frames, int* b_out, int* nstar_out) {
+  int b = batch_frames > 0 ? batch_frames : std::min(1024, cap / 4);
+  b = std::max(1, std::min(b, 8192));
+  const int nstar = cap - 2 * b;
+  if (nstar < 1) return false;
+  *b_out = b;
+  *nstar_out = nstar;
+  return true;
+}
+
+// The sweeps of bands 1 .. n_bands-1 over a stack of N frames, as a sequence of uploads and launches.  Band k holds
+// the requested lags in (k N*, (k+1) N*], smallest tmin, largest tmax.  Its sweep walks the frames s = tmin .. N-1 in
+// batches of b: the batch goes into the NEW ring, the OLD frames s - tmax .. s - tmin it pairs with are kept in the
+// OLD ring, every frame of the window being uploaded once per band (the paper's FIFO: "one diagonal is filled by
+// subsequently replacing one FIFO image and uploading one 'current image'").  The same walk serves the device (uploads
+// and kernel launches) and the host-only transfer count of nfs_band_plan.
+template <typename UploadOld, typename UploadNew, typename Launch>
+bool band_sweeps(int64_t N, int b, int n_bands, const std::vector<int>& band_l0, const std::vector<int32_t>& lags,
+                 UploadOld&& upload_old, UploadNew&& upload_new, Launch&& launch) {
+  for (int k = 1; k < n_bands; ++k) {
+    const int l0 = band_l0[(size_t)k], l1 = band_l0[(size_t)k + 1];
+    if (l1 <= l0) continue;  // no requested lag in this band
+    const int64_t tmin = lags[(size_t)l0], tmax = lags[(size_t)l1 - 1];
+    int64_t old_next = -1;  // first OLD frame not yet in the OLD ring
+    for (int64_t t0 = tmin; t0 < N; t0 += b) {
+      const int bb = (int)std::min<int64_t>(b, N - t0);
+      const int64_t lo = std::max<int64_t>(0, t0 - tmax), hi = t0 + bb - 1 - tmin;  // OLD frames lo .. hi
+      const int64_t from = std::max(lo, old_next);
+      if (hi >= from && !upload_old(from, hi + 1)) return false;
+      old_next = std::max(old_next, hi + 1);
+      if (!upload_new(t0, t0 + bb)) return false;
+      if (!launch(t0, bb, k)) return false;
+    }
+  }
+  return true;
+}
+
+// frames [f0, f1) between a ring of `slots` frames at `base` (slot = frame mod slots) and the pinned host store
+bool copy_frames(Ctx& c, float2* base, int slots, int64_t f0, int64_t f1, bool to_device) {
+  while (f0 < f1) {
+    const int64_t s0 = f0 % slots;
+    const int64_t n = std::min<int64_t>(f1 - f0, slots - s0);
+    float2* dev = base + (size_t)s0 * c.P;
+    float2* host = c.h_store + (size_t)f0 * c.P;
+    const size_t bytes = sizeof(float2) * (size_t)n * c.P;
+    if (!NFS_CUDA(c, to_device ? cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, c.stream)
+                               : cudaMemcpyAsync(host, dev, bytes, cudaMemcpyDeviceToHost, c.stream)))
+      return false;
+    (to_device ? c.h2d_frames : c.d2h_frames) += n;
+    f0 += n;
+  }
+  return true;
+}
+
+// bring the totals of bands >= 1 up to date with the frames pushed so far (idempotent: they are rebuilt from zero)
+bool run_band_sweeps(Ctx& c) {
+  if (c.band_width <= 0 || c.n_bands <= 1 || c.swept_frames == c.n_frames) return true;
+  const int l_first = c.band_l0[1];
+  if (l_first < c.n_lags &&
+      !NFS_CUDA(c, cudaMemsetAsync(c.totals + (size_t)l_first * c.P, 0, sizeof(double) * (size_t)(c.n_lags - l_first) * c.P, c.stream)))
+    return false;
+  c.ring_dirty = true;
+  const bool ok = band_sweeps(
+      c.n_frames, c.B, c.n_bands, c.band_l0, c.lags,
+      [&](int64_t f0, int64_t f1) { return copy_frames(c, c.ring, c.R, f0, f1, true); },
+      [&](int64_t f0, int64_t f1) { return copy_frames(c, c.ringN, c.RN, f0, f1, true); },
+      [&](int64_t t0, int bb, int band) {
+        c.n_launches += launch_lag_tiled(c, t0, bb, band);
+        return NFS_CUDA(c, cudaGetLastError()) && c.status == NFS_OK;
+      });
+  if (ok) c.swept_frames = c.n_frames;
+  return ok;
+}
+
 // step S5 (+ the I accumulators) for the frames transformed since the last accumulation
 bool flush_pending(Ctx& c) {
   const int b = (int)(c.n_frames - c.n_acc);
@@ -212,7 +294,7 @@ bool lags_ok(const int32_t* lags, int n_lags) {
 }
 
 int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream, int batch_frames,
-                unsigned flags) {
+                unsigned flags, int ring_frames_cap = 0, int64_t max_frames = 0) {
   if (!out) return NFS_ERR_INVALID_ARG;
   *out = nullptr;
   if (!lags_ok(lags, n_lags) || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
@@ -236,6 +318,26 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   c.B = batch_frames > 0 ? batch_frames : 1024;
   c.R = c.Lmax + c.B;
   c.bin_only = (flags & NFS_FLAG_BIN_ONLY) != 0;
+  // band schedule: asked for by a ring capacity that cannot hold the whole lag window plus a batch
+  if (ring_frames_cap < 0 || max_frames < 0) {
+    delete h;
+    return NFS_ERR_INVALID_ARG;
+  }
+  if (ring_frames_cap > 0 && ring_frames_cap < c.Lmax + (batch_frames > 0 ? batch_frames : 1)) {
+    int b = 0, nstar = 0;
+    if (c.bin_only || max_frames < 1 || !band_memory_plan(ring_frames_cap, batch_frames, &b, &nstar) || lags[0] > nstar) {
+      delete h;
+      return c.bin_only ? NFS_ERR_UNSUPPORTED : NFS_ERR_INVALID_ARG;
+    }
+    c.B = b;
+    c.band_width = nstar;
+    c.R = nstar + b;  // the FIFO of the paper: the OLD window of one band plus a batch
+    c.RN = b;         // the "current image area"
+    c.max_frames = max_frames;
+  } else if (ring_frames_cap > 0 && batch_frames == 0) {
+    c.B = std::max(1, std::min(1024, ring_frames_cap - c.Lmax));
+    c.R = c.Lmax + c.B;
+  }
 
   bool ok = NFS_CUDA(c, cudaGetDevice(&c.device));
   int smem_sm = 0;
@@ -259,11 +361,11 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
     size_t free_b = 0, total_b = 0;
     ok = NFS_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     // default batch: 1024 frames, halved (down to 128) while the ring would take more than a third of the free memory
-    while (ok && batch_frames == 0 && c.B > 128 && (double)c.R * (double)c.P * 8.0 > (double)free_b / 3.0) {
+    while (ok && batch_frames == 0 && ring_frames_cap == 0 && c.B > 128 && (double)c.R * (double)c.P * 8.0 > (double)free_b / 3.0) {
       c.B /= 2;
       c.R = c.Lmax + c.B;
     }
-    const double need = (double)c.P * ((double)c.R * 8 + 8 + (double)totals_rows(c) * 8 + 8 + 16 + 8) +
+    const double need = (double)c.P * ((double)(c.R + c.RN) * 8 + 8 + (double)totals_rows(c) * 8 + 8 + 16 + 8) +
                         (double)fft_rowT_elems(c) * 8 + (double)W * H * 4 + (double)(2 * n_lags + 2) * n_qbins * 8 +
                         (64 << 20);
     if (ok && need > (double)free_b) {
@@ -271,7 +373,17 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
       ok = false;
     }
   }
-  ok = ok && dev_alloc(c, &c.ring, (size_t)c.R * c.P);
+  ok = ok && dev_alloc(c, &c.ring, (size_t)(c.R + c.RN) * c.P);
+  if (ok && c.band_width > 0) {
+    c.ringN = c.ring + (size_t)c.R * c.P;
+    void* hp = nullptr;
+    if (cudaHostAlloc(&hp, sizeof(float2) * (size_t)c.max_frames * c.P, cudaHostAllocDefault) != cudaSuccess) {
+      cudaGetLastError();
+      c.status = NFS_ERR_OOM;  // the pinned host store of the Fourier frames does not fit
+      ok = false;
+    }
+    c.h_store = reinterpret_cast<float2*>(hp);
+  }
   ok = ok && lag_configure(c);
   ok = ok && fft_configure(c);
   ok = ok && dev_alloc(c, &c.rowbuf, fft_rowT_elems(c));
@@ -287,7 +399,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   ok = ok && dev_alloc(c, &c.d_tmp, (size_t)c.P);
   ok = ok && dev_alloc(c, &c.d_flags, 1);
   ok = ok && build_tables(c);
-  ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)c.R * c.P, c.stream));
+  ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)(c.R + c.RN) * c.P, c.stream));
   ok = ok && zero_state(c);
   ok = ok && NFS_CUDA(c, cudaStreamSynchronize(c.stream));
   if (ok) {
@@ -318,6 +430,7 @@ int ready(nfs_ctx* h) {
   if (!enter(c)) return c.status;
   if (c.n_frames < 1) return NFS_ERR_STATE;
   if (!flush_pending(c)) return c.status;
+  if (!run_band_sweeps(c)) return c.status;
   return NFS_OK;
 }
 
@@ -340,6 +453,41 @@ int nfs_create_opts(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags
   NFS_GUARDED(create_impl(out, W, H, lags, n_lags, n_qbins, cuda_stream, batch_frames, flags))
 }
 
+int nfs_create_banded(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
+                      int batch_frames, unsigned flags, int ring_frames_cap, int64_t max_frames) {
+  NFS_GUARDED(create_impl(out, W, H, lags, n_lags, n_qbins, cuda_stream, batch_frames, flags, ring_frames_cap, max_frames))
+}
+
+int nfs_get_transfer_counts(const nfs_ctx* h, int64_t* out) {
+  if (!h || !out) return NFS_ERR_INVALID_ARG;
+  const Ctx& c = h->c;
+  out[0] = c.band_width > 0 ? c.n_bands : 1;
+  out[1] = c.band_width;
+  out[2] = c.h2d_frames;
+  out[3] = c.d2h_frames;
+  return NFS_OK;
+}
+
+static int band_plan_impl(int64_t n_frames, const int32_t* lags, int n_lags, int ring_frames_cap, int batch_frames, int64_t* out) {
+  if (!lags_ok(lags, n_lags) || !out || n_frames < 1 || ring_frames_cap < 1) return NFS_ERR_INVALID_ARG;
+  int b = 0, nstar = 0;
+  if (!band_memory_plan(ring_frames_cap, batch_frames, &b, &nstar) || lags[0] > nstar) return NFS_ERR_INVALID_ARG;
+  const int n_bands = (lags[n_lags - 1] - 1) / nstar + 1;
+  std::vector<int32_t> L(lags, lags + n_lags);
+  std::vector<int> l0((size_t)n_bands + 1, n_lags);
+  for (int l = n_lags - 1; l >= 0; --l)
+    for (int k = 0; k <= (L[(size_t)l] - 1) / nstar; ++k) l0[(size_t)k] = l;
+  int64_t up_old = 0, up_new = 0, launches = 0;
+  band_sweeps(
+      n_frames, b, n_bands, l0, L, [&](int64_t f0, int64_t f1) { up_old += f1 - f0; return true; },
+      [&](int64_t f0, int64_t f1) { up_new += f1 - f0; return true; }, [&](int64_t, int, int) { ++launches; return true; });
+  out[0] = n_bands, out[1] = nstar, out[2] = b, out[3] = up_old, out[4] = up_new, out[5] = launches;
+  return NFS_OK;
+}
+int nfs_band_plan(int64_t n_frames, const int32_t* lags, int n_lags, int ring_frames_cap, int batch_frames, int64_t* out) {
+  NFS_GUARDED(band_plan_impl(n_frames, lags, n_lags, ring_frames_cap, batch_frames, out))
+}
+
 int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
                   int batch_frames) {
   return nfs_create_opts(out, W, H, lags, n_lags, n_qbins, cuda_stream, batch_frames, 0u);
@@ -355,6 +503,13 @@ static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n) {
   Ctx& c = h->c;
   if (!enter(c)) return c.status;
   const int64_t fpx = (int64_t)c.W * c.H;
+  if (c.band_width > 0) {
+    if (c.n_frames + n > c.max_frames) return NFS_ERR_INVALID_ARG;  // the host store was sized for max_frames
+    if (c.ring_dirty) {  // sweeps of an earlier finalize overwrote the streaming ring: bring its newest frames back
+      if (!copy_frames(c, c.ring, c.R, std::max<int64_t>(0, c.n_frames - c.R), c.n_frames, true)) return c.status;
+      c.ring_dirty = false;
+    }
+  }
   int done = 0;
   while (done < n) {
     // transform as many frames as the ring has room for; accumulate whenever a full batch is pending
@@ -364,6 +519,8 @@ static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n) {
     if (c.n_frames == 0) c.n_launches += launch_make_ref(c, fr);
     c.n_launches += launch_fft_frames(c, fr, b, c.n_frames);
     if (c.status != NFS_OK) return c.status;
+    // band schedule: every Fourier frame also goes to the pinned host store, once
+    if (c.band_width > 0 && !copy_frames(c, c.ring, c.R, c.n_frames, c.n_frames + b, false)) return c.status;
     c.n_frames += b;
     done += b;
     if (c.n_frames - c.n_acc == c.B && !flush_pending(c)) return c.status;

@@ -58,6 +58,24 @@ struct Ctx {
   int device = 0;
   int n_sm = 0;
   bool bin_only = false;  // accumulate |q|-binned totals only (no 2-D spectra kept)
+  // Out-of-core band schedule (Fig. 2(b) L37): the device holds only `ring cap` Fourier frames, fewer
+  // than Lmax + batch.  The lags are cut into bands of band_width = N* lags (the paper's FIFO length); band 0 is
+  // accumulated while the frames stream through the ring (the "first triangle" and its diagonal), every Fourier frame
+  // is also kept in pinned host memory, and the further bands are swept at finalize: per band a window of N* + batch
+  // OLD frames (the FIFO, in `ring`) and a batch of NEW frames (the "current image area", in `ringN`) are uploaded
+  // again from the host store.
+  int band_width = 0;           // N*; 0: everything fits (Fig. 2(a)), no host store
+  int n_bands = 1;
+  int RN = 0;                   // slots of ringN (= batch)
+  float2* ringN = nullptr;      // ring + R * P
+  CUtensorMap ringN_map;
+  float2* h_store = nullptr;    // pinned host memory [max_frames][P]
+  int64_t max_frames = 0;
+  std::vector<int> band_g0;     // [n_bands + 1] first lag group of each band
+  std::vector<int> band_l0;     // [n_bands + 1] index of the first lag of each band
+  int64_t swept_frames = -1;    // the sweeps of bands >= 1 are up to date for this many frames
+  bool ring_dirty = false;      // the sweeps overwrote the streaming ring: restored from the host store at the next push
+  int64_t h2d_frames = 0, d2h_frames = 0;  // Fourier frames moved by the band schedule (the paper's N_FFT counts the uploads)
   std::vector<int32_t> lags;
   std::vector<int64_t> counts;  // full-plane pixel count per bin
   cudaStream_t stream = nullptr;
@@ -155,7 +173,7 @@ int launch_fft_frames(Ctx& c, const uint16_t* frames, int nf, int64_t t_first); 
 size_t fft_rowT_elems(const Ctx& c);                              // float2 elements of the row-pass buffer
 size_t fft_cnt_elems(const Ctx& c);                               // unsigned ints of the work-queue counters
 // nfs_lag.cu
-int launch_lag_tiled(Ctx& c, int64_t t0, int b);
+int launch_lag_tiled(Ctx& c, int64_t t0, int b, int band = 0);  // band > 0: a sweep of the band schedule (NEW frames from ringN)
 // host only (no CUDA call): tasks, groups, tile width, pipeline depth from the lag list, the shared memory per SM and
 // c.max_smem_optin; false if a lag group cannot fit shared memory
 bool lag_plan(Ctx& c, int smem_per_sm, int n_sm, int64_t P);

@@ -374,7 +374,8 @@ __device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* o
 
 template <int NCW, int SLOTS, bool PERS, bool SKIP>
 __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
-    k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R, int64_t P,
+    k_lag_tiled(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ ring, int R,
+                const __grid_constant__ CUtensorMap tmapN, const float2* __restrict__ ringN, int RN, int64_t P,
                 int64_t t0_batch, int b_batch, int gbase, int ngroups, int lbase, int stages,
                 const LagTask* __restrict__ tasks, const LagGroup* __restrict__ groups, const int32_t* __restrict__ lags,
                 double* __restrict__ totals, double* __restrict__ I2, double2* __restrict__ I1, int ntiles,
@@ -473,7 +474,7 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
           f2x* dup = slot == 0 ? OLD + (size_t)NSLOT * kChunk * TPX : nullptr;
           unsigned bytes = load_chunk<TPX>(&tmap, ring, R, P, p0, E0 + (int64_t)j * kChunk, dst, dup, &full[st], lane);
           if (!single && j >= LEAD)
-            bytes += load_chunk<TPX>(&tmap, ring, R, P, p0, t0 + (int64_t)(j - LEAD) * kChunk,
+            bytes += load_chunk<TPX>(&tmapN, ringN, RN, P, p0, t0 + (int64_t)(j - LEAD) * kChunk,
                                      NEW + (size_t)st * kChunk * TPX, nullptr, &full[st], lane);
           bytes = __reduce_add_sync(0xffffffffu, bytes);
           if (lane == 0) mbar_arrive_expect_tx(&full[st], bytes);
@@ -488,7 +489,7 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
         if (c >= stages) mbar_wait_relaxed(&empty[st], ph ^ 1u);
         unsigned bytes = 0;
         if (!single)
-          bytes = load_chunk<TPX>(&tmap, ring, R, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * TPX, nullptr,
+          bytes = load_chunk<TPX>(&tmapN, ringN, RN, P, p0, t0 + (int64_t)c * kChunk, NEW + (size_t)st * kChunk * TPX, nullptr,
                                   &full[st], lane);
         for (int m = (c == 0 ? 0 : c + LEAD); m <= c + LEAD; ++m) {
           f2x* dst = OLD + (size_t)slot * kChunk * TPX;
@@ -837,11 +838,14 @@ static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
   // shared memory a CTA may use: the opt-in maximum (one CTA per SM) bounds a group's window; two CTAs of 32-pixel
   // tiles share an SM when the plan's footprint allows it (1 KB per CTA is reserved, 1 KB static)
   const size_t budget = (size_t)std::max(0, std::min(smem_sm - 2048, c.max_smem_optin - 1024));
+  // band of a lag in the out-of-core schedule: lags (k N*, (k+1) N*] form band k; no task or group
+  // straddles two bands, and only band 0 streams its batch as the head of its window
+  auto band_of = [&](int tau) { return c.band_width > 0 ? (tau - 1) / c.band_width : 0; };
   // atoms
   std::vector<Atom> atoms;
   for (int i = 0; i < c.n_lags;) {
     int j = i;
-    while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1) ++j;
+    while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1 && band_of(L[j + 1]) == band_of(L[i])) ++j;
     const int len = j - i + 1;
     if (len >= kDenseMin) {
       const int nt = (len + kG - 1) / kG;
@@ -862,12 +866,13 @@ static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
   }
   // greedy groups: a group is streamed as a single window when that costs no more shared memory than two streams
   auto single_of = [&](int tmin, int tmax) {
-    return lag_smem_bytes(0, tmax, true, kMinStages, 32) <= lag_smem_bytes(tmin, tmax, false, kMinStages, 32);
+    return band_of(tmin) == 0 && lag_smem_bytes(0, tmax, true, kMinStages, 32) <= lag_smem_bytes(tmin, tmax, false, kMinStages, 32);
   };
   c.tasks.clear();
   c.groups.clear();
   auto fits = [&](size_t a0, size_t a1) {  // atoms [a0, a1) as one group
     const int tmin = L[atoms[a0].l0], tmax = L[atoms[a1 - 1].l0 + atoms[a1 - 1].cnt - 1];
+    if (band_of(tmin) != band_of(tmax)) return false;
     const bool sg = single_of(tmin, tmax);
     if (lag_smem_bytes(sg ? 0 : tmin, tmax, sg, kMinStages, 32) > budget && a1 - a0 > 1) return false;
     int need = 0;
@@ -897,13 +902,20 @@ static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
     return n;
   };
   c.max_group_lags = 0;
-  for (size_t k = 0; k < cuts.size(); ++k) {
-    if (nl(cuts[k]) < nl(cuts[gI])) gI = k;
+  for (size_t k = 0; k < cuts.size(); ++k) {  // (band schedule: among the groups of band 0, which run as the frames stream in)
+    if (band_of(L[atoms[cuts[k].first].l0]) == 0 && nl(cuts[k]) < nl(cuts[gI])) gI = k;
     c.max_group_lags = std::max(c.max_group_lags, nl(cuts[k]));
   }
   for (size_t k = 0; k < cuts.size(); ++k) close_group(L, atoms, cuts[k].first, cuts[k].second, k == gI, slots, c.tasks, c.groups);
   for (LagGroup& g : c.groups)
     if (single_of(g.tau_min, g.tau_max)) g.flags |= 2;
+  c.n_bands = band_of(L.back()) + 1;
+  c.band_g0.assign((size_t)c.n_bands + 1, (int)c.groups.size());
+  c.band_l0.assign((size_t)c.n_bands + 1, c.n_lags);
+  for (int g = (int)c.groups.size() - 1; g >= 0; --g)
+    for (int k = 0; k <= band_of(c.groups[g].tau_min); ++k) c.band_g0[(size_t)k] = g;
+  for (int l = c.n_lags - 1; l >= 0; --l)
+    for (int k = 0; k <= band_of(L[l]); ++k) c.band_l0[(size_t)k] = l;
   // tile width and pipeline depth.  64-pixel tiles (16 consumer warps, one CTA per SM, 512-byte rows) when every
   // group's window then still leaves kMinStages + 1 stages; else 32-pixel tiles, two CTAs per SM if they fit.
   auto smem_for = [&](int stages, int tpx) {
@@ -984,6 +996,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
       c.tasks = alt.tasks, c.groups = alt.groups;
       c.lag_stages = alt.lag_stages, c.lag_smem = alt.lag_smem, c.lag_tpx = alt.lag_tpx, c.lag_slots = alt.lag_slots;
       c.lag_ctas_per_sm = alt.lag_ctas_per_sm, c.lag_grid = alt.lag_grid, c.max_group_lags = alt.max_group_lags;
+      c.n_bands = alt.n_bands, c.band_g0 = alt.band_g0, c.band_l0 = alt.band_l0;
     }
   }
   return true;
@@ -993,7 +1006,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
 // launchers
 // ------------------------------------------------------------------------------------------------
 namespace {
-typedef void (*LagKernel)(const CUtensorMap, const float2*, int, int64_t, int64_t, int, int, int, int, int, const LagTask*,
+typedef void (*LagKernel)(const CUtensorMap, const float2*, int, const CUtensorMap, const float2*, int, int64_t, int64_t, int, int, int, int, int, const LagTask*,
                           const LagGroup*, const int32_t*, double*, double*, double2*, int, int*);
 template <int NCW, int SLOTS>
 LagKernel lag_kernel_of(bool pers, bool skip) {
@@ -1023,17 +1036,20 @@ bool lag_configure(Ctx& c) {
     c.cuda_err = "cuTensorMapEncodeTiled not available";
     return false;
   }
-  const cuuint64_t gdim[2] = {(cuuint64_t)(2 * c.P), (cuuint64_t)c.R};
   const cuuint64_t gstride[1] = {(cuuint64_t)c.P * sizeof(float2)};
   const cuuint32_t box[2] = {(cuuint32_t)(2 * c.lag_tpx), (cuuint32_t)kChunk};
   const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = reinterpret_cast<EncodeFn>(fn)(&c.ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c.ring, gdim, gstride, box,
-                                                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) {
-    c.status = NFS_ERR_CUDA;
-    c.cuda_err = "cuTensorMapEncodeTiled failed";
-    return false;
+  for (int which = 0; which < (c.band_width > 0 ? 2 : 1); ++which) {  // the ring; band schedule: also the NEW ring of the sweeps
+    const cuuint64_t gdim[2] = {(cuuint64_t)(2 * c.P), (cuuint64_t)(which ? c.RN : c.R)};
+    const CUresult r = reinterpret_cast<EncodeFn>(fn)(which ? &c.ringN_map : &c.ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                                                      which ? c.ringN : c.ring, gdim, gstride, box, estr,
+                                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      c.status = NFS_ERR_CUDA;
+      c.cuda_err = "cuTensorMapEncodeTiled failed";
+      return false;
+    }
   }
   for (int v = 0; v < 4; ++v)
     if (!NFS_CUDA(c, cudaFuncSetAttribute(lag_kernel(c.lag_tpx, c.lag_slots, (v & 1) != 0, (v & 2) != 0),
@@ -1042,8 +1058,17 @@ bool lag_configure(Ctx& c) {
   return true;
 }
 
-int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
-  const int ngroups = (int)c.groups.size();
+int launch_lag_tiled(Ctx& c, int64_t t0, int b, int band) {
+  // band schedule: only the groups of one band per launch; a sweep (band > 0) takes the batch's own
+  // frames from the NEW ring, the streaming pass (band 0) from the ring itself
+  const bool banded = c.band_width > 0;
+  const int g0 = banded ? c.band_g0[(size_t)band] : 0;
+  const int ngroups = banded ? c.band_g0[(size_t)band + 1] - g0 : (int)c.groups.size();
+  if (ngroups <= 0) return 0;
+  const bool sweep = banded && band > 0;
+  const CUtensorMap& mapN = sweep ? c.ringN_map : c.ring_map;
+  const float2* ringN = sweep ? c.ringN : c.ring;
+  const int RN = sweep ? c.RN : c.R;
   const int tpx = c.lag_tpx;
   const int ntiles = (int)((c.P + tpx - 1) / tpx);
   const int nthreads = (c.lag_slots * (tpx / 32) + 4) * 32;
@@ -1063,8 +1088,8 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
           ProfScope ps(c, kKLag);
           if (!NFS_CUDA(c, cudaMemsetAsync(c.totals, 0, sizeof(double) * (size_t)nl * c.P, c.stream))) return n;
           lag_kernel(tpx, c.lag_slots, false, skip)<<<(unsigned)ntiles, nthreads, c.lag_smem, c.stream>>>(
-              c.ring_map, c.ring, c.R, c.P, t0, b, g, 1, lbase, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2,
-              c.I1, ntiles, c.d_claim);
+              c.ring_map, c.ring, c.R, c.ring_map, c.ring, c.R, c.P, t0, b, g, 1, lbase, c.lag_stages, c.d_tasks, c.d_groups,
+              c.d_lags, c.totals, c.I2, c.I1, ntiles, c.d_claim);
           n += 1;
         }
         n += launch_bin_accumulate(c, lbase, nl);
@@ -1081,17 +1106,18 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b) {
   // cost is amortised anyway (measurements: profiles/).
   int max_lead = 0;
   for (const LagGroup& g : c.groups) max_lead = std::max(max_lead, lag_lead(lag_tau_lo(g), g.tau_max));
-  const bool persistent = c.lag_shape ? c.lag_shape == 2 : (b <= 2 * kChunk && ngroups <= 2 && max_lead <= c.lag_stages);
+  const bool persistent =
+      !banded && (c.lag_shape ? c.lag_shape == 2 : (b <= 2 * kChunk && ngroups <= 2 && max_lead <= c.lag_stages));
   const unsigned grid = persistent ? (unsigned)c.lag_grid : (unsigned)ntiles * (unsigned)ngroups;
   ProfScope ps(c, kKLag);
   // some group (other than the one that accumulates the I sums) has whole chunks without a pair in this batch
   bool skip = false;
-  for (const LagGroup& g : c.groups)
-    skip |= !(g.flags & 1) && (int64_t)g.tau_min - t0 >= kChunk && (int64_t)g.tau_min <= t0 + b - 1;
+  for (int g = g0; g < g0 + ngroups; ++g)
+    skip |= !(c.groups[g].flags & 1) && (int64_t)c.groups[g].tau_min - t0 >= kChunk && (int64_t)c.groups[g].tau_min <= t0 + b - 1;
   if (persistent && !NFS_CUDA(c, cudaMemsetAsync(c.d_claim, 0, sizeof(int) * (size_t)ngroups, c.stream))) return 0;
   lag_kernel(tpx, c.lag_slots, persistent, skip)<<<grid, nthreads, c.lag_smem, c.stream>>>(
-      c.ring_map, c.ring, c.R, c.P, t0, b, 0, ngroups, 0, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags, c.totals, c.I2, c.I1,
-      ntiles, c.d_claim);
+      c.ring_map, c.ring, c.R, mapN, ringN, RN, c.P, t0, b, g0, ngroups, 0, c.lag_stages, c.d_tasks, c.d_groups, c.d_lags,
+      c.totals, c.I2, c.I1, ntiles, c.d_claim);
   return 1;
 }
 
