@@ -173,7 +173,7 @@ template <int L>
 struct Plan {
   static constexpr int T = L / 32;                       // threads per FFT
   static constexpr int NT = (L == 512 || L == 1024) ? 128 : 256;  // threads per CTA
-  static constexpr int minBlocks = 512 / NT;  // CTAs per SM the kernel is compiled for (128 registers per thread)
+  static constexpr int minBlocks = L == 1024 ? 5 : 512 / NT;  // CTAs per SM the kernel is compiled for (1024: 96 registers, no spill)
   static constexpr int Fc = NT / T;                      // FFTs per CTA item
   static constexpr bool two = L > 1024;                  // two-level plan
   static constexpr int Mi = two ? L / 1024 : T;          // lanes per (inner) FFT
