@@ -257,6 +257,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-hbm-regime", action="store_true", help="skip the small-batch run of the lag kernel")
+    ap.add_argument("--sharding", default="replicas", choices=["replicas", "time"],
+                    help="N > 1: 'replicas' = every rank analyses its own stack (weak scaling, the default); 'time' = ONE "
+                         "stack cut into time chunks with halos, one NCCL all-reduce of the partial sums (strong scaling, "
+                         "SURVEY.md 8(e))")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -294,15 +298,26 @@ def run_ours(args, cfg):
 
     from paper_1209_3362_b200 import replicas
 
-    # every rank analyses its own stack (replicas; seed differs per rank)
-    stack = synth.make_stack(replicas.rank_config(cfg, rank), dev)
+    from paper_1209_3362_b200 import sharding
+
+    time_sharded = args.sharding == "time"
+    # replicas: every rank analyses its own stack (seed differs per rank); time sharding: the same stack everywhere,
+    # each rank feeds its context the halo and the own frames of its time chunk
+    stack = synth.make_stack(cfg if time_sharded else replicas.rank_config(cfg, rank), dev)
     stream = torch.cuda.Stream(device=dev)
     nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch)
     torch.cuda.synchronize()
+    shard = sharding.shard_plan(cfg.N, world, cfg.lags[-1])[rank] if time_sharded else None
+    merge_bytes = 0
 
     def step():
+        nonlocal merge_bytes
         nfs.reset()
-        nfs.push(stack)
+        if time_sharded:
+            sharding.push_shard(nfs, stack, shard)
+            merge_bytes = sharding.merge(nfs, dist)   # the path's one collective: all-reduce of the fp64 partial sums
+        else:
+            nfs.push(stack)
         return nfs.finalize()
 
     for _ in range(max(args.warmup, 1) if args.warmup else 0):
@@ -341,11 +356,11 @@ def run_ours(args, cfg):
     ktimes = nfs.kernel_times()
     nfs.set_profiling(False)
     ms_step_profiled = e2.elapsed_time(e3) / args.steps
-    value = world * cfg.N / (ms_step * 1e-3)
+    value = (1 if time_sharded else world) * cfg.N / (ms_step * 1e-3)   # time sharding: ONE stack over all ranks
 
     # ---- end to end through the C-ABI with the stack in pinned HOST memory ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not time_sharded:
         e2e = run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world)
 
     if rank != 0:
@@ -359,7 +374,7 @@ def run_ours(args, cfg):
     # comes from CUDA events recorded around every launch on the library's stream (nfs_set_profiling).
     lag_ms, lag_n = ktimes["lag_accum"]
     lag_s_per_launch = lag_ms * 1e-3 / max(lag_n, 1)
-    upd_per_launch = updates * args.steps / max(lag_n, 1)
+    upd_per_launch = updates / (world if time_sharded else 1) * args.steps / max(lag_n, 1)   # this rank's share
     inst_step, flop_step, plan = lag_algorithmic_work(cfg, binding)
     n_l = len(cfg.lags)
     inst_per_update, flop_per_update = inst_step / n_l, flop_step / n_l   # averaged over the lags of the plan
@@ -413,12 +428,15 @@ def run_ours(args, cfg):
         cpu = dict(value=v, unit="frames/s", cores=cores, kind="oracle", sample=desc, seconds=dt, **extra)
 
     out = dict(metric="frames_per_s", value=value, unit="frames/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
-               ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=vs_baseline, dtype="f32", data="synthetic",
+               ms_per_step=ms_step, higher_is_better=True, scaling="strong" if time_sharded else "weak", vs_baseline=vs_baseline,
+               dtype="f32", data="synthetic",
                config=dict(workload="%s: %dx%d uint16 x %d frames, %d lags (max %d), %d |q| bins" % (
                    cfg.name, cfg.W, cfg.H, cfg.N, len(cfg.lags), cfg.lags[-1], cfg.n_qbins),
-                   parallelism="replicas x%d" % world, internal_batch=B,
+                   parallelism=("time chunks x%d, halo %d frames, one all-reduce of %.1f MB" % (world, cfg.lags[-1], merge_bytes / 1e6))
+                   if time_sharded else "replicas x%d" % world, internal_batch=B,
                    l2_policy="inputs larger than L2 (%.2f GB stack streamed from HBM every step)" % (stack.numel() * 2 / 1e9)),
-               frame_pairs_per_s=world * pairs / (ms_step * 1e-3), pair_updates_per_s=world * updates / (ms_step * 1e-3),
+               frame_pairs_per_s=(1 if time_sharded else world) * pairs / (ms_step * 1e-3),
+               pair_updates_per_s=(1 if time_sharded else world) * updates / (ms_step * 1e-3),
                wall_s_per_step=t_wall / args.steps, ms_per_step_with_kernel_events=ms_step_profiled, gpu_launches=n_launch,
                clocks=clocks, e2e=e2e, roofline=roofline,
                fft=fft, kernels=kernels, cpu_baseline=cpu)

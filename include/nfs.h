@@ -128,6 +128,30 @@ NFS_API int nfs_band_plan(int64_t n_frames, const int32_t* lags, int n_lags, int
 NFS_API int nfs_push_frames(nfs_ctx* ctx, const uint16_t* d_frames, int n);
 
 /*
+ * Time-chunk sharding over several contexts, one per GPU (the path of PAPER.md:L31-33 is a sum over
+ * frame pairs, so it splits by the later frame of each pair).  Context g takes the frames [g N / G, (g+1) N / G) of the
+ * stack as its own and, first, the Lmax frames before them as a halo:
+ *   nfs_push_halo      d_frames DEVICE [n][H][W] as in nfs_push_frames.  Halo frames are normalised, transformed and
+ *                      kept in the ring, and are paired with the own frames that follow as the EARLIER frame of a
+ *                      pair; they are never the later frame of a pair, do not enter I(q) and are not counted.  Only
+ *                      before the first own frame, at most Lmax frames in total (NFS_ERR_STATE otherwise; not in
+ *                      band mode).  nfs_get_pair_counts then reports the pairs this context holds.
+ *   nfs_partials_count doubles in a partial-sum buffer of this context.
+ *   nfs_export_partials d_buf DEVICE [nfs_partials_count]: the context's sums in a form that adds up over contexts:
+ *                      pair sums per lag and pixel (per lag and |q| bin for NFS_FLAG_BIN_ONLY), sum |F_t|^2 and
+ *                      sum F_t over the own frames (absolute: independent of the context's reference frame), pair
+ *                      counts per lag, own-frame count.  Synchronises the stream.
+ *   nfs_import_partials d_buf DEVICE: replaces the context's sums by the buffer's — the caller has added the buffers
+ *                      of all contexts (one all-reduce(sum), e.g. ncclAllReduce over NVLink).
+ *                      Afterwards nfs_finalize and the getters return the result of the whole stack (counts and
+ *                      divisors come from the buffer); pushing more frames returns NFS_ERR_STATE until nfs_reset.
+ */
+NFS_API int nfs_push_halo(nfs_ctx* ctx, const uint16_t* d_frames, int n);
+NFS_API int64_t nfs_partials_count(const nfs_ctx* ctx);
+NFS_API int nfs_export_partials(nfs_ctx* ctx, double* d_buf);
+NFS_API int nfs_import_partials(nfs_ctx* ctx, const double* d_buf);
+
+/*
  * nfs_finalize — step 5 ("azimuthally averaged power spectra") for the N frames pushed
  * so far.  Synchronises the stream; non-destructive snapshot: pushing may continue afterwards.
  *   D_q_tau   HOST [n_lags][n_qbins] double   mean of D2d over bin b; rows with tau >= N are 0.

@@ -31,6 +31,10 @@ SYMBOLS = [
     ("nfs_get_transfer_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
     ("nfs_band_plan", C.c_int, [C.c_int64, C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]),
     ("nfs_push_frames", C.c_int, [_P, _P, C.c_int]),
+    ("nfs_push_halo", C.c_int, [_P, _P, C.c_int]),
+    ("nfs_partials_count", C.c_int64, [_P]),
+    ("nfs_export_partials", C.c_int, [_P, _P]),
+    ("nfs_import_partials", C.c_int, [_P, _P]),
     ("nfs_finalize", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_get_pair_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
     ("nfs_get_D2d", C.c_int, [_P, C.c_int, C.POINTER(C.c_double)]),
@@ -202,6 +206,33 @@ class NFS:
             self._stream.wait_stream(cur)
             frames.record_stream(self._stream)
         nfs_push_frames(self.handle, frames.data_ptr(), frames.shape[0])
+
+    def push_halo(self, frames):
+        """Frames that precede this context's own frames (time-chunk sharding, include/nfs.h)."""
+        import torch
+
+        assert frames.is_cuda and frames.dtype == torch.uint16 and frames.is_contiguous()
+        cur = torch.cuda.current_stream(frames.device)
+        if cur != self._stream:
+            self._stream.wait_stream(cur)
+            frames.record_stream(self._stream)
+        _check(self.lib.nfs_push_halo(self.handle, _P(frames.data_ptr()), int(frames.shape[0])), self.handle)
+
+    def export_partials(self):
+        """The context's partial sums as a float64 torch tensor on its device (ready for all_reduce)."""
+        import torch
+
+        buf = torch.empty(int(self.lib.nfs_partials_count(self.handle)), dtype=torch.float64, device="cuda")
+        _check(self.lib.nfs_export_partials(self.handle, _P(buf.data_ptr())), self.handle)
+        return buf
+
+    def import_partials(self, buf):
+        import torch
+
+        assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous()
+        assert buf.numel() == int(self.lib.nfs_partials_count(self.handle))
+        torch.cuda.current_stream(buf.device).synchronize()   # the caller's all-reduce ran on torch's stream
+        _check(self.lib.nfs_import_partials(self.handle, _P(buf.data_ptr())), self.handle)
 
     def push_ptr(self, ptr, n):
         nfs_push_frames(self.handle, ptr, n)

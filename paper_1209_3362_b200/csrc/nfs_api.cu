@@ -143,7 +143,7 @@ bool build_tables(Ctx& c) {
 
 void free_all(Ctx& c) {
   void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.totals_b, c.I2,      c.I1,       c.sums,    c.tw,     c.tw_out,
-                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim};
+                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim, c.d_npairs};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (c.h_store) cudaFreeHost(c.h_store);
@@ -166,6 +166,10 @@ bool zero_state(Ctx& c) {
   c.n_frames = 0;
   c.n_acc = 0;
   c.n_launches = 0;
+  c.n_halo = 0;
+  c.merged = false;
+  c.merged_pairs.clear();
+  c.merged_frames = 0;
   c.swept_frames = -1;
   c.ring_dirty = false;
   c.h2d_frames = c.d2h_frames = 0;
@@ -398,6 +402,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   ok = ok && dev_alloc(c, &c.d_out, (size_t)(c.n_lags + 2) * c.n_qbins);
   ok = ok && dev_alloc(c, &c.d_tmp, (size_t)c.P);
   ok = ok && dev_alloc(c, &c.d_flags, 1);
+  ok = ok && dev_alloc(c, &c.d_npairs, (size_t)c.n_lags);
   ok = ok && build_tables(c);
   ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)(c.R + c.RN) * c.P, c.stream));
   ok = ok && zero_state(c);
@@ -497,11 +502,13 @@ int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int
   return nfs_create_opts(out, W, H, lags, n_lags, n_qbins, cuda_stream, 0, 0u);
 }
 
-static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n) {
+static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n, bool halo) {
   if (!h || !d_frames || n < 1) return NFS_ERR_INVALID_ARG;
   if ((reinterpret_cast<uintptr_t>(d_frames) & 15u) != 0) return NFS_ERR_INVALID_ARG;  // 128-bit loads
   Ctx& c = h->c;
   if (!enter(c)) return c.status;
+  if (c.merged) return NFS_ERR_STATE;  // the sums are those of all contexts: start over with nfs_reset
+  if (halo && (c.n_frames != c.n_halo || c.band_width > 0 || c.n_frames + n > c.R - c.B)) return NFS_ERR_STATE;
   const int64_t fpx = (int64_t)c.W * c.H;
   if (c.band_width > 0) {
     if (c.n_frames + n > c.max_frames) return NFS_ERR_INVALID_ARG;  // the host store was sized for max_frames
@@ -523,11 +530,70 @@ static int push_impl(nfs_ctx* h, const uint16_t* d_frames, int n) {
     if (c.band_width > 0 && !copy_frames(c, c.ring, c.R, c.n_frames, c.n_frames + b, false)) return c.status;
     c.n_frames += b;
     done += b;
-    if (c.n_frames - c.n_acc == c.B && !flush_pending(c)) return c.status;
+    if (halo) {  // halo frames only enter the ring: no pair has one of them as its later frame
+      c.n_halo = c.n_frames;
+      c.n_acc = c.n_frames;
+    } else if (c.n_frames - c.n_acc == c.B && !flush_pending(c)) {
+      return c.status;
+    }
   }
   return NFS_OK;
 }
-int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) { NFS_GUARDED(push_impl(h, d_frames, n)) }
+int nfs_push_frames(nfs_ctx* h, const uint16_t* d_frames, int n) { NFS_GUARDED(push_impl(h, d_frames, n, false)) }
+int nfs_push_halo(nfs_ctx* h, const uint16_t* d_frames, int n) { NFS_GUARDED(push_impl(h, d_frames, n, true)) }
+
+// ---- partial sums of a context, for the one all-reduce of time-chunk sharding ----
+// layout (doubles): [n_lags][P] pair sums (bin-only contexts: [n_lags][n_qbins]) | S2 [P] | S1 [P][2] | pairs [n_lags] | frames [1]
+static int64_t partials_rows(const Ctx& c) { return c.bin_only ? (int64_t)c.n_qbins : c.P; }
+int64_t nfs_partials_count(const nfs_ctx* h) {
+  if (!h) return 0;
+  const Ctx& c = h->c;
+  return (int64_t)c.n_lags * partials_rows(c) + 3 * c.P + c.n_lags + 1;
+}
+static int export_impl(nfs_ctx* h, double* d_buf) {
+  if (!d_buf) return NFS_ERR_INVALID_ARG;
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
+  Ctx& c = h->c;
+  if (c.merged) return NFS_ERR_STATE;
+  const size_t nA = (size_t)c.n_lags * (size_t)partials_rows(c);
+  if (!NFS_CUDA(c, cudaMemcpyAsync(d_buf, c.bin_only ? c.totals_b : c.totals, sizeof(double) * nA, cudaMemcpyDeviceToDevice, c.stream)))
+    return c.status;
+  c.n_launches += launch_absolute_I(c, d_buf + nA, reinterpret_cast<double2*>(d_buf + nA + c.P));
+  std::vector<double> tail((size_t)c.n_lags + 1);
+  for (int l = 0; l < c.n_lags; ++l) tail[(size_t)l] = (double)pair_count(c, l);  // exact: counts < 2^53
+  tail[(size_t)c.n_lags] = (double)frames_in_I(c);
+  if (!NFS_CUDA(c, cudaMemcpyAsync(d_buf + nA + 3 * c.P, tail.data(), sizeof(double) * tail.size(), cudaMemcpyHostToDevice, c.stream)))
+    return c.status;
+  return sync_and_check(c);
+}
+int nfs_export_partials(nfs_ctx* h, double* d_buf) { NFS_GUARDED(export_impl(h, d_buf)) }
+
+static int import_impl(nfs_ctx* h, const double* d_buf) {
+  if (!h || !d_buf) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (!enter(c)) return c.status;
+  if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (!flush_pending(c)) return c.status;
+  const size_t nA = (size_t)c.n_lags * (size_t)partials_rows(c);
+  std::vector<double> tail((size_t)c.n_lags + 1);
+  bool ok = NFS_CUDA(c, cudaMemcpyAsync(c.bin_only ? c.totals_b : c.totals, d_buf, sizeof(double) * nA, cudaMemcpyDeviceToDevice, c.stream));
+  ok = ok && NFS_CUDA(c, cudaMemcpyAsync(c.I2, d_buf + nA, sizeof(double) * (size_t)c.P, cudaMemcpyDeviceToDevice, c.stream));
+  ok = ok && NFS_CUDA(c, cudaMemcpyAsync(c.I1, d_buf + nA + c.P, sizeof(double2) * (size_t)c.P, cudaMemcpyDeviceToDevice, c.stream));
+  // the imported I sums are absolute: from here on the context's reference frame is zero
+  ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.Fref, 0, sizeof(float2) * (size_t)c.P, c.stream));
+  ok = ok && NFS_CUDA(c, cudaMemcpyAsync(tail.data(), d_buf + nA + 3 * c.P, sizeof(double) * tail.size(), cudaMemcpyDeviceToHost, c.stream));
+  if (!ok) return c.status;
+  const int st = sync_and_check(c);
+  if (st != NFS_OK) return st;
+  c.merged_pairs.resize((size_t)c.n_lags);
+  for (int l = 0; l < c.n_lags; ++l) c.merged_pairs[(size_t)l] = (int64_t)llround(tail[(size_t)l]);
+  c.merged_frames = (int64_t)llround(tail[(size_t)c.n_lags]);
+  c.merged = true;
+  c.swept_frames = c.n_frames;
+  return c.merged_frames >= 1 ? NFS_OK : NFS_ERR_STATE;
+}
+int nfs_import_partials(nfs_ctx* h, const double* d_buf) { NFS_GUARDED(import_impl(h, d_buf)) }
 
 static int finalize_impl(nfs_ctx* h, double* D_q_tau, double* I_q, int64_t* counts) {
   const int rc = ready(h);
@@ -553,7 +619,7 @@ int nfs_get_pair_counts(nfs_ctx* h, int64_t* n_pairs) {
   if (!h || !n_pairs) return NFS_ERR_INVALID_ARG;
   const Ctx& c = h->c;
   if (c.status != NFS_OK) return c.status;
-  for (int l = 0; l < c.n_lags; ++l) n_pairs[l] = c.lags[l] < c.n_frames ? c.n_frames - c.lags[l] : 0;
+  for (int l = 0; l < c.n_lags; ++l) n_pairs[l] = pair_count(c, l);
   return NFS_OK;
 }
 

@@ -36,16 +36,16 @@ __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, 
                                              const double* __restrict__ I2,
                                              const double2* __restrict__ I1, const float2* __restrict__ Fref,
                                              const uint32_t* __restrict__ perm, const int32_t* __restrict__ bin_start,
-                                             const int32_t* __restrict__ lags, int n_lags, int n_qbins, int64_t P,
+                                             const long long* __restrict__ npairs, int n_lags, int n_qbins, int64_t P,
                                              int64_t N, double* __restrict__ out) {
   const int b = blockIdx.x, row = blockIdx.y;
   const int beg = bin_start[b], end = bin_start[b + 1];
   double inv;
   if (row < n_lags) {
-    const int64_t np = N - (int64_t)lags[row];
+    const long long np = npairs[row];  // frame pairs accumulated at this lag (N - tau for a whole stack on one context)
     inv = np > 0 ? 1.0 / (double)np : 0.0;
   } else {
-    inv = 1.0 / (double)N;
+    inv = 1.0 / (double)N;  // N: frames in the I sums
   }
   double acc = 0.0, wsum = 0.0;
   for (int i = beg + (int)threadIdx.x; i < end; i += 128) {
@@ -122,11 +122,34 @@ __global__ void __launch_bounds__(256) k_D2d(const double* __restrict__ tot, int
   if (p < P) dst[p] = tot[p] * inv;
 }
 
+// partial sums of one context in a form that adds up over contexts (time-chunk sharding): the I sums
+// relative to this context's reference frame become absolute, S2 = sum |F_t|^2 and S1 = sum F_t over its n own frames
+__global__ void __launch_bounds__(256) k_absolute_I(const double* __restrict__ I2, const double2* __restrict__ I1,
+                                                    const float2* __restrict__ Fref, int64_t P, double n,
+                                                    double* __restrict__ S2, double2* __restrict__ S1) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const float2 fr = Fref[p];
+  const double2 s1 = I1[p];
+  const double rx = (double)fr.x, ry = (double)fr.y;
+  S2[p] = I2[p] + 2.0 * (s1.x * rx + s1.y * ry) + n * (rx * rx + ry * ry);
+  S1[p] = make_double2(s1.x + n * rx, s1.y + n * ry);
+}
+
+int launch_absolute_I(Ctx& c, double* d_S2, double2* d_S1) {
+  k_absolute_I<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, (double)frames_in_I(c), d_S2, d_S1);
+  NFS_CUDA(c, cudaGetLastError());
+  return 1;
+}
+
 int launch_bin(Ctx& c) {
   dim3 grid((unsigned)c.n_qbins, (unsigned)(c.n_lags + 2));
   ProfScope ps(c, kKBin);
+  std::vector<long long> np((size_t)c.n_lags);
+  for (int l = 0; l < c.n_lags; ++l) np[(size_t)l] = (long long)pair_count(c, l);
+  if (!NFS_CUDA(c, cudaMemcpyAsync(c.d_npairs, np.data(), sizeof(long long) * np.size(), cudaMemcpyHostToDevice, c.stream))) return 0;
   k_bin<<<grid, 128, 0, c.stream>>>(c.totals, c.bin_only ? c.totals_b : nullptr, c.I2, c.I1, c.Fref, c.perm, c.bin_start,
-                                    c.d_lags, c.n_lags, c.n_qbins, c.P, c.n_frames, c.d_out);
+                                    c.d_npairs, c.n_lags, c.n_qbins, c.P, frames_in_I(c), c.d_out);
   NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
@@ -141,19 +164,19 @@ int launch_bin_accumulate(Ctx& c, int l_first, int n_rows) {
 }
 
 int launch_I2d(Ctx& c, double* d_dst) {
-  k_I2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, c.n_frames, d_dst);
+  k_I2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.Fref, c.P, frames_in_I(c), d_dst);
   NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
 int launch_V2d(Ctx& c, double* d_dst) {
-  k_V2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.P, c.n_frames, d_dst);
+  k_V2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.I2, c.I1, c.P, frames_in_I(c), d_dst);
   NFS_CUDA(c, cudaGetLastError());
   return 1;
 }
 
 int launch_D2d(Ctx& c, int l, double* d_dst) {
-  const int64_t np = c.n_frames - (int64_t)c.lags[l];
+  const int64_t np = pair_count(c, l);
   const double inv = np > 0 ? 1.0 / (double)np : 0.0;
   k_D2d<<<(unsigned)((c.P + 255) / 256), 256, 0, c.stream>>>(c.totals + (int64_t)l * c.P, c.P, inv, d_dst);
   NFS_CUDA(c, cudaGetLastError());

@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -80,7 +81,15 @@ struct Ctx {
   std::vector<int64_t> counts;  // full-plane pixel count per bin
   cudaStream_t stream = nullptr;
   bool own_stream = false;
-  int64_t n_frames = 0;  // frames pushed (all transformed into the ring)
+  // time-chunk sharding over several contexts / GPUs: halo frames precede this context's own frames
+  // (they are transformed and paired with the own frames, but are no later frame of a pair and not in the I sums);
+  // after nfs_import_partials the sums are those of all contexts (`merged`): pair and frame counts come with them
+  int64_t n_halo = 0;
+  bool merged = false;
+  std::vector<int64_t> merged_pairs;  // [n_lags]
+  int64_t merged_frames = 0;
+  long long* d_npairs = nullptr;      // [n_lags] divisors of the binning kernel
+  int64_t n_frames = 0;  // frames pushed (all transformed into the ring), halo included
   int64_t n_acc = 0;     // of those, frames whose pairs are already in the totals
   int64_t n_launches = 0;
   int status = 0;  // sticky
@@ -132,6 +141,15 @@ struct Ctx {
   int64_t prof_n[kNumKernelClasses] = {0, 0, 0, 0, 0};
 };
 
+// frames in the I sums, and frame pairs accumulated at lag index l (N - tau for a whole stack)
+inline int64_t frames_in_I(const Ctx& c) { return c.merged ? c.merged_frames : c.n_frames - c.n_halo; }
+inline int64_t pair_count(const Ctx& c, int l) {
+  if (c.merged) return c.merged_pairs[(size_t)l];
+  const int64_t own = c.n_frames - c.n_halo;  // later frames s = n_halo .. n_frames-1; pair (s - tau, s) exists iff s >= tau
+  const int64_t missing = std::max<int64_t>(0, (int64_t)c.lags[(size_t)l] - c.n_halo);
+  return std::max<int64_t>(0, own - missing);
+}
+
 // record the first CUDA error of the context (sticky)
 inline bool cuda_ok(Ctx& c, cudaError_t e, const char* what) {
   if (e == cudaSuccess) return true;
@@ -181,6 +199,7 @@ bool lag_configure(Ctx& c);        // once at create, after the ring is allocate
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1), I (row n_lags), V (row n_lags+1)
 int launch_bin_accumulate(Ctx& c, int l_first, int n_rows);  // bin-only mode: totals_b[l_first..] += binned scratch rows
+int launch_absolute_I(Ctx& c, double* d_S2, double2* d_S1);  // S2 = sum |F_t|^2, S1 = sum F_t over the context's own frames
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
 int launch_V2d(Ctx& c, double* d_dst);       // d_dst[P] = V2d (variance form) in ring layout
 int launch_D2d(Ctx& c, int l, double* d_dst);
