@@ -181,6 +181,19 @@ NFS_API int nfs_get_I2d(nfs_ctx* ctx, double* out);
 NFS_API int nfs_get_variance(nfs_ctx* ctx, double* V_q);
 NFS_API int nfs_get_V2d(nfs_ctx* ctx, double* out);
 
+/* Per-|q| fit of Eq. 1 (<|Delta I_m(q,tau)|^2> = 2a { T I_s [1 - f(q,tau)] + B })
+ * to the azimuthally averaged structure function of the frames pushed so far:
+ *     D(b,tau) = A_b [1 - exp(-Gamma_b tau)] + C_b,   A = 2a T I_s (signal plateau), C = 2a B (noise floor),
+ * with the single-exponential intermediate scattering function f = exp(-Gamma tau) of diffusive fluctuations (the
+ * paper does not print its fitting procedure: reading R19 in DESIGN.md).  Unweighted least squares over the lags that
+ * have a frame pair; (A, C) by linear least squares for a trial Gamma, Gamma by a scan of 64 log-spaced rates between
+ * 1e-3 / tau_max and 1e2 / tau_min refined by 48 golden-section steps — run on the device, one warp per |q| bin,
+ * deterministic.  The model-free f follows as 1 - (D - C) / A.
+ *   A_q, C_q, Gamma_q, chi2_q  HOST [n_qbins] double (Gamma per frame; chi2 = sum of squared residuals); any may be
+ *                              NULL.  Empty bins and fewer than three usable lags give 0.
+ * Synchronises the stream; non-destructive. */
+NFS_API int nfs_fit_eq1(nfs_ctx* ctx, double* A_q, double* C_q, double* Gamma_q, double* chi2_q);
+
 /* Number of frames pushed so far; ring capacity in frames; bytes of device memory held. */
 NFS_API int64_t nfs_num_frames(const nfs_ctx* ctx);
 NFS_API int nfs_ring_capacity(const nfs_ctx* ctx);

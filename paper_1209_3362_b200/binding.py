@@ -41,6 +41,7 @@ SYMBOLS = [
     ("nfs_get_I2d", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_get_variance", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_get_V2d", C.c_int, [_P, C.POINTER(C.c_double)]),
+    ("nfs_fit_eq1", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     ("nfs_num_frames", C.c_int64, [_P]),
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
@@ -264,6 +265,12 @@ class NFS:
         out = np.zeros((self.H, self.W // 2 + 1), dtype=np.float64)
         _check(self.lib.nfs_get_V2d(self.handle, _dp(out, C.c_double)), self.handle)
         return out
+
+    def fit_eq1(self):
+        """Per-|q| fit of Eq. 1 to the binned structure function: (A, C, Gamma, chi2), each [n_qbins]."""
+        out = [np.zeros(self.n_qbins, dtype=np.float64) for _ in range(4)]
+        _check(self.lib.nfs_fit_eq1(self.handle, *[_dp(a, C.c_double) for a in out]), self.handle)
+        return tuple(out)
 
     def set_launch_shape(self, shape):
         _check(self.lib.nfs_set_launch_shape(self.handle, int(shape)), self.handle)

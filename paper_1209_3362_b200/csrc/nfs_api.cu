@@ -143,7 +143,7 @@ bool build_tables(Ctx& c) {
 
 void free_all(Ctx& c) {
   void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.totals_b, c.I2,      c.I1,       c.sums,    c.tw,     c.tw_out,
-                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim, c.d_npairs};
+                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim, c.d_npairs, c.d_fit};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (c.h_store) cudaFreeHost(c.h_store);
@@ -403,6 +403,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   ok = ok && dev_alloc(c, &c.d_tmp, (size_t)c.P);
   ok = ok && dev_alloc(c, &c.d_flags, 1);
   ok = ok && dev_alloc(c, &c.d_npairs, (size_t)c.n_lags);
+  ok = ok && dev_alloc(c, &c.d_fit, 4 * (size_t)c.n_qbins);
   ok = ok && build_tables(c);
   ok = ok && NFS_CUDA(c, cudaMemsetAsync(c.ring, 0, sizeof(float2) * (size_t)(c.R + c.RN) * c.P, c.stream));
   ok = ok && zero_state(c);
@@ -661,6 +662,24 @@ static int variance_impl(nfs_ctx* h, double* V_q) {
   return sync_and_check(c);
 }
 int nfs_get_variance(nfs_ctx* h, double* V_q) { NFS_GUARDED(variance_impl(h, V_q)) }
+
+static int fit_impl(nfs_ctx* h, double* A_q, double* C_q, double* Gamma_q, double* chi2_q) {
+  const int rc = ready(h);
+  if (rc != NFS_OK) return rc;
+  Ctx& c = h->c;
+  c.n_launches += launch_bin(c);
+  c.n_launches += launch_fit_eq1(c);
+  if (c.status != NFS_OK) return c.status;
+  double* dst[4] = {A_q, C_q, Gamma_q, chi2_q};
+  for (int k = 0; k < 4; ++k)
+    if (dst[k] && !NFS_CUDA(c, cudaMemcpyAsync(dst[k], c.d_fit + (size_t)k * c.n_qbins, sizeof(double) * c.n_qbins,
+                                               cudaMemcpyDeviceToHost, c.stream)))
+      return c.status;
+  return sync_and_check(c);
+}
+int nfs_fit_eq1(nfs_ctx* h, double* A_q, double* C_q, double* Gamma_q, double* chi2_q) {
+  NFS_GUARDED(fit_impl(h, A_q, C_q, Gamma_q, chi2_q))
+}
 
 int64_t nfs_num_frames(const nfs_ctx* h) { return h ? h->c.n_frames : 0; }
 int nfs_ring_capacity(const nfs_ctx* h) { return h ? h->c.R : 0; }

@@ -154,6 +154,122 @@ int launch_bin(Ctx& c) {
   return 1;
 }
 
+// ---- per-|q| fit of Eq. 1 (reading R19 in DESIGN.md) -----------------------
+// D(b,tau) = A_b [1 - exp(-Gamma_b tau)] + C_b by unweighted least squares over the lags that have a frame pair:
+// A = 2a T I_s (plateau), C = 2a B (noise floor), f = exp(-Gamma tau).  Variable projection: for a trial x = log Gamma
+// the pair (A, C) is the linear least-squares solution; chi2(x) is scanned on 64 grid points of
+// [log(1e-3 / tau_max), log(1e2 / tau_min)] and refined by 48 golden-section steps around the best one.  One warp per
+// |q| bin, the lags spread over its lanes, fixed shuffle tree: deterministic.  Everything in fp64.
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+struct Eq1Lin {
+  double A, C, chi2;
+};
+__device__ __forceinline__ Eq1Lin eq1_linear(double x, const double* __restrict__ Db, int n_qbins,
+                                             const long long* __restrict__ npairs, const int32_t* __restrict__ lags, int n_lags,
+                                             int lane) {
+  const double G = exp(x);
+  double n = 0.0, Sg = 0.0, Sgg = 0.0, Sd = 0.0, Sgd = 0.0;
+  for (int l = lane; l < n_lags; l += 32) {
+    if (npairs[l] > 0) {
+      const double g = -expm1(-G * (double)lags[l]), d = Db[(int64_t)l * n_qbins];
+      n += 1.0, Sg += g, Sgg += g * g, Sd += d, Sgd += g * d;
+    }
+  }
+  n = warp_sum(n), Sg = warp_sum(Sg), Sgg = warp_sum(Sgg), Sd = warp_sum(Sd), Sgd = warp_sum(Sgd);
+  Eq1Lin r;
+  const double det = n * Sgg - Sg * Sg;
+  if (det <= 1e-14 * n * Sgg) {
+    r.A = 0.0;
+    r.C = Sd / n;
+  } else {
+    r.A = (n * Sgd - Sg * Sd) / det;
+    r.C = (Sd - r.A * Sg) / n;
+  }
+  double c2 = 0.0;
+  for (int l = lane; l < n_lags; l += 32) {
+    if (npairs[l] > 0) {
+      const double g = -expm1(-G * (double)lags[l]);
+      const double e = Db[(int64_t)l * n_qbins] - r.A * g - r.C;
+      c2 += e * e;
+    }
+  }
+  r.chi2 = warp_sum(c2);
+  return r;
+}
+
+// grid: ceil(n_qbins / 4) CTAs of 4 warps.  D = binned structure function [n_lags][n_qbins]; fit = [4][n_qbins]: A, C, Gamma, chi2
+__global__ void __launch_bounds__(128) k_fit_eq1(const double* __restrict__ D, const long long* __restrict__ npairs,
+                                                 const int32_t* __restrict__ lags, const int32_t* __restrict__ bin_start,
+                                                 int n_lags, int n_qbins, double* __restrict__ fit) {
+  const int b = (int)blockIdx.x * 4 + ((int)threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (b >= n_qbins) return;
+  int used = 0, tmin = 0x7fffffff, tmax = 0;
+  for (int l = lane; l < n_lags; l += 32) {
+    if (npairs[l] > 0) {
+      ++used;
+      tmin = min(tmin, lags[l]);
+      tmax = max(tmax, lags[l]);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    used += __shfl_xor_sync(0xffffffffu, used, o);
+    tmin = min(tmin, __shfl_xor_sync(0xffffffffu, tmin, o));
+    tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+  }
+  double A = 0.0, C = 0.0, G = 0.0, chi2 = 0.0;
+  if (used >= 3 && bin_start[b + 1] > bin_start[b]) {
+    const double* Db = D + b;
+    const double lo = log(1e-3 / (double)tmax), hi = log(1e2 / (double)tmin);
+    constexpr int K = 64;
+    int kbest = 0;
+    double cbest = 0.0;
+    for (int k = 0; k < K; ++k) {
+      const double c2 = eq1_linear(lo + (hi - lo) * (double)k / (double)(K - 1), Db, n_qbins, npairs, lags, n_lags, lane).chi2;
+      if (k == 0 || c2 < cbest) cbest = c2, kbest = k;
+    }
+    double a = lo + (hi - lo) * (double)max(kbest - 1, 0) / (double)(K - 1);
+    double c = lo + (hi - lo) * (double)min(kbest + 1, K - 1) / (double)(K - 1);
+    const double inv_phi = 0.61803398874989484820;
+    double x1 = c - inv_phi * (c - a), x2 = a + inv_phi * (c - a);
+    double f1 = eq1_linear(x1, Db, n_qbins, npairs, lags, n_lags, lane).chi2;
+    double f2 = eq1_linear(x2, Db, n_qbins, npairs, lags, n_lags, lane).chi2;
+    for (int it = 0; it < 48; ++it) {
+      if (f1 <= f2) {
+        c = x2, x2 = x1, f2 = f1;
+        x1 = c - inv_phi * (c - a);
+        f1 = eq1_linear(x1, Db, n_qbins, npairs, lags, n_lags, lane).chi2;
+      } else {
+        a = x1, x1 = x2, f1 = f2;
+        x2 = a + inv_phi * (c - a);
+        f2 = eq1_linear(x2, Db, n_qbins, npairs, lags, n_lags, lane).chi2;
+      }
+    }
+    const double x = 0.5 * (a + c);
+    const Eq1Lin r = eq1_linear(x, Db, n_qbins, npairs, lags, n_lags, lane);
+    A = r.A, C = r.C, G = exp(x), chi2 = r.chi2;
+  }
+  if (lane == 0) {
+    fit[b] = A;
+    fit[(int64_t)n_qbins + b] = C;
+    fit[2 * (int64_t)n_qbins + b] = G;
+    fit[3 * (int64_t)n_qbins + b] = chi2;
+  }
+}
+
+// after launch_bin (d_out and d_npairs are up to date): d_fit = [4][n_qbins]
+int launch_fit_eq1(Ctx& c) {
+  ProfScope ps(c, kKBin);
+  k_fit_eq1<<<(unsigned)((c.n_qbins + 3) / 4), 128, 0, c.stream>>>(c.d_out, c.d_npairs, c.d_lags, c.bin_start, c.n_lags, c.n_qbins,
+                                                                 c.d_fit);
+  NFS_CUDA(c, cudaGetLastError());
+  return 1;
+}
+
 int launch_bin_accumulate(Ctx& c, int l_first, int n_rows) {
   dim3 grid((unsigned)c.n_qbins, (unsigned)n_rows);
   ProfScope ps(c, kKBin);

@@ -116,6 +116,7 @@ struct Ctx {
   uint32_t* perm = nullptr;      // [n_binned] pixel index | (weight-2 flag << 31), grouped by bin
   int32_t* bin_start = nullptr;  // [n_qbins + 1]
   double* d_out = nullptr;       // [(n_lags + 2)][n_qbins] binned results: D rows, I row, V row
+  double* d_fit = nullptr;       // [4][n_qbins] Eq. 1 fit: A, C, Gamma, chi2
   double* d_tmp = nullptr;       // [P] scratch for the 2-D getters
   int* d_flags = nullptr;        // [1] bit0 = zero-mean frame seen
   LagTask* d_tasks = nullptr;
@@ -198,6 +199,7 @@ bool lag_plan(Ctx& c, int smem_per_sm, int n_sm, int64_t P);
 bool lag_configure(Ctx& c);        // once at create, after the ring is allocated: tensor map, kernel attributes
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1), I (row n_lags), V (row n_lags+1)
+int launch_fit_eq1(Ctx& c);                  // after launch_bin: d_fit = per-|q| fit of Eq. 1 to the binned D
 int launch_bin_accumulate(Ctx& c, int l_first, int n_rows);  // bin-only mode: totals_b[l_first..] += binned scratch rows
 int launch_absolute_I(Ctx& c, double* d_S2, double2* d_S1);  // S2 = sum |F_t|^2, S1 = sum F_t over the context's own frames
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
