@@ -28,6 +28,7 @@ constexpr int kMinStages = 2;
 constexpr int kMaxStages = 8;     // pipeline depth is chosen at create from the shared memory left
 constexpr int kFoldChunks = 40;   // fp32 partial sums are folded into the fp64 totals every kFoldChunks * kChunk (1040) steps
 constexpr int kSparseMax = 6;     // lags per lag-list task (one LDS.64 per pair update, exact-count code paths)
+constexpr int kDenseMaxWide = 5;  // lags per register-window task in a 16-slot plan (long windows): balances the runs against the lag lists
 constexpr int kDenseMin = 2;      // runs of >= kDenseMin consecutive lags use the register-window path
 
 struct LagTask {

@@ -833,7 +833,7 @@ void close_group(const std::vector<int32_t>& L, const std::vector<Atom>& atoms, 
 }
 }  // namespace
 
-static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
+static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P, int dense_max = kG) {
   const std::vector<int32_t>& L = c.lags;
   // shared memory a CTA may use: the opt-in maximum (one CTA per SM) bounds a group's window; two CTAs of 32-pixel
   // tiles share an SM when the plan's footprint allows it (1 KB per CTA is reserved, 1 KB static)
@@ -848,7 +848,7 @@ static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P) {
     while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1 && band_of(L[j + 1]) == band_of(L[i])) ++j;
     const int len = j - i + 1;
     if (len >= kDenseMin) {
-      const int nt = (len + kG - 1) / kG;
+      const int nt = (len + dense_max - 1) / dense_max;
       int l = i;
       for (int k = 0; k < nt; ++k) {
         const int cnt = len / nt + (k < len % nt ? 1 : 0);
@@ -992,7 +992,7 @@ bool lag_plan(Ctx& c, int smem_sm, int n_sm, int64_t P) {
   if (!plan_with(c, kTaskSlots, smem_sm, n_sm, P)) return false;
   if (c.lag_tpx == 32 && c.lag_ctas_per_sm == 1) {
     Ctx alt = c;
-    if (plan_with(alt, 2 * kTaskSlots, smem_sm, n_sm, P)) {
+    if (plan_with(alt, 2 * kTaskSlots, smem_sm, n_sm, P, kDenseMaxWide)) {
       c.tasks = alt.tasks, c.groups = alt.groups;
       c.lag_stages = alt.lag_stages, c.lag_smem = alt.lag_smem, c.lag_tpx = alt.lag_tpx, c.lag_slots = alt.lag_slots;
       c.lag_ctas_per_sm = alt.lag_ctas_per_sm, c.lag_grid = alt.lag_grid, c.max_group_lags = alt.max_group_lags;
