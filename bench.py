@@ -462,6 +462,7 @@ def run_hbm_regime(torch, binding, stack, cfg, P, peaks, inst_per_update):
         if i == 0:
             h.kernel_times()
     ms, n = h.kernel_times()["lag_accum"]
+    probe_ms, probe_bytes = h.probe_lag_traffic(B, 20)
     h.close()
     nb = (cfg.N + B - 1) // B
     alg = P * (8.0 * (cfg.N + nb * cfg.lags[-1]) + 16.0 * len(cfg.lags) * nb)  # bytes per stack
@@ -469,7 +470,13 @@ def run_hbm_regime(torch, binding, stack, cfg, P, peaks, inst_per_update):
     return dict(internal_batch=B, launches_per_step=n / steps, ms_per_step=ms / steps, algorithmic_gb_per_step=alg / 1e9,
                 achieved_gbs=ach, peak_gbs=peaks["hbm_gbs"], frac=ach / peaks["hbm_gbs"],
                 alu_floor_ms=(sum(max(0, cfg.N - t) for t in cfg.lags) * P * inst_per_update) / (SM_COUNT * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6) * 1e3,
-                note="same kernel and stack, batches of 26 frames: algorithmic HBM time exceeds the ALU floor, HBM is the bound")
+                note="same kernel and stack, batches of 26 frames: algorithmic HBM time exceeds the ALU floor, HBM is the bound",
+                access_pattern_probe=dict(ms_per_launch=probe_ms, algorithmic_gb_per_launch=probe_bytes / 1e9,
+                                          achieved_gbs=probe_bytes / (probe_ms * 1e-3) / 1e9,
+                                          frac_of_copy_peak=probe_bytes / (probe_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                          kernel_ms_per_launch=ms / max(n, 1),
+                                          note="nfs_probe_lag_traffic: the same TMA box copies and fp64 reductions per launch, no "
+                                               "arithmetic — what this access pattern reaches on this device"))
 
 
 def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):

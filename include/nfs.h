@@ -212,6 +212,15 @@ NFS_API int64_t nfs_num_launches(const nfs_ctx* ctx);
 NFS_API int nfs_set_profiling(nfs_ctx* ctx, int enable);
 NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
 
+/* Measurement aid for bench.py (not part of the analysis): launches `reps` times a kernel with the memory access
+ * pattern of ONE lag-accumulation launch over a batch of batch_frames frames — the 2-D TMA box copies of every pixel
+ * tile's lag window into shared memory and two fp64 reductions (of 0.0: the accumulators keep their values) per
+ * (lag, pixel) — without the arithmetic, and returns its mean duration (CUDA events on the context's stream) and the
+ * algorithmic bytes P (8 (window + batch) + 16 n_lags) it moves: the ceiling of the access pattern on this device, to
+ * which the real kernel's small-batch (HBM-bound) regime is compared.  Synchronises.  NFS_ERR_STATE for bin-only or
+ * banded contexts. */
+NFS_API int nfs_probe_lag_traffic(nfs_ctx* ctx, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch);
+
 /* Launch shape of the lag-accumulation kernel: 0 = chosen per batch (default), 1 = always one CTA per (pixel tile,
  * lag group), 2 = always persistent CTAs that claim pixel tiles.  The same kernel code handles the same tile either
  * way (results are bit-identical); used by the tests and by bench.py's small-batch measurement. */

@@ -42,6 +42,7 @@ SYMBOLS = [
     ("nfs_get_variance", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_get_V2d", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_fit_eq1", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    ("nfs_probe_lag_traffic", C.c_int, [_P, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     ("nfs_num_frames", C.c_int64, [_P]),
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
@@ -271,6 +272,12 @@ class NFS:
         out = [np.zeros(self.n_qbins, dtype=np.float64) for _ in range(4)]
         _check(self.lib.nfs_fit_eq1(self.handle, *[_dp(a, C.c_double) for a in out]), self.handle)
         return tuple(out)
+
+    def probe_lag_traffic(self, batch_frames, reps=20):
+        """(ms per launch, algorithmic bytes per launch) of the lag kernel's memory access pattern without its arithmetic."""
+        ms, by = C.c_double(0.0), C.c_double(0.0)
+        _check(self.lib.nfs_probe_lag_traffic(self.handle, int(batch_frames), int(reps), C.byref(ms), C.byref(by)), self.handle)
+        return ms.value, by.value
 
     def set_launch_shape(self, shape):
         _check(self.lib.nfs_set_launch_shape(self.handle, int(shape)), self.handle)

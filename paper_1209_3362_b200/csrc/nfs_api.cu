@@ -681,6 +681,31 @@ int nfs_fit_eq1(nfs_ctx* h, double* A_q, double* C_q, double* Gamma_q, double* c
   NFS_GUARDED(fit_impl(h, A_q, C_q, Gamma_q, chi2_q))
 }
 
+static int probe_impl(nfs_ctx* h, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch) {
+  if (!h || batch_frames < 1 || reps < 1 || !ms_per_launch) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (!enter(c)) return c.status;
+  if (c.bin_only || c.band_width > 0) return NFS_ERR_STATE;
+  cudaEvent_t e0, e1;
+  if (!NFS_CUDA(c, cudaEventCreate(&e0)) || !NFS_CUDA(c, cudaEventCreate(&e1))) return c.status;
+  double bytes = 0.0;
+  launch_lag_probe(c, batch_frames, &bytes);  // warm-up
+  NFS_CUDA(c, cudaEventRecord(e0, c.stream));
+  for (int r = 0; r < reps; ++r) c.n_launches += launch_lag_probe(c, batch_frames, &bytes);
+  NFS_CUDA(c, cudaEventRecord(e1, c.stream));
+  NFS_CUDA(c, cudaStreamSynchronize(c.stream));
+  float ms = 0.f;
+  NFS_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *ms_per_launch = (double)ms / reps;
+  if (bytes_per_launch) *bytes_per_launch = bytes;
+  return c.status;
+}
+int nfs_probe_lag_traffic(nfs_ctx* h, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch) {
+  NFS_GUARDED(probe_impl(h, batch_frames, reps, ms_per_launch, bytes_per_launch))
+}
+
 int64_t nfs_num_frames(const nfs_ctx* h) { return h ? h->c.n_frames : 0; }
 int nfs_ring_capacity(const nfs_ctx* h) { return h ? h->c.R : 0; }
 int64_t nfs_device_bytes(const nfs_ctx* h) { return h ? h->c.dev_bytes : 0; }

@@ -198,6 +198,8 @@ int launch_lag_tiled(Ctx& c, int64_t t0, int b, int band = 0);  // band > 0: a s
 // c.max_smem_optin; false if a lag group cannot fit shared memory
 bool lag_plan(Ctx& c, int smem_per_sm, int n_sm, int64_t P);
 bool lag_configure(Ctx& c);        // once at create, after the ring is allocated: tensor map, kernel attributes
+// nfs_probe.cu (measurement aid): the traffic of one small-batch lag launch without its arithmetic
+int launch_lag_probe(Ctx& c, int b, double* bytes);
 // nfs_bin.cu
 int launch_bin(Ctx& c);                      // d_out = azimuthal means of D (rows 0..n_lags-1), I (row n_lags), V (row n_lags+1)
 int launch_fit_eq1(Ctx& c);                  // after launch_bin: d_fit = per-|q| fit of Eq. 1 to the binned D
