@@ -78,6 +78,12 @@ typedef enum nfs_status {
  *                       NFS_ERR_STATE.
  */
 #define NFS_FLAG_BIN_ONLY 1u
+/*   NFS_FLAG_GUARD      debugging aid: every device buffer of the context is allocated between two 64 KB guard zones
+ *                       filled with a canary byte; nfs_check_guards(ctx, &n_bad) synchronises, reads the zones back and
+ *                       returns NFS_OK if they are intact, NFS_ERR_STATE otherwise (n_bad HOST: overwritten bytes; may
+ *                       be NULL) — an out-of-bounds write of a kernel beside one of the library's buffers is caught
+ *                       without an external tool.  NFS_ERR_STATE also if the context was created without the flag. */
+#define NFS_FLAG_GUARD 2u
 NFS_API int nfs_create(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream);
 NFS_API int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
                           int batch_frames);
@@ -193,6 +199,8 @@ NFS_API int nfs_get_V2d(nfs_ctx* ctx, double* out);
  *                              NULL.  Empty bins and fewer than three usable lags give 0.
  * Synchronises the stream; non-destructive. */
 NFS_API int nfs_fit_eq1(nfs_ctx* ctx, double* A_q, double* C_q, double* Gamma_q, double* chi2_q);
+
+NFS_API int nfs_check_guards(nfs_ctx* ctx, int64_t* n_bad);
 
 /* Number of frames pushed so far; ring capacity in frames; bytes of device memory held. */
 NFS_API int64_t nfs_num_frames(const nfs_ctx* ctx);

@@ -43,6 +43,7 @@ SYMBOLS = [
     ("nfs_get_V2d", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_fit_eq1", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     ("nfs_probe_lag_traffic", C.c_int, [_P, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    ("nfs_check_guards", C.c_int, [_P, C.POINTER(C.c_int64)]),
     ("nfs_num_frames", C.c_int64, [_P]),
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
@@ -59,6 +60,7 @@ SYMBOLS = [
 
 KERNEL_CLASSES = ["ref_setup", "fft", "unused", "lag_accum", "bin"]
 NFS_FLAG_BIN_ONLY = 1
+NFS_FLAG_GUARD = 2
 SHAPE_AUTO, SHAPE_ONE_TILE, SHAPE_PERSISTENT = 0, 1, 2
 
 _lib = None
@@ -176,7 +178,8 @@ class NFS:
     temporary passed to push() is not recycled while the kernels still read it): include/nfs.h puts both duties on
     the caller of nfs_push_frames."""
 
-    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False, ring_frames_cap=0, max_frames=0):
+    def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False, ring_frames_cap=0, max_frames=0,
+                 guard=False):
         import torch
 
         self.lib = load_library()
@@ -187,7 +190,8 @@ class NFS:
             stream = torch.cuda.Stream()
         self._stream = stream  # without a device nfs_create itself reports NFS_ERR_CUDA: no fallback
         self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None, batch_frames,
-                                 NFS_FLAG_BIN_ONLY if bin_only else 0, ring_frames_cap, max_frames)
+                                 (NFS_FLAG_BIN_ONLY if bin_only else 0) | (NFS_FLAG_GUARD if guard else 0), ring_frames_cap,
+                                 max_frames)
 
     def transfer_counts(self):
         out = np.zeros(4, dtype=np.int64)
@@ -278,6 +282,14 @@ class NFS:
         ms, by = C.c_double(0.0), C.c_double(0.0)
         _check(self.lib.nfs_probe_lag_traffic(self.handle, int(batch_frames), int(reps), C.byref(ms), C.byref(by)), self.handle)
         return ms.value, by.value
+
+    def check_guards(self):
+        """Overwritten guard bytes around the context's device buffers (0 = intact); needs guard=True at creation."""
+        n = C.c_int64(0)
+        rc = self.lib.nfs_check_guards(self.handle, C.byref(n))
+        if rc not in (NFS_OK, NFS_ERR_STATE) or (rc == NFS_ERR_STATE and n.value == 0):
+            _check(rc, self.handle)
+        return int(n.value)
 
     def set_launch_shape(self, shape):
         _check(self.lib.nfs_set_launch_shape(self.handle, int(shape)), self.handle)

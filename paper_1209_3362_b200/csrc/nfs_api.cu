@@ -20,12 +20,24 @@ namespace {
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
+// Every device buffer of a context comes from here.  With NFS_FLAG_GUARD each one sits between two guard zones of
+// kGuardBytes filled with a canary byte, which nfs_check_guards reads back: an out-of-bounds write of any kernel next
+// to one of the library's buffers is then detected (the substitute for compute-sanitizer memcheck where that tool is
+// not available).
+constexpr size_t kGuardBytes = 64 << 10;
+constexpr int kGuardByte = 0xA5;
 template <typename T>
 bool dev_alloc(Ctx& c, T** p, size_t count) {
   void* q = nullptr;
   const size_t bytes = sizeof(T) * (count ? count : 1);
-  if (!cuda_ok(c, cudaMalloc(&q, bytes), "cudaMalloc")) return false;
-  *p = reinterpret_cast<T*>(q);
+  const size_t user = (bytes + 255) / 256 * 256;
+  const size_t g = c.guard ? kGuardBytes : 0;
+  if (!cuda_ok(c, cudaMalloc(&q, user + 2 * g), "cudaMalloc")) return false;
+  c.allocs.push_back(Ctx::Alloc{q, user});
+  if (g && (!cuda_ok(c, cudaMemset(q, kGuardByte, g), "cudaMemset") ||
+            !cuda_ok(c, cudaMemset(static_cast<char*>(q) + g + bytes, kGuardByte, (user - bytes) + g), "cudaMemset")))
+    return false;
+  *p = reinterpret_cast<T*>(static_cast<char*>(q) + g);
   c.dev_bytes += (int64_t)bytes;
   return true;
 }
@@ -142,10 +154,8 @@ bool build_tables(Ctx& c) {
 }
 
 void free_all(Ctx& c) {
-  void* ptrs[] = {c.ring,   c.rowbuf, c.ref,       c.Fref,  c.totals, c.totals_b, c.I2,      c.I1,       c.sums,    c.tw,     c.tw_out,
-                  c.d_lags, c.perm,   c.bin_start, c.d_out, c.d_tmp,  c.d_flags,  c.d_tasks, c.d_groups, c.fft_cnt, c.d_claim, c.d_npairs, c.d_fit};
-  for (void* p : ptrs)
-    if (p) cudaFree(p);
+  for (const Ctx::Alloc& a : c.allocs) cudaFree(a.base);
+  c.allocs.clear();
   if (c.h_store) cudaFreeHost(c.h_store);
   c.h_store = nullptr;
   for (cudaEvent_t e : c.ev_pool) cudaEventDestroy(e);
@@ -303,7 +313,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   *out = nullptr;
   if (!lags_ok(lags, n_lags) || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
     return NFS_ERR_INVALID_ARG;
-  if ((flags & ~(unsigned)NFS_FLAG_BIN_ONLY) != 0) return NFS_ERR_INVALID_ARG;
+  if ((flags & ~(unsigned)(NFS_FLAG_BIN_ONLY | NFS_FLAG_GUARD)) != 0) return NFS_ERR_INVALID_ARG;
   if (!is_pow2(W) || !is_pow2(H) || W < 32 || H < 32 || W > 4096 || H > 4096) return NFS_ERR_INVALID_ARG;
   if (W != H) return NFS_ERR_UNSUPPORTED;
   if (n_lags > 65533) return NFS_ERR_INVALID_ARG;  // one grid row of the binning kernel per lag (+ I and V)
@@ -322,6 +332,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   c.B = batch_frames > 0 ? batch_frames : 1024;
   c.R = c.Lmax + c.B;
   c.bin_only = (flags & NFS_FLAG_BIN_ONLY) != 0;
+  c.guard = (flags & NFS_FLAG_GUARD) != 0;
   // band schedule: asked for by a ring capacity that cannot hold the whole lag window plus a batch
   if (ring_frames_cap < 0 || max_frames < 0) {
     delete h;
@@ -705,6 +716,27 @@ static int probe_impl(nfs_ctx* h, int batch_frames, int reps, double* ms_per_lau
 int nfs_probe_lag_traffic(nfs_ctx* h, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch) {
   NFS_GUARDED(probe_impl(h, batch_frames, reps, ms_per_launch, bytes_per_launch))
 }
+
+static int guards_impl(nfs_ctx* h, int64_t* n_bad) {
+  if (!h) return NFS_ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (!c.guard) return NFS_ERR_STATE;
+  if (!enter(c)) return c.status;
+  if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
+  std::vector<unsigned char> buf(kGuardBytes);
+  int64_t bad = 0;
+  for (const Ctx::Alloc& a : c.allocs) {
+    const char* base = static_cast<const char*>(a.base);
+    for (int side = 0; side < 2; ++side) {  // the zone in front of the buffer, then the one behind its 256-byte rounded end
+      if (!NFS_CUDA(c, cudaMemcpy(buf.data(), base + (side ? kGuardBytes + a.user_bytes : 0), kGuardBytes, cudaMemcpyDeviceToHost)))
+        return c.status;
+      for (unsigned char v : buf) bad += v != (unsigned char)kGuardByte;
+    }
+  }
+  if (n_bad) *n_bad = bad;
+  return bad == 0 ? NFS_OK : NFS_ERR_STATE;
+}
+int nfs_check_guards(nfs_ctx* h, int64_t* n_bad) { NFS_GUARDED(guards_impl(h, n_bad)) }
 
 int64_t nfs_num_frames(const nfs_ctx* h) { return h ? h->c.n_frames : 0; }
 int nfs_ring_capacity(const nfs_ctx* h) { return h ? h->c.R : 0; }

@@ -60,6 +60,12 @@ struct Ctx {
   int device = 0;
   int n_sm = 0;
   bool bin_only = false;  // accumulate |q|-binned totals only (no 2-D spectra kept)
+  bool guard = false;     // NFS_FLAG_GUARD: canary zones around every device buffer (nfs_check_guards)
+  struct Alloc {
+    void* base;         // what cudaMalloc returned
+    size_t user_bytes;  // the buffer's size rounded up to 256 bytes
+  };
+  std::vector<Alloc> allocs;
   // Out-of-core band schedule (Fig. 2(b) L37): the device holds only `ring cap` Fourier frames, fewer
   // than Lmax + batch.  The lags are cut into bands of band_width = N* lags (the paper's FIFO length); band 0 is
   // accumulated while the frames stream through the ring (the "first triangle" and its diagonal), every Fourier frame
