@@ -180,7 +180,11 @@ struct Plan {
   static constexpr int Li = two ? L / 32 : L;            // inner FFT length
   static constexpr int pitchO = T + Mi;                  // two-level: pitch of the 32 inner sequences
   static constexpr int foot = two ? 32 * pitchO : T * 33;  // float2 per FFT buffer
-  static constexpr int Sf = foot + ((2 - foot % 16) + 16) % 16;  // buffer stride == 2 (mod 16)
+  // buffer stride == 16 / (FFTs per item) (mod 16) float2: the transposed store reads element kx of every FFT of the
+  // item side by side, one 8-byte bank each within a half-warp
+  // (even, so that every buffer stays 16-byte aligned for the 128-bit staging stores)
+  static constexpr int padTo = Fc >= 8 ? 2 : (Fc >= 4 ? 4 : 8);
+  static constexpr int Sf = foot + ((padTo - foot % 16) + 16) % 16;
   static constexpr int n = L / 2;
   static constexpr int rowFfts = L / 2;                  // complex FFTs per frame in the row pass
   static constexpr int FcRow = Fc < rowFfts ? Fc : rowFfts;
@@ -482,7 +486,6 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
   const int tid = threadIdx.x;
   const int team = tid / P::T, tau = tid % P::T;
   float2* buf = sm + (size_t)team * P::Sf;
-  float2* nyq = sm + (size_t)P::Fc * P::Sf;  // [2 Fc]
   const unsigned total = (unsigned)(j.nf + P::Dr + P::Dc) * P::perStep;
   const size_t Pn = (size_t)(n + 1) * H;
 
@@ -579,23 +582,7 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
 #pragma unroll
       for (int r = 0; r < 32; ++r) buf[out_index<L>(tau, r)] = u[r];
       team_sync<P::T>(team);
-      // untangle the two real rows: A[k] = (Z[k] + conj Z[L-k]) / 2,  B[k] = (Z[k] - conj Z[L-k]) / (2i).
-      // In place: slot k <- A[k], slot L-k <- B[k] (1 <= k < n); slot 0 <- A[0], slot n <- B[0]; Nyquist aside.
-#pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        const int k = tau + P::T * i;
-        if (k == 0) {
-          const float2 z0 = buf[0], zh = buf[n];
-          buf[0] = make_float2(z0.x, 0.f);
-          buf[n] = make_float2(z0.y, 0.f);
-          nyq[2 * team] = make_float2(zh.x, 0.f);
-          nyq[2 * team + 1] = make_float2(zh.y, 0.f);
-        } else {
-          const float2 zk = buf[k], zm = buf[L - k];
-          buf[k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-          buf[L - k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-        }
-      }
+      // (the two real rows are untangled on the way out, below: no further pass over shared memory)
       // the intermediate slot must have been drained by the column pass of frame f - slots
       if (tid == 0 && pB) {
         spin_until(pB, tgtB, curB);
@@ -607,13 +594,17 @@ __global__ void __launch_bounds__(Plan<L>::NT, Plan<L>::minBlocks) k_fft(const F
       constexpr int FcR = P::FcRow;
       for (int e = tid; e < n * FcR; e += P::NT) {
         const int kxl = e & 1, ft = (e >> 1) % FcR, kx = 2 * (e / (2 * FcR)) + kxl;
+        // untangle the two real rows packed into one complex FFT: A[k] = (Z[k] + conj Z[L-k]) / 2,
+        // B[k] = (Z[k] - conj Z[L-k]) / (2i);  k = 0: A = Re Z[0], B = Im Z[0]
         const float2* b = sm + (size_t)ft * P::Sf;
-        const float2 A = b[kx], B = b[kx ? L - kx : n];
-        st_f4_hint(reinterpret_cast<float4*>(rowT + (size_t)kx * H + y0 + 2 * ft), make_float4(A.x, A.y, B.x, B.y), pol_evict_last());
+        const float2 zk = b[kx], zm = b[kx ? L - kx : 0];
+        const float4 v = kx ? make_float4(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y), 0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x))
+                            : make_float4(zk.x, 0.f, zk.y, 0.f);
+        st_f4_hint(reinterpret_cast<float4*>(rowT + (size_t)kx * H + y0 + 2 * ft), v, pol_evict_last());
       }
-      if (tid < FcR) {
-        *reinterpret_cast<float4*>(rowT + (size_t)n * H + y0 + 2 * tid) =
-            make_float4(nyq[2 * tid].x, nyq[2 * tid].y, nyq[2 * tid + 1].x, nyq[2 * tid + 1].y);
+      if (tid < FcR) {  // the Nyquist column: A = Re Z[n], B = Im Z[n]
+        const float2 zh = sm[(size_t)tid * P::Sf + n];
+        *reinterpret_cast<float4*>(rowT + (size_t)n * H + y0 + 2 * tid) = make_float4(zh.x, 0.f, zh.y, 0.f);
       }
       signal_count(&j.cnt[1 + j.nf + f]);
     } else {
