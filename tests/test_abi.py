@@ -105,6 +105,24 @@ def test_null_arguments(lib):
     assert lib.nfs_reset(None) == b.NFS_ERR_INVALID_ARG
     assert lib.nfs_num_frames(None) == 0
     assert lib.nfs_num_launches(None) == 0
+    # the calls added for the band schedule, sharding, the Eq. 1 fit and the measurement aids
+    assert lib.nfs_push_halo(None, None, 1) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_partials_count(None) == 0
+    assert lib.nfs_export_partials(None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_import_partials(None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_fit_eq1(None, None, None, None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_get_variance(None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_get_transfer_counts(None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_check_guards(None, None) == b.NFS_ERR_INVALID_ARG
+    assert lib.nfs_probe_lag_traffic(None, 26, 1, None, None) == b.NFS_ERR_INVALID_ARG
+    h = C.c_void_p()
+    lg = np.array([1, 2, 3], dtype=np.int32)
+    ptr = lg.ctypes.data_as(C.POINTER(C.c_int32))
+    assert lib.nfs_create_banded(C.byref(h), 64, 64, ptr, 3, 8, None, 0, 0, -1, 0) == b.NFS_ERR_INVALID_ARG   # negative ring cap
+    assert lib.nfs_create_banded(C.byref(h), 64, 64, ptr, 3, 8, None, 4, 0, 5, 0) == b.NFS_ERR_INVALID_ARG    # banded without max_frames
+    assert lib.nfs_create_banded(C.byref(h), 64, 64, ptr, 3, 8, None, 1, 1, 3, 100) == b.NFS_ERR_UNSUPPORTED  # banded + bin-only
+    assert lib.nfs_create_opts(C.byref(h), 64, 64, ptr, 3, 8, None, 0, 8) == b.NFS_ERR_INVALID_ARG            # unknown flag
+    assert not h.value
     lib.nfs_destroy(None)  # no-op
 
 

@@ -121,6 +121,14 @@ def test_sharded_contexts_equal_single_context(oracle, world, bin_only):
     outs = [nfs.finalize() + (nfs.variance(), nfs.pair_counts()) for nfs in ctxs]
     with pytest.raises(binding.NFSError):
         ctxs[0].push(st[:4])                            # merged sums: no more frames until reset
+    ctxs[0].reset()                                     # ... after which the context starts over
+    with pytest.raises(binding.NFSError):
+        ctxs[0].push_halo(st[:max(lags) + 1])           # a halo is at most Lmax frames
+    ctxs[0].push_halo(st[:5])
+    ctxs[0].push(st[5:40])
+    with pytest.raises(binding.NFSError):
+        ctxs[0].push_halo(st[40:44])                    # ... and only precedes the own frames
+    assert ctxs[0].pair_counts().tolist() == [max(0, 35 - max(0, t - 5)) for t in lags]
     for nfs in ctxs:
         nfs.close()
     nz = ref.counts > 0
