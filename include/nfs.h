@@ -222,8 +222,8 @@ NFS_API int nfs_get_kernel_times(nfs_ctx* ctx, double* ms, int64_t* launches);
 
 /* Measurement aid for bench.py (not part of the analysis): launches `reps` times a kernel with the memory access
  * pattern of ONE lag-accumulation launch over a batch of batch_frames frames — the 2-D TMA box copies of every pixel
- * tile's lag window into shared memory and two fp64 reductions (of 0.0: the accumulators keep their values) per
- * (lag, pixel) — without the arithmetic, and returns its mean duration (CUDA events on the context's stream) and the
+ * tile's lag window into shared memory and the kernel's fp64 reductions (one per (lag, pixel) for a batch of one chunk,
+ * two for longer batches; of 0.0: the accumulators keep their values) — without the arithmetic, and returns its mean duration (CUDA events on the context's stream) and the
  * algorithmic bytes P (8 (window + batch) + 16 n_lags) it moves: the ceiling of the access pattern on this device, to
  * which the real kernel's small-batch (HBM-bound) regime is compared.  Synchronises.  NFS_ERR_STATE for bin-only or
  * banded contexts. */

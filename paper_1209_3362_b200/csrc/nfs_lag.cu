@@ -354,17 +354,23 @@ __device__ __forceinline__ void sparse_masked_dispatch(int cnt, int ns, f2x (&ac
 // the totals when the segment opened, the second is the OLD row oend - g of the step after the last whole chunk (that
 // chunk's window is still resident: call before the chunk that follows is released), everything in fp64.
 template <int TPX>
-__device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* oldl, int oend, int DEPTH, double* tot,
-                                           int64_t P, int64_t p) {
+__device__ __forceinline__ void dense_fold(f2x (&acc)[kG], int cnt, const f2x* oldl, int oend, int oopen, int DEPTH,
+                                           double* tot, int64_t P, int64_t p) {
   double run = (double)f2x_sum(acc[0]);
   atomicAdd(&tot[p], run);
-  int r = oend;
+  int r = oend, r2 = oopen;
 #pragma unroll
   for (int g = 1; g < kG; ++g) {
     if (g < cnt) {
       if (--r < 0) r += DEPTH;
       const f2x z = oldl[(size_t)r * TPX];
       run -= 2.0 * (double)f2x_sum(acc[g]) + norm2_f64(make_float2(f2x_lo(z), f2x_hi(z)));
+      if (oopen >= 0) {  // one-chunk segment: the opening terms |z_{oopen - g}|^2 are still resident and join here (one
+                         // reduction per lag and pixel instead of two)
+        if (--r2 < 0) r2 += DEPTH;
+        const f2x y = oldl[(size_t)r2 * TPX];
+        run += norm2_f64(make_float2(f2x_lo(y), f2x_hi(y)));
+      }
       atomicAdd(&tot[(int64_t)g * P + p], run);
     }
   }
@@ -587,6 +593,7 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
   const int cend = min(nchunks, cseg + kFoldChunks);
   bool open = false;  // dense: whole chunks have been accumulated in this segment (their boundary terms are open)
   int oend = 0;       // dense: OLD row of the step after the segment's last whole chunk
+  int oopen = -1;     // dense, one-chunk segment: OLD row at its opening (the opening terms are added at the fold)
 #pragma unroll 1
   for (int c = cseg; c < cend; ++c) {
     if (!waited) mbar_wait(&full[st], ph);
@@ -598,6 +605,10 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
     if (j0 >= j_all && j0 + kChunk <= b) {
       // ---- fast chunk: every pair of every step exists ----
       if (dense) {
+        if (!open && cend - cseg == 1) {
+          open = true;
+          oopen = o0;  // the window of this one chunk is still resident at the fold
+        }
         if (!open) {
           // first whole chunk of the segment: the |z|^2 of the OLD frames just before it enter the totals of the
           // further lags (they telescope against the ones subtracted at the fold): lag tau0 + g gets
@@ -653,8 +664,9 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
         // iff u - g >= vbase and u < ns; straight into the fp64 totals (rare: the warm-up of a stack and the
         // ragged tail of a batch).  Rows o0 - (G-1) .. o0 + G-1 are contiguous thanks to the duplicated slot. ----
         if (open) {  // (not reached in practice: warm-up blocks precede the whole chunks) fold what is open first
-          if (p < P) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
+          if (p < P) dense_fold<TPX>(acc, cnt, oldl, oend, oopen, DEPTH, tot, P, p);
           open = false;
+          oopen = -1;
         }
         const int vbase = (int)max((int64_t)-64, (int64_t)tk.tau0 - t0 - jb);
         int rb = o0 - (G - 1);
@@ -700,7 +712,7 @@ __global__ void __launch_bounds__((NCW + 4) * 32, NCW <= 8 ? 2 : 1)
   // is fixed and the result deterministic.
   if (p < P) {
     if (dense) {
-      if (open) dense_fold<TPX>(acc, cnt, oldl, oend, DEPTH, tot, P, p);
+      if (open) dense_fold<TPX>(acc, cnt, oldl, oend, oopen, DEPTH, tot, P, p);
     } else {
 #pragma unroll
       for (int g = 0; g < G; ++g)

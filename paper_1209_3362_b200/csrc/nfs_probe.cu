@@ -1,8 +1,9 @@
 // nfs_probe.cu — measurement aid for bench.py (not on the hot path): the memory traffic of one small-batch launch of
 // the lag-accumulation kernel (step S5) WITHOUT its arithmetic.  Same access pattern as k_lag_tiled in
 // its HBM-bound regime: per pixel tile the window of LEAD + nchunks chunks is brought into shared memory by 2-D TMA
-// boxes (tile pixels x kChunk ring slots, mbarrier pipeline), and every (lag, pixel) of the fp64 totals receives two
-// RED.ADD.F64 (the value added is 0.0, so the totals are left as they are).  What this kernel reaches is the ceiling
+// boxes (tile pixels x kChunk ring slots, mbarrier pipeline), and every (lag, pixel) of the fp64 totals receives the
+// RED.ADD.F64 the kernel issues per launch (one for a batch of one chunk, two for longer batches: opening and fold of a
+// segment; the value added is 0.0, so the totals are left as they are).  What this kernel reaches is the ceiling
 // of the pattern on this device; k_lag_tiled's distance to it is what its arithmetic, folds and bookkeeping cost.
 #include "nfs_common.cuh"
 
@@ -46,7 +47,7 @@ constexpr int kProbeWarps = 8;  // consumer warps; warp kProbeWarps issues the c
 // persistent CTAs; CTA i takes the tiles i, i + gridDim.x, ...  V chunks per tile starting at ring slot s_first.
 template <int TPX>
 __global__ void __launch_bounds__((kProbeWarps + 1) * 32) k_lag_probe(const __grid_constant__ CUtensorMap tmap, int V, int s_first,
-                                                                      int ntiles, int n_lags, int64_t P,
+                                                                      int ntiles, int n_lags, int n_red, int64_t P,
                                                                       double* __restrict__ totals) {
   extern __shared__ __align__(1024) unsigned char smraw[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
@@ -84,14 +85,12 @@ __global__ void __launch_bounds__((kProbeWarps + 1) * 32) k_lag_probe(const __gr
       if (lane == 0) p_mbar_arrive(&empty[st]);
       if (++st == kProbeStages) st = 0, ph ^= 1u;
     }
-    // the totals of the tile: two reductions per (lag, pixel), as at the opening and the fold of a segment
+    // the totals of the tile: n_red reductions per (lag, pixel)
     for (int sub = 0; sub < TPX / 32; ++sub) {
       const int64_t p = (int64_t)tile * TPX + sub * 32 + lane;
       if (p < P)
-        for (int l = warp; l < n_lags; l += kProbeWarps) {
-          atomicAdd(&totals[(int64_t)l * P + p], 0.0);
-          atomicAdd(&totals[(int64_t)l * P + p], 0.0);
-        }
+        for (int l = warp; l < n_lags; l += kProbeWarps)
+          for (int k = 0; k < n_red; ++k) atomicAdd(&totals[(int64_t)l * P + p], 0.0);
     }
   }
   if (sink == 123456.789f) totals[0] += 1.0;  // keeps the shared-memory reads alive
@@ -108,13 +107,14 @@ int launch_lag_probe(Ctx& c, int b, double* bytes) {
   if (V * kChunk > c.R) V = c.R / kChunk;
   const size_t smem = 128 + (size_t)kProbeStages * kChunk * tpx * 8;
   const int grid = std::min(ntiles, std::max(1, c.n_sm) * (tpx == 64 ? 2 : 4));
+  const int n_red = b <= kChunk ? 1 : 2;
   if (bytes) *bytes = (double)c.P * (8.0 * V * kChunk + 16.0 * c.n_lags);
   if (tpx == 64) {
     if (!NFS_CUDA(c, cudaFuncSetAttribute(k_lag_probe<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return 0;
-    k_lag_probe<64><<<grid, (kProbeWarps + 1) * 32, smem, c.stream>>>(c.ring_map, V, 0, ntiles, c.n_lags, c.P, c.totals);
+    k_lag_probe<64><<<grid, (kProbeWarps + 1) * 32, smem, c.stream>>>(c.ring_map, V, 0, ntiles, c.n_lags, n_red, c.P, c.totals);
   } else {
     if (!NFS_CUDA(c, cudaFuncSetAttribute(k_lag_probe<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return 0;
-    k_lag_probe<32><<<grid, (kProbeWarps + 1) * 32, smem, c.stream>>>(c.ring_map, V, 0, ntiles, c.n_lags, c.P, c.totals);
+    k_lag_probe<32><<<grid, (kProbeWarps + 1) * 32, smem, c.stream>>>(c.ring_map, V, 0, ntiles, c.n_lags, n_red, c.P, c.totals);
   }
   NFS_CUDA(c, cudaGetLastError());
   return 1;
