@@ -51,7 +51,9 @@ typedef enum nfs_status {
                                Detected on the device, surfaced by the next synchronising call (sticky) */
   NFS_ERR_STATE = -5,       /* call not valid in this state (finalize before any frame; a 2-D difference
                                spectrum asked of a bin-only context)                                   */
-  NFS_ERR_UNSUPPORTED = -6  /* W != H (all of the paper's sizes, L33, are square)                      */
+  NFS_ERR_UNSUPPORTED = -6, /* W != H (all of the paper's sizes, L33, are square)                      */
+  NFS_ERR_TOO_LARGE = -7    /* nfs_azimuthal_mean_static only: n_qbins exceeds NFS_STATIC_MAX_QBINS, the size its
+                               fixed scratch array was built for                                       */
 } nfs_status;
 
 /*
@@ -252,6 +254,48 @@ NFS_API int nfs_set_launch_shape(nfs_ctx* ctx, int shape);
  * task's lag span exceeding shared memory). */
 NFS_API int nfs_plan_lags(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,
                           int cap);
+
+/*
+ * nfs_azimuthal_mean_static — the azimuthal average of step 5 ("azimuthally averaged power spectra";
+ * same |q| bins, DC exclusion and Hermitian weights as nfs_finalize) of ONE 2-D spectrum, for callers that are not
+ * allowed to allocate device memory.
+ *
+ * Why it exists.  Everything else in this header works on a context whose buffers nfs_create obtains with cudaMalloc.
+ * That is the wrong shape for three kinds of caller: a live acquisition loop, where a cudaMalloc / cudaFree stalls the
+ * whole device for an unpredictable time and so nothing on the per-frame path may allocate; a process whose device
+ * memory is owned in full by another allocator (a framework's caching pool, an arena sized at start-up, a MIG / MPS
+ * share with a hard cap), where a library-side cudaMalloc fails or eats into somebody else's budget; and plug-in
+ * code that is handed device pointers and a stream and told to leave the allocator alone.  This call needs no context
+ * and calls no cudaMalloc, cudaFree or allocating library routine, ever.  Its working memory is one array compiled into
+ * the library (NFS_STATIC_SCRATCH_BYTES, 2.3 MiB) — the price being that every GPU on which the library is loaded
+ * carries that array until the process ends, whether or not this call is used.
+ *
+ *   d_spec2d    DEVICE [H][W/2+1] double, the layout nfs_get_D2d / nfs_get_I2d / nfs_get_V2d return (ky in FFT order,
+ *               kx = 0..W/2), 8-byte aligned.  Read only.
+ *   W, H        powers of two in [32,4096], W == H (NFS_ERR_UNSUPPORTED otherwise).
+ *   n_qbins     1..NFS_STATIC_MAX_QBINS.  More bins than that do not fit the fixed array: the call returns
+ *               NFS_ERR_TOO_LARGE and does nothing (use a context, which sizes its own tables).
+ *   d_mean_q    DEVICE [n_qbins] double: mean of the spectrum over bin b, counting the mirrored half plane (0.0 for an
+ *               empty bin).
+ *   d_counts    DEVICE [n_qbins] int64 or NULL: full-plane pixel count of each bin.
+ *   cuda_stream a cudaStream_t cast to void* (NULL: the default stream).  Two kernels are enqueued on it and the call
+ *               returns without waiting; outputs are valid, and d_spec2d may be changed, once they have run.
+ * The device is the one current at the call.  The FIRST call on each device also looks up where the array lives on that
+ * device (cudaGetSymbolAddress, which may make the runtime load the library's code onto the GPU): make that first
+ * call during set-up, on every device you will use, and before any stream capture is begun.
+ * All calls on one device share the one array.  Nothing in it has to be zero beforehand — each call overwrites every
+ * slot it later reads, so leftovers of the previous call are harmless — but two calls whose kernels can run at the same
+ * time on the same device (different streams, no ordering between them) overwrite each other's partial sums: order
+ * them on one stream or with events.  Calls on different devices are independent.
+ * Results are deterministic (fixed summation order, no floating-point atomics) and agree with nfs_finalize's binning
+ * of the same spectrum to fp64 rounding; bin counts agree exactly.
+ * Returns NFS_OK, NFS_ERR_INVALID_ARG (NULL / misaligned pointer, bad size), NFS_ERR_UNSUPPORTED, NFS_ERR_TOO_LARGE, or
+ * NFS_ERR_CUDA (no device, launch failure).
+ */
+#define NFS_STATIC_MAX_QBINS 1024
+#define NFS_STATIC_SCRATCH_BYTES (148 * 2 * NFS_STATIC_MAX_QBINS * 8)
+NFS_API int nfs_azimuthal_mean_static(const double* d_spec2d, int W, int H, int n_qbins, double* d_mean_q, int64_t* d_counts,
+                                      void* cuda_stream);
 
 /* Forget all frames (accumulators, ring, reference, sticky errors); keeps the plan and the memory. */
 NFS_API int nfs_reset(nfs_ctx* ctx);

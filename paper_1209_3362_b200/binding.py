@@ -19,6 +19,8 @@ NFS_ERR_CUDA = -3
 NFS_ERR_ZERO_MEAN = -4
 NFS_ERR_STATE = -5
 NFS_ERR_UNSUPPORTED = -6
+NFS_ERR_TOO_LARGE = -7
+NFS_STATIC_MAX_QBINS = 1024
 
 # every symbol include/nfs.h declares: (name, restype, argtypes)
 _P = C.c_void_p
@@ -52,6 +54,7 @@ SYMBOLS = [
     ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
     ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
     ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
+    ("nfs_azimuthal_mean_static", C.c_int, [_P, C.c_int, C.c_int, C.c_int, _P, _P, _P]),
     ("nfs_reset", C.c_int, [_P]),
     ("nfs_destroy", None, [_P]),
     ("nfs_strerror", C.c_char_p, [C.c_int]),
@@ -166,6 +169,20 @@ def nfs_plan_lags(lags, n_px=1024 * 513, smem_per_sm=233472, smem_optin=232448, 
 
 def nfs_destroy(handle):
     load_library().nfs_destroy(handle)
+
+
+def nfs_azimuthal_mean_static(d_spec2d_ptr: int, W: int, H: int, n_qbins: int, d_mean_q_ptr: int, d_counts_ptr: int = 0,
+                              cuda_stream: int = 0):
+    """Azimuthal average of one device-resident [H][W/2+1] float64 spectrum into n_qbins |q| bins without any device
+    allocation (include/nfs.h).  It is meant for code that may not call cudaMalloc where it runs: per-frame analysis
+    loops, processes whose GPU memory is owned by another pool, plug-ins that only get pointers and a stream.  All
+    arguments are raw device addresses / a raw stream handle supplied by the caller; this wrapper allocates nothing
+    either.  n_qbins above NFS_STATIC_MAX_QBINS raises NFSError(NFS_ERR_TOO_LARGE).  Asynchronous on `cuda_stream`;
+    calls that may overlap on one device race on the library's fixed scratch array, so keep them stream ordered.  The
+    first call on a device does a one-time address lookup: make it during set-up."""
+    _check(load_library().nfs_azimuthal_mean_static(_P(d_spec2d_ptr), int(W), int(H), int(n_qbins), _P(d_mean_q_ptr),
+                                                    _P(d_counts_ptr) if d_counts_ptr else None,
+                                                    _P(cuda_stream) if cuda_stream else None))
 
 
 # ---- convenience wrapper ----------------------------------------------------------------------------------

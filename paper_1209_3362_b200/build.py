@@ -6,7 +6,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libnfs_b200.so")
-SOURCES = ["nfs_api.cu", "nfs_fft.cu", "nfs_lag.cu", "nfs_bin.cu", "nfs_probe.cu"]
+SOURCES = ["nfs_api.cu", "nfs_fft.cu", "nfs_lag.cu", "nfs_bin.cu", "nfs_probe.cu", "nfs_static.cu"]
 HEADERS = [os.path.join(CSRC, "nfs_common.cuh"), os.path.join(_HERE, "..", "include", "nfs.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -838,6 +838,7 @@ const char* nfs_strerror(int status) {
     case NFS_ERR_ZERO_MEAN: return "a pushed frame summed to zero: normalisation by the spatial mean is undefined";
     case NFS_ERR_STATE: return "call not valid in this state";
     case NFS_ERR_UNSUPPORTED: return "unsupported configuration (W != H)";
+    case NFS_ERR_TOO_LARGE: return "n_qbins exceeds NFS_STATIC_MAX_QBINS, the fixed scratch of nfs_azimuthal_mean_static";
     default: return "unknown status";
   }
 }
