@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <memory>
 #include <new>
 
 #include "nfs_common.cuh"
@@ -318,7 +319,16 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   if (W != H) return NFS_ERR_UNSUPPORTED;
   if (n_lags > 65533) return NFS_ERR_INVALID_ARG;  // one grid row of the binning kernel per lag (+ I and V)
 
-  nfs_ctx* h = new (std::nothrow) nfs_ctx();
+  // owned here until handed to the caller: every early return and a throwing host allocation (caught by NFS_GUARDED)
+  // release the device memory, the stream and the context itself
+  struct Release {
+    void operator()(nfs_ctx* p) const {
+      free_all(p->c);
+      delete p;
+    }
+  };
+  std::unique_ptr<nfs_ctx, Release> owner(new (std::nothrow) nfs_ctx());
+  nfs_ctx* h = owner.get();
   if (!h) return NFS_ERR_OOM;
   Ctx& c = h->c;
   c.W = W;
@@ -334,16 +344,12 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   c.bin_only = (flags & NFS_FLAG_BIN_ONLY) != 0;
   c.guard = (flags & NFS_FLAG_GUARD) != 0;
   // band schedule: asked for by a ring capacity that cannot hold the whole lag window plus a batch
-  if (ring_frames_cap < 0 || max_frames < 0) {
-    delete h;
-    return NFS_ERR_INVALID_ARG;
-  }
+  if (ring_frames_cap < 0 || max_frames < 0) return NFS_ERR_INVALID_ARG;
   if (ring_frames_cap > 0 && ring_frames_cap < c.Lmax + (batch_frames > 0 ? batch_frames : 1)) {
     int b = 0, nstar = 0;
-    if (c.bin_only || max_frames < 1 || !band_memory_plan(ring_frames_cap, batch_frames, &b, &nstar) || lags[0] > nstar) {
-      delete h;
-      return c.bin_only ? NFS_ERR_UNSUPPORTED : NFS_ERR_INVALID_ARG;
-    }
+    if (c.bin_only) return NFS_ERR_UNSUPPORTED;  // band schedule with bin-only accumulation
+    if (max_frames < 1 || !band_memory_plan(ring_frames_cap, batch_frames, &b, &nstar) || lags[0] > nstar)
+      return NFS_ERR_INVALID_ARG;
     c.B = b;
     c.band_width = nstar;
     c.R = nstar + b;  // the FIFO of the paper: the OLD window of one band plus a batch
@@ -420,14 +426,12 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   ok = ok && zero_state(c);
   ok = ok && NFS_CUDA(c, cudaStreamSynchronize(c.stream));
   if (ok) {
-    *out = h;
+    *out = owner.release();
     return NFS_OK;
   }
   const int st = (c.status != NFS_OK) ? c.status : NFS_ERR_CUDA;
   const bool oom = c.cuda_err.find("out of memory") != std::string::npos;
-  free_all(c);
-  delete h;
-  return oom ? NFS_ERR_OOM : st;
+  return oom ? NFS_ERR_OOM : st;  // `owner` frees everything
 }
 
 int get_plane(Ctx& c, double* out) {
