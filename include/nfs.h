@@ -15,6 +15,16 @@
  *   5. both are azimuthally averaged into n_qbins uniform |q| bins on [0, q_Nyquist),
  *      DC pixel excluded, bin index by exact integer arithmetic                (L25; R6, R7)
  *
+ * Accuracy.  Transforms and pair differences are fp32, partial sums are folded into fp64.  Binned D and
+ * I agree with the fp64 definition to 1e-4 relative, D2d per pixel to 1e-3 wherever D2d > 1e-6 of its maximum.  A lag
+ * that opens a run of consecutive requested lags (or stands alone) is summed directly and carries only its own relative
+ * rounding; the further lags of a run are built from their neighbour, and their ABSOLUTE error at pixel k is bounded by
+ *     1e-6 * Z(k) * E(k),   Z = max_t |F_t(k) - F_0(k)|,   E = max_t |F_t(k) - F_{t-1}(k)|,
+ * i.e. it scales with how far the stack has wandered from its first frame, not with D2d(k,tau) itself.  For stationary
+ * fluctuations (Z^2 of the order of the plateau) this is far inside the relative bars above; for a stack that drifts
+ * away from frame 0 by more than ~1000 frame-to-frame increments at a pixel, small-lag values there lose relative
+ * accuracy accordingly (request such lags as isolated lags, or reset and re-reference the context, if that matters).
+ *
  * Every step runs in hand-written CUDA kernels; there is no CPU fallback and no cuFFT.
  * One context = one CUDA device (the one current at nfs_create; later calls switch to it) = one CUDA
  * stream = not thread-safe; contexts are independent; no global state.
@@ -49,9 +59,10 @@ typedef enum nfs_status {
   NFS_ERR_CUDA = -3,        /* first failing CUDA call (sticky)                                        */
   NFS_ERR_ZERO_MEAN = -4,   /* a pushed frame summed to zero: its normalisation (L21) is undefined.
                                Detected on the device, surfaced by the next synchronising call (sticky) */
-  NFS_ERR_STATE = -5,       /* call not valid in this state (finalize before any frame; a 2-D difference
-                               spectrum asked of a bin-only context)                                   */
-  NFS_ERR_UNSUPPORTED = -6, /* W != H (all of the paper's sizes, L33, are square)                      */
+  NFS_ERR_STATE = -5,       /* call not valid in this state (finalize or a getter before any own frame — halo
+                               frames do not count; a 2-D difference spectrum asked of a bin-only context) */
+  NFS_ERR_UNSUPPORTED = -6, /* W != H (all of the paper's sizes, L33, are square); the band schedule asked
+                               for together with NFS_FLAG_BIN_ONLY                                     */
   NFS_ERR_TOO_LARGE = -7    /* nfs_azimuthal_mean_static only: n_qbins exceeds NFS_STATIC_MAX_QBINS, the size its
                                fixed scratch array was built for                                       */
 } nfs_status;
@@ -148,11 +159,16 @@ NFS_API int nfs_push_frames(nfs_ctx* ctx, const uint16_t* d_frames, int n);
  *   nfs_export_partials d_buf DEVICE [nfs_partials_count]: the context's sums in a form that adds up over contexts:
  *                      pair sums per lag and pixel (per lag and |q| bin for NFS_FLAG_BIN_ONLY), sum |F_t|^2 and
  *                      sum F_t over the own frames (absolute: independent of the context's reference frame), pair
- *                      counts per lag, own-frame count.  Synchronises the stream.
+ *                      counts per lag, own-frame count.  Synchronises the stream.  A context without own frames (the
+ *                      rank of an empty time chunk, or one that has only seen its halo) exports zeros, so that it can
+ *                      take part in the all-reduce like every other rank; it may import the total as well.
  *   nfs_import_partials d_buf DEVICE: replaces the context's sums by the buffer's — the caller has added the buffers
  *                      of all contexts (one all-reduce(sum), e.g. ncclAllReduce over NVLink).
  *                      Afterwards nfs_finalize and the getters return the result of the whole stack (counts and
- *                      divisors come from the buffer); pushing more frames returns NFS_ERR_STATE until nfs_reset.
+ *                      divisors come from the buffer); pushing more frames, exporting, and a second import return
+ *                      NFS_ERR_STATE until nfs_reset.
+ * Export and import return NFS_ERR_STATE on a context created with a band schedule (nfs_create_banded with a binding
+ * ring_frames_cap): the two ways of handling a stack that does not fit one device's memory are not combined.
  */
 NFS_API int nfs_push_halo(nfs_ctx* ctx, const uint16_t* d_frames, int n);
 NFS_API int64_t nfs_partials_count(const nfs_ctx* ctx);

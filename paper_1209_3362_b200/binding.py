@@ -242,19 +242,30 @@ class NFS:
         _check(self.lib.nfs_push_halo(self.handle, _P(frames.data_ptr()), int(frames.shape[0])), self.handle)
 
     def export_partials(self):
-        """The context's partial sums as a float64 torch tensor on its device (ready for all_reduce)."""
+        """The context's partial sums as a float64 torch tensor on the context's device (ready for all_reduce).  The
+        buffer is allocated on the context's stream, where the library writes it; nfs_export_partials synchronises that
+        stream before it returns, and the tensor is then marked as in use on torch's current stream, where the caller
+        will read it."""
         import torch
 
-        buf = torch.empty(int(self.lib.nfs_partials_count(self.handle)), dtype=torch.float64, device="cuda")
+        n = int(self.lib.nfs_partials_count(self.handle))
+        with torch.cuda.stream(self._stream):
+            buf = torch.empty(n, dtype=torch.float64, device=self._stream.device)
         _check(self.lib.nfs_export_partials(self.handle, _P(buf.data_ptr())), self.handle)
+        buf.record_stream(torch.cuda.current_stream(buf.device))
         return buf
 
     def import_partials(self, buf):
+        """`buf`: the sum over all contexts of their exported buffers (the caller's all-reduce, enqueued on torch's
+        current stream): the context's stream is ordered after that stream, no host synchronisation of it."""
         import torch
 
         assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous()
         assert buf.numel() == int(self.lib.nfs_partials_count(self.handle))
-        torch.cuda.current_stream(buf.device).synchronize()   # the caller's all-reduce ran on torch's stream
+        cur = torch.cuda.current_stream(buf.device)
+        if cur != self._stream:
+            self._stream.wait_stream(cur)
+            buf.record_stream(self._stream)
         _check(self.lib.nfs_import_partials(self.handle, _P(buf.data_ptr())), self.handle)
 
     def push_ptr(self, ptr, n):

@@ -449,7 +449,7 @@ int ready(nfs_ctx* h) {
   if (!h) return NFS_ERR_INVALID_ARG;
   Ctx& c = h->c;
   if (!enter(c)) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
+  if (frames_in_I(c) < 1) return NFS_ERR_STATE;  // no frame yet, or only halo frames: every average would be 0 / 0
   if (!flush_pending(c)) return c.status;
   if (!run_band_sweeps(c)) return c.status;
   return NFS_OK;
@@ -567,18 +567,25 @@ int64_t nfs_partials_count(const nfs_ctx* h) {
   return (int64_t)c.n_lags * partials_rows(c) + 3 * c.P + c.n_lags + 1;
 }
 static int export_impl(nfs_ctx* h, double* d_buf) {
-  if (!d_buf) return NFS_ERR_INVALID_ARG;
-  const int rc = ready(h);
-  if (rc != NFS_OK) return rc;
+  if (!h || !d_buf) return NFS_ERR_INVALID_ARG;
   Ctx& c = h->c;
-  if (c.merged) return NFS_ERR_STATE;
+  if (!enter(c)) return c.status;
+  if (c.band_width > 0 || c.merged) return NFS_ERR_STATE;  // not combined with the band schedule; sums already replaced
+  if (!flush_pending(c)) return c.status;
   const size_t nA = (size_t)c.n_lags * (size_t)partials_rows(c);
+  const int64_t own = frames_in_I(c);
+  if (own == 0) {
+    // a rank whose time chunk is empty (more ranks than frames), or which has seen only halo frames, contributes
+    // nothing: an all-zero buffer with frame count 0, so that it can still take part in the all-reduce
+    if (!NFS_CUDA(c, cudaMemsetAsync(d_buf, 0, sizeof(double) * (size_t)nfs_partials_count(h), c.stream))) return c.status;
+    return sync_and_check(c);
+  }
   if (!NFS_CUDA(c, cudaMemcpyAsync(d_buf, c.bin_only ? c.totals_b : c.totals, sizeof(double) * nA, cudaMemcpyDeviceToDevice, c.stream)))
     return c.status;
   c.n_launches += launch_absolute_I(c, d_buf + nA, reinterpret_cast<double2*>(d_buf + nA + c.P));
   std::vector<double> tail((size_t)c.n_lags + 1);
   for (int l = 0; l < c.n_lags; ++l) tail[(size_t)l] = (double)pair_count(c, l);  // exact: counts < 2^53
-  tail[(size_t)c.n_lags] = (double)frames_in_I(c);
+  tail[(size_t)c.n_lags] = (double)own;
   if (!NFS_CUDA(c, cudaMemcpyAsync(d_buf + nA + 3 * c.P, tail.data(), sizeof(double) * tail.size(), cudaMemcpyHostToDevice, c.stream)))
     return c.status;
   return sync_and_check(c);
@@ -589,7 +596,10 @@ static int import_impl(nfs_ctx* h, const double* d_buf) {
   if (!h || !d_buf) return NFS_ERR_INVALID_ARG;
   Ctx& c = h->c;
   if (!enter(c)) return c.status;
-  if (c.n_frames < 1) return NFS_ERR_STATE;
+  // once per context (a second import would silently replace sums whose counts no longer describe the ring), and not
+  // for the band schedule, whose bands >= 1 are rebuilt from the host store at every finalize
+  // (a context without any frame may import: the rank of an empty time chunk receives the whole result like the others)
+  if (c.merged || c.band_width > 0) return NFS_ERR_STATE;
   if (!flush_pending(c)) return c.status;
   const size_t nA = (size_t)c.n_lags * (size_t)partials_rows(c);
   std::vector<double> tail((size_t)c.n_lags + 1);
@@ -701,8 +711,12 @@ static int probe_impl(nfs_ctx* h, int batch_frames, int reps, double* ms_per_lau
   Ctx& c = h->c;
   if (!enter(c)) return c.status;
   if (c.bin_only || c.band_width > 0) return NFS_ERR_STATE;
-  cudaEvent_t e0, e1;
-  if (!NFS_CUDA(c, cudaEventCreate(&e0)) || !NFS_CUDA(c, cudaEventCreate(&e1))) return c.status;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (!NFS_CUDA(c, cudaEventCreate(&e0))) return c.status;
+  if (!NFS_CUDA(c, cudaEventCreate(&e1))) {
+    cudaEventDestroy(e0);
+    return c.status;
+  }
   double bytes = 0.0;
   launch_lag_probe(c, batch_frames, &bytes);  // warm-up
   NFS_CUDA(c, cudaEventRecord(e0, c.stream));
@@ -841,7 +855,7 @@ const char* nfs_strerror(int status) {
     case NFS_ERR_CUDA: return "CUDA error (see nfs_last_cuda_error)";
     case NFS_ERR_ZERO_MEAN: return "a pushed frame summed to zero: normalisation by the spatial mean is undefined";
     case NFS_ERR_STATE: return "call not valid in this state";
-    case NFS_ERR_UNSUPPORTED: return "unsupported configuration (W != H)";
+    case NFS_ERR_UNSUPPORTED: return "unsupported configuration (W != H, or the band schedule together with NFS_FLAG_BIN_ONLY)";
     case NFS_ERR_TOO_LARGE: return "n_qbins exceeds NFS_STATIC_MAX_QBINS, the fixed scratch of nfs_azimuthal_mean_static";
     default: return "unknown status";
   }

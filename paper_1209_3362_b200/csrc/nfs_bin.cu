@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(128) k_bin(const double* __restrict__ totals, 
     const long long np = npairs[row];  // frame pairs accumulated at this lag (N - tau for a whole stack on one context)
     inv = np > 0 ? 1.0 / (double)np : 0.0;
   } else {
-    inv = 1.0 / (double)N;  // N: frames in the I sums
+    inv = N > 0 ? 1.0 / (double)N : 0.0;  // N: frames in the I sums
   }
   double acc = 0.0, wsum = 0.0;
   for (int i = beg + (int)threadIdx.x; i < end; i += 128) {

@@ -29,7 +29,8 @@ class Shard:
 
 def shard_plan(n_frames: int, world: int, lag_max: int):
     """Contiguous time chunks of (almost) equal length, each preceded by a halo of min(lag_max, frames before it)
-    frames.  Ranks beyond the number of frames get an empty chunk."""
+    frames.  With more ranks than frames some chunks are empty (own_start == own_end); such a rank pushes nothing, and
+    merge() still works on it: its context exports zeros and imports the total (include/nfs.h)."""
     assert n_frames >= 1 and world >= 1 and lag_max >= 1
     out = []
     for g in range(world):

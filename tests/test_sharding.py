@@ -141,3 +141,48 @@ def test_sharded_contexts_equal_single_context(oracle, world, bin_only):
         assert np.max(np.abs(V[nz] - V1[nz]) / V1[nz]) < 1e-4
     for o in outs[1:]:
         assert all(np.array_equal(a, b) for a, b in zip(o, outs[0])), "every rank returns the same result"
+
+
+@pytest.mark.gpu
+def test_more_ranks_than_frames_and_halo_only_contexts(oracle):
+    """with fewer frames than ranks some time chunks are empty.  Such a rank must still get through the one
+    collective (its export is all zeros, frame count 0) and hold the whole result afterwards; a context that has seen
+    only halo frames has no average to give (NFS_ERR_STATE, not NaN)."""
+    from paper_1209_3362_b200 import binding
+
+    assert torch.cuda.is_available()
+    lags = [1, 2]
+    cfg = synth.config(0, W=64, N=3, lags=lags, n_qbins=16)
+    st = synth.make_stack(cfg, "cuda")
+    ref = oracle.structure_function(st.cpu().numpy(), lags, cfg.n_qbins)
+    plan = sharding.shard_plan(cfg.N, 4, max(lags))
+    assert [s.n_own for s in plan] == [0, 1, 1, 1]
+    ctxs = [binding.NFS(cfg.W, cfg.H, lags, cfg.n_qbins) for _ in plan]
+    for nfs, sh in zip(ctxs, plan):
+        sharding.push_shard(nfs, st, sh)
+    with pytest.raises(binding.NFSError) as e:
+        ctxs[0].finalize()                                  # nothing pushed
+    assert e.value.status == binding.NFS_ERR_STATE
+    bufs = [nfs.export_partials() for nfs in ctxs]
+    assert float(bufs[0].abs().max()) == 0.0
+    total = torch.stack(bufs).sum(dim=0)
+    for nfs in ctxs:
+        nfs.import_partials(total.clone())
+    with pytest.raises(binding.NFSError) as e:
+        ctxs[1].import_partials(total.clone())              # once per context
+    assert e.value.status == binding.NFS_ERR_STATE
+    nz = ref.counts > 0
+    for nfs in ctxs:
+        D, I_q, cnt = nfs.finalize()
+        assert nfs.pair_counts().tolist() == [2, 1]
+        assert np.max(np.abs(D[:, nz] - ref.D[:, nz]) / ref.D[:, nz]) < 1e-4
+        assert np.max(np.abs(I_q[nz] - ref.I_q[nz]) / ref.I_q[nz]) < 1e-4
+        nfs.close()
+    halo_only = binding.NFS(cfg.W, cfg.H, lags, cfg.n_qbins)
+    halo_only.push_halo(st[:2])
+    for call in (halo_only.finalize, halo_only.I2d, halo_only.variance):
+        with pytest.raises(binding.NFSError) as e:
+            call()
+        assert e.value.status == binding.NFS_ERR_STATE
+    assert float(halo_only.export_partials().abs().max()) == 0.0
+    halo_only.close()
