@@ -517,7 +517,7 @@ def run_e2e(torch, nfs, stack, cfg, stream, dev, args, dist, world):
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    steps = max(1, min(args.steps, 3))
+    steps = max(1, args.steps)  # the same number of steps as the device-timed headline
     t = time.time()
     for _ in range(steps):
         D, I, cnt = step()
