@@ -279,6 +279,7 @@ def run_ours(args, cfg):
     import synth
     from paper_1209_3362_b200 import binding
 
+    binding.use_dev_library()  # per-kernel timing, launch counts, the traffic probe: include/nfs_dev.h (same kernels)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))

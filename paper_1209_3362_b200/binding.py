@@ -2,7 +2,12 @@
 
 Same names as the C ABI: nfs_create / nfs_push_frames / nfs_finalize / getters, plus a small
 `NFS` convenience class.  torch is used only for device memory and streams.  There is no CPU
-fallback: if libnfs_b200.so is missing or does not load, importing this module raises.
+fallback: if the library is missing or does not load, load_library() raises.
+
+Two builds of the same object files exist (paper_1209_3362_b200/build.py): libnfs_b200.so exports include/nfs.h and is
+what this module loads by default; libnfs_b200_dev.so additionally exports the measurement / debugging aids of
+include/nfs_dev.h (per-kernel timing, launch counts, guard zones, plan introspection, the traffic probe) and is loaded
+instead after use_dev_library() — the tests (tests/conftest.py) and bench.py do that before they create a context.
 """
 import ctypes as C
 import os
@@ -11,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnfs_b200.so")
+DEV_LIB_PATH = os.path.join(_HERE, "libnfs_b200_dev.so")
 
 NFS_OK = 0
 NFS_ERR_INVALID_ARG = -1
@@ -31,7 +37,6 @@ SYMBOLS = [
     ("nfs_create_banded", C.c_int, [C.POINTER(_P), C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int, C.c_int, _P, C.c_int, C.c_uint,
                                     C.c_int, C.c_int64]),
     ("nfs_get_transfer_counts", C.c_int, [_P, C.POINTER(C.c_int64)]),
-    ("nfs_band_plan", C.c_int, [C.c_int64, C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]),
     ("nfs_push_frames", C.c_int, [_P, _P, C.c_int]),
     ("nfs_push_halo", C.c_int, [_P, _P, C.c_int]),
     ("nfs_partials_count", C.c_int64, [_P]),
@@ -44,21 +49,25 @@ SYMBOLS = [
     ("nfs_get_variance", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_get_V2d", C.c_int, [_P, C.POINTER(C.c_double)]),
     ("nfs_fit_eq1", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]),
-    ("nfs_probe_lag_traffic", C.c_int, [_P, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
-    ("nfs_check_guards", C.c_int, [_P, C.POINTER(C.c_int64)]),
     ("nfs_num_frames", C.c_int64, [_P]),
     ("nfs_ring_capacity", C.c_int, [_P]),
     ("nfs_device_bytes", C.c_int64, [_P]),
-    ("nfs_num_launches", C.c_int64, [_P]),
-    ("nfs_set_launch_shape", C.c_int, [_P, C.c_int]),
-    ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
-    ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
-    ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     ("nfs_azimuthal_mean_static", C.c_int, [_P, C.c_int, C.c_int, C.c_int, _P, _P, _P]),
     ("nfs_reset", C.c_int, [_P]),
     ("nfs_destroy", None, [_P]),
     ("nfs_strerror", C.c_char_p, [C.c_int]),
     ("nfs_last_cuda_error", C.c_char_p, [_P]),
+]
+# include/nfs_dev.h: exported by libnfs_b200_dev.so only
+DEV_SYMBOLS = [
+    ("nfs_band_plan", C.c_int, [C.c_int64, C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64)]),
+    ("nfs_probe_lag_traffic", C.c_int, [_P, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    ("nfs_check_guards", C.c_int, [_P, C.POINTER(C.c_int64)]),
+    ("nfs_num_launches", C.c_int64, [_P]),
+    ("nfs_set_launch_shape", C.c_int, [_P, C.c_int]),
+    ("nfs_plan_lags", C.c_int, [C.POINTER(C.c_int32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int32), C.c_int]),
+    ("nfs_set_profiling", C.c_int, [_P, C.c_int]),
+    ("nfs_get_kernel_times", C.c_int, [_P, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
 ]
 
 KERNEL_CLASSES = ["ref_setup", "fft", "unused", "lag_accum", "bin"]
@@ -67,23 +76,43 @@ NFS_FLAG_GUARD = 2
 SHAPE_AUTO, SHAPE_ONE_TILE, SHAPE_PERSISTENT = 0, 1, 2
 
 _lib = None
+_use_dev = False
 
 
-def load_library(path: str = LIB_PATH):
+def use_dev_library():
+    """From now on load_library() returns libnfs_b200_dev.so (include/nfs.h + include/nfs_dev.h).  Call it before the
+    first context is created: a context belongs to the library that created it."""
+    global _lib, _use_dev
+    if not _use_dev:
+        _use_dev = True
+        _lib = None
+
+
+def load_library(path: str = None):
     """Loads the C-ABI library; raises (never falls back) if it is missing."""
     global _lib
     if _lib is None:
+        path = path or (DEV_LIB_PATH if _use_dev else LIB_PATH)
         if not os.path.exists(path):
             raise ImportError(
                 "%s not found: build it with `python -m paper_1209_3362_b200.build` "
                 "(there is no CPU fallback for the hot path)" % path)
         lib = C.CDLL(path)
-        for name, res, args in SYMBOLS:
+        for name, res, args in SYMBOLS + (DEV_SYMBOLS if _use_dev else []):
             fn = getattr(lib, name)  # AttributeError if the symbol is not exported
             fn.restype = res
             fn.argtypes = args
         _lib = lib
     return _lib
+
+
+def _dev_fn(name):
+    """A function of include/nfs_dev.h; a clear error if the product library is the one loaded."""
+    lib = load_library()
+    if not _use_dev:
+        raise RuntimeError("%s is a measurement / debugging aid (include/nfs_dev.h) that libnfs_b200.so does not export: "
+                           "call binding.use_dev_library() before creating contexts" % name)
+    return getattr(lib, name)
 
 
 class NFSError(RuntimeError):
@@ -125,7 +154,7 @@ def nfs_band_plan(n_frames, lags, ring_frames_cap, batch_frames=0):
     new_uploads, launches)."""
     lg = np.ascontiguousarray(lags, dtype=np.int32)
     out = np.zeros(6, dtype=np.int64)
-    _check(load_library().nfs_band_plan(int(n_frames), _dp(lg, C.c_int32), int(lg.size), int(ring_frames_cap), int(batch_frames),
+    _check(_dev_fn("nfs_band_plan")(int(n_frames), _dp(lg, C.c_int32), int(lg.size), int(ring_frames_cap), int(batch_frames),
                                         _dp(out, C.c_int64)))
     return dict(zip(("bands", "band_width", "batch", "old_uploads", "new_uploads", "launches"), (int(v) for v in out)))
 
@@ -148,7 +177,7 @@ def nfs_plan_lags(lags, n_px=1024 * 513, smem_per_sm=233472, smem_optin=232448, 
     lags = np.ascontiguousarray(lags, dtype=np.int32)
     cap = 7 + 27 * (len(lags) + 1)
     out = np.zeros(cap, dtype=np.int32)
-    n = load_library().nfs_plan_lags(_dp(lags, C.c_int32), len(lags), int(n_px), int(smem_per_sm), int(smem_optin), int(n_sm),
+    n = _dev_fn("nfs_plan_lags")(_dp(lags, C.c_int32), len(lags), int(n_px), int(smem_per_sm), int(smem_optin), int(n_sm),
                                      _dp(out, C.c_int32), cap)
     if n < 0:
         raise NFSError(n)
@@ -308,28 +337,28 @@ class NFS:
     def probe_lag_traffic(self, batch_frames, reps=20):
         """(ms per launch, algorithmic bytes per launch) of the lag kernel's memory access pattern without its arithmetic."""
         ms, by = C.c_double(0.0), C.c_double(0.0)
-        _check(self.lib.nfs_probe_lag_traffic(self.handle, int(batch_frames), int(reps), C.byref(ms), C.byref(by)), self.handle)
+        _check(_dev_fn("nfs_probe_lag_traffic")(self.handle, int(batch_frames), int(reps), C.byref(ms), C.byref(by)), self.handle)
         return ms.value, by.value
 
     def check_guards(self):
         """Overwritten guard bytes around the context's device buffers (0 = intact); needs guard=True at creation."""
         n = C.c_int64(0)
-        rc = self.lib.nfs_check_guards(self.handle, C.byref(n))
+        rc = _dev_fn("nfs_check_guards")(self.handle, C.byref(n))
         if rc not in (NFS_OK, NFS_ERR_STATE) or (rc == NFS_ERR_STATE and n.value == 0):
             _check(rc, self.handle)
         return int(n.value)
 
     def set_launch_shape(self, shape):
-        _check(self.lib.nfs_set_launch_shape(self.handle, int(shape)), self.handle)
+        _check(_dev_fn("nfs_set_launch_shape")(self.handle, int(shape)), self.handle)
 
     def set_profiling(self, enable):
-        _check(self.lib.nfs_set_profiling(self.handle, int(bool(enable))), self.handle)
+        _check(_dev_fn("nfs_set_profiling")(self.handle, int(bool(enable))), self.handle)
 
     def kernel_times(self):
         """-> dict class -> (milliseconds, launches) since the last call (synchronises)."""
         ms = np.zeros(len(KERNEL_CLASSES), dtype=np.float64)
         n = np.zeros(len(KERNEL_CLASSES), dtype=np.int64)
-        _check(self.lib.nfs_get_kernel_times(self.handle, _dp(ms, C.c_double), _dp(n, C.c_int64)), self.handle)
+        _check(_dev_fn("nfs_get_kernel_times")(self.handle, _dp(ms, C.c_double), _dp(n, C.c_int64)), self.handle)
         return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     def reset(self):
@@ -341,7 +370,7 @@ class NFS:
 
     @property
     def num_launches(self):
-        return int(self.lib.nfs_num_launches(self.handle))
+        return int(_dev_fn("nfs_num_launches")(self.handle))
 
     @property
     def ring_capacity(self):

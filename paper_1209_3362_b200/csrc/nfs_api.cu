@@ -13,10 +13,6 @@
 
 using namespace nfs;
 
-struct nfs_ctx {
-  Ctx c;
-};
-
 namespace {
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -25,8 +21,6 @@ bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 // kGuardBytes filled with a canary byte, which nfs_check_guards reads back: an out-of-bounds write of any kernel next
 // to one of the library's buffers is then detected (the substitute for compute-sanitizer memcheck where that tool is
 // not available).
-constexpr size_t kGuardBytes = 64 << 10;
-constexpr int kGuardByte = 0xA5;
 template <typename T>
 bool dev_alloc(Ctx& c, T** p, size_t count) {
   void* q = nullptr;
@@ -187,15 +181,6 @@ bool zero_state(Ctx& c) {
   return ok;
 }
 
-// every entry point that touches the device runs on the context's device
-bool enter(Ctx& c) {
-  if (c.status != NFS_OK) return false;
-  int dev = -1;
-  if (!NFS_CUDA(c, cudaGetDevice(&dev))) return false;
-  if (dev != c.device && !NFS_CUDA(c, cudaSetDevice(c.device))) return false;
-  return true;
-}
-
 // synchronise and surface device-side flags
 int sync_and_check(Ctx& c) {
   if (c.status != NFS_OK) return c.status;
@@ -211,46 +196,6 @@ void ring_to_plane(const Ctx& c, const double* src, double* out) {
   const int n = c.n, H = c.H;
   for (int y = 0; y < H; ++y)
     for (int x = 0; x <= n; ++x) out[(size_t)y * (n + 1) + x] = src[(size_t)x * H + y];
-}
-
-// ---- out-of-core band schedule (Fig. 2(b) L37) ----------------------------------------------------
-// Memory plan for a device that holds only `cap` Fourier frames: batch b, band width N* = cap - 2 b (a window of
-// N* + b OLD frames and b NEW frames).  Returns false if no band fits.
-bool band_memory_plan(int cap, int batch_frames, int* b_out, int* nstar_out) {
-  int b = batch_frames > 0 ? batch_frames : std::min(1024, cap / 4);
-  b = std::max(1, std::min(b, 8192));
-  const int nstar = cap - 2 * b;
-  if (nstar < 1) return false;
-  *b_out = b;
-  *nstar_out = nstar;
-  return true;
-}
-
-// The sweeps of bands 1 .. n_bands-1 over a stack of N frames, as a sequence of uploads and launches.  Band k holds
-// the requested lags in (k N*, (k+1) N*], smallest tmin, largest tmax.  Its sweep walks the frames s = tmin .. N-1 in
-// batches of b: the batch goes into the NEW ring, the OLD frames s - tmax .. s - tmin it pairs with are kept in the
-// OLD ring, every frame of the window being uploaded once per band (the paper's FIFO: "one diagonal is filled by
-// subsequently replacing one FIFO image and uploading one 'current image'").  The same walk serves the device (uploads
-// and kernel launches) and the host-only transfer count of nfs_band_plan.
-template <typename UploadOld, typename UploadNew, typename Launch>
-bool band_sweeps(int64_t N, int b, int n_bands, const std::vector<int>& band_l0, const std::vector<int32_t>& lags,
-                 UploadOld&& upload_old, UploadNew&& upload_new, Launch&& launch) {
-  for (int k = 1; k < n_bands; ++k) {
-    const int l0 = band_l0[(size_t)k], l1 = band_l0[(size_t)k + 1];
-    if (l1 <= l0) continue;  // no requested lag in this band
-    const int64_t tmin = lags[(size_t)l0], tmax = lags[(size_t)l1 - 1];
-    int64_t old_next = -1;  // first OLD frame not yet in the OLD ring
-    for (int64_t t0 = tmin; t0 < N; t0 += b) {
-      const int bb = (int)std::min<int64_t>(b, N - t0);
-      const int64_t lo = std::max<int64_t>(0, t0 - tmax), hi = t0 + bb - 1 - tmin;  // OLD frames lo .. hi
-      const int64_t from = std::max(lo, old_next);
-      if (hi >= from && !upload_old(from, hi + 1)) return false;
-      old_next = std::max(old_next, hi + 1);
-      if (!upload_new(t0, t0 + bb)) return false;
-      if (!launch(t0, bb, k)) return false;
-    }
-  }
-  return true;
 }
 
 // frames [f0, f1) between a ring of `slots` frames at `base` (slot = frame mod slots) and the pinned host store
@@ -298,13 +243,6 @@ bool flush_pending(Ctx& c) {
   if (!NFS_CUDA(c, cudaGetLastError())) return false;
   if (c.status != NFS_OK) return false;
   c.n_acc = c.n_frames;
-  return true;
-}
-
-bool lags_ok(const int32_t* lags, int n_lags) {
-  if (!lags || n_lags < 1) return false;
-  for (int l = 0; l < n_lags; ++l)
-    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return false;
   return true;
 }
 
@@ -457,16 +395,6 @@ int ready(nfs_ctx* h) {
 
 }  // namespace
 
-// Nothing may throw across the C boundary: allocation failures of the host-side containers become NFS_ERR_OOM.
-#define NFS_GUARDED(expr)            \
-  try {                              \
-    return (expr);                   \
-  } catch (const std::bad_alloc&) {  \
-    return NFS_ERR_OOM;              \
-  } catch (...) {                    \
-    return NFS_ERR_STATE;            \
-  }
-
 extern "C" {
 
 int nfs_create_opts(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
@@ -487,26 +415,6 @@ int nfs_get_transfer_counts(const nfs_ctx* h, int64_t* out) {
   out[2] = c.h2d_frames;
   out[3] = c.d2h_frames;
   return NFS_OK;
-}
-
-static int band_plan_impl(int64_t n_frames, const int32_t* lags, int n_lags, int ring_frames_cap, int batch_frames, int64_t* out) {
-  if (!lags_ok(lags, n_lags) || !out || n_frames < 1 || ring_frames_cap < 1) return NFS_ERR_INVALID_ARG;
-  int b = 0, nstar = 0;
-  if (!band_memory_plan(ring_frames_cap, batch_frames, &b, &nstar) || lags[0] > nstar) return NFS_ERR_INVALID_ARG;
-  const int n_bands = (lags[n_lags - 1] - 1) / nstar + 1;
-  std::vector<int32_t> L(lags, lags + n_lags);
-  std::vector<int> l0((size_t)n_bands + 1, n_lags);
-  for (int l = n_lags - 1; l >= 0; --l)
-    for (int k = 0; k <= (L[(size_t)l] - 1) / nstar; ++k) l0[(size_t)k] = l;
-  int64_t up_old = 0, up_new = 0, launches = 0;
-  band_sweeps(
-      n_frames, b, n_bands, l0, L, [&](int64_t f0, int64_t f1) { up_old += f1 - f0; return true; },
-      [&](int64_t f0, int64_t f1) { up_new += f1 - f0; return true; }, [&](int64_t, int, int) { ++launches; return true; });
-  out[0] = n_bands, out[1] = nstar, out[2] = b, out[3] = up_old, out[4] = up_new, out[5] = launches;
-  return NFS_OK;
-}
-int nfs_band_plan(int64_t n_frames, const int32_t* lags, int n_lags, int ring_frames_cap, int batch_frames, int64_t* out) {
-  NFS_GUARDED(band_plan_impl(n_frames, lags, n_lags, ring_frames_cap, batch_frames, out))
 }
 
 int nfs_create_ex(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, int n_qbins, void* cuda_stream,
@@ -706,127 +614,9 @@ int nfs_fit_eq1(nfs_ctx* h, double* A_q, double* C_q, double* Gamma_q, double* c
   NFS_GUARDED(fit_impl(h, A_q, C_q, Gamma_q, chi2_q))
 }
 
-static int probe_impl(nfs_ctx* h, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch) {
-  if (!h || batch_frames < 1 || reps < 1 || !ms_per_launch) return NFS_ERR_INVALID_ARG;
-  Ctx& c = h->c;
-  if (!enter(c)) return c.status;
-  if (c.bin_only || c.band_width > 0) return NFS_ERR_STATE;
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (!NFS_CUDA(c, cudaEventCreate(&e0))) return c.status;
-  if (!NFS_CUDA(c, cudaEventCreate(&e1))) {
-    cudaEventDestroy(e0);
-    return c.status;
-  }
-  double bytes = 0.0;
-  launch_lag_probe(c, batch_frames, &bytes);  // warm-up
-  NFS_CUDA(c, cudaEventRecord(e0, c.stream));
-  for (int r = 0; r < reps; ++r) c.n_launches += launch_lag_probe(c, batch_frames, &bytes);
-  NFS_CUDA(c, cudaEventRecord(e1, c.stream));
-  NFS_CUDA(c, cudaStreamSynchronize(c.stream));
-  float ms = 0.f;
-  NFS_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  *ms_per_launch = (double)ms / reps;
-  if (bytes_per_launch) *bytes_per_launch = bytes;
-  return c.status;
-}
-int nfs_probe_lag_traffic(nfs_ctx* h, int batch_frames, int reps, double* ms_per_launch, double* bytes_per_launch) {
-  NFS_GUARDED(probe_impl(h, batch_frames, reps, ms_per_launch, bytes_per_launch))
-}
-
-static int guards_impl(nfs_ctx* h, int64_t* n_bad) {
-  if (!h) return NFS_ERR_INVALID_ARG;
-  Ctx& c = h->c;
-  if (!c.guard) return NFS_ERR_STATE;
-  if (!enter(c)) return c.status;
-  if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
-  std::vector<unsigned char> buf(kGuardBytes);
-  int64_t bad = 0;
-  for (const Ctx::Alloc& a : c.allocs) {
-    const char* base = static_cast<const char*>(a.base);
-    for (int side = 0; side < 2; ++side) {  // the zone in front of the buffer, then the one behind its 256-byte rounded end
-      if (!NFS_CUDA(c, cudaMemcpy(buf.data(), base + (side ? kGuardBytes + a.user_bytes : 0), kGuardBytes, cudaMemcpyDeviceToHost)))
-        return c.status;
-      for (unsigned char v : buf) bad += v != (unsigned char)kGuardByte;
-    }
-  }
-  if (n_bad) *n_bad = bad;
-  return bad == 0 ? NFS_OK : NFS_ERR_STATE;
-}
-int nfs_check_guards(nfs_ctx* h, int64_t* n_bad) { NFS_GUARDED(guards_impl(h, n_bad)) }
-
 int64_t nfs_num_frames(const nfs_ctx* h) { return h ? h->c.n_frames : 0; }
 int nfs_ring_capacity(const nfs_ctx* h) { return h ? h->c.R : 0; }
 int64_t nfs_device_bytes(const nfs_ctx* h) { return h ? h->c.dev_bytes : 0; }
-int64_t nfs_num_launches(const nfs_ctx* h) { return h ? h->c.n_launches : 0; }
-
-int nfs_set_launch_shape(nfs_ctx* h, int shape) {
-  if (!h || shape < 0 || shape > 2) return NFS_ERR_INVALID_ARG;
-  h->c.lag_shape = shape;
-  return NFS_OK;
-}
-
-static int plan_impl(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out,
-                     int cap) {
-  if (!lags_ok(lags, n_lags) || !out || cap < 7 || n_px < 32 || n_sm < 1) return NFS_ERR_INVALID_ARG;
-  Ctx c;
-  c.lags.assign(lags, lags + n_lags);
-  c.n_lags = n_lags;
-  c.Lmax = lags[n_lags - 1];
-  c.max_smem_optin = smem_optin;
-  if (!lag_plan(c, smem_per_sm, n_sm, (int64_t)n_px)) return NFS_ERR_INVALID_ARG;
-  const size_t need = 7 + c.groups.size() * 23 + c.tasks.size() * 4;
-  if (need > (size_t)cap) return NFS_ERR_INVALID_ARG;
-  int32_t* o = out;
-  *o++ = (int32_t)c.groups.size();
-  *o++ = (int32_t)c.tasks.size();
-  *o++ = c.lag_stages;
-  *o++ = (int32_t)c.lag_smem;
-  *o++ = c.lag_tpx;
-  *o++ = c.lag_ctas_per_sm;
-  *o++ = c.lag_slots;
-  for (const LagGroup& g : c.groups) {
-    *o++ = g.task0, *o++ = g.ntasks, *o++ = g.tau_min, *o++ = g.tau_max, *o++ = g.flags;
-    for (int w = 0; w < 16; ++w) *o++ = g.warp_task[w];
-    *o++ = g.cta0, *o++ = g.nctas;
-  }
-  for (const LagTask& t : c.tasks) *o++ = t.tau0, *o++ = t.cnt, *o++ = t.l0, *o++ = t.kind;
-  return (int)need;
-}
-int nfs_plan_lags(const int32_t* lags, int n_lags, int n_px, int smem_per_sm, int smem_optin, int n_sm, int32_t* out, int cap) {
-  NFS_GUARDED(plan_impl(lags, n_lags, n_px, smem_per_sm, smem_optin, n_sm, out, cap))
-}
-
-int nfs_set_profiling(nfs_ctx* h, int enable) {
-  if (!h) return NFS_ERR_INVALID_ARG;
-  h->c.prof = enable != 0;
-  return NFS_OK;
-}
-
-static int times_impl(nfs_ctx* h, double* ms, int64_t* launches) {
-  if (!h) return NFS_ERR_INVALID_ARG;
-  Ctx& c = h->c;
-  if (!enter(c)) return c.status;
-  if (!NFS_CUDA(c, cudaStreamSynchronize(c.stream))) return c.status;
-  for (size_t i = 0; i < c.ev_class.size(); ++i) {
-    float t = 0.f;
-    if (cudaEventElapsedTime(&t, c.ev_pool[2 * i], c.ev_pool[2 * i + 1]) == cudaSuccess) {
-      c.prof_ms[c.ev_class[i]] += (double)t;
-      c.prof_n[c.ev_class[i]] += 1;
-    }
-  }
-  c.ev_class.clear();
-  c.ev_used = 0;
-  for (int k = 0; k < kNumKernelClasses; ++k) {
-    if (ms) ms[k] = c.prof_ms[k];
-    if (launches) launches[k] = c.prof_n[k];
-    c.prof_ms[k] = 0.0;
-    c.prof_n[k] = 0;
-  }
-  return NFS_OK;
-}
-int nfs_get_kernel_times(nfs_ctx* h, double* ms, int64_t* launches) { NFS_GUARDED(times_impl(h, ms, launches)) }
 
 int nfs_reset(nfs_ctx* h) {
   if (!h) return NFS_ERR_INVALID_ARG;

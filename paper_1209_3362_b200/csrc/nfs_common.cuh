@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "../../include/nfs.h"
+#include "../../include/nfs_dev.h"  // internal code sees the debugging aids too (NFS_FLAG_GUARD is handled at create)
 
 namespace nfs {
 
@@ -214,5 +215,86 @@ int launch_absolute_I(Ctx& c, double* d_S2, double2* d_S1);  // S2 = sum |F_t|^2
 int launch_I2d(Ctx& c, double* d_dst);       // d_dst[P] = I2d in ring layout
 int launch_V2d(Ctx& c, double* d_dst);       // d_dst[P] = V2d (variance form) in ring layout
 int launch_D2d(Ctx& c, int l, double* d_dst);
+
+// ---- shared by nfs_api.cu (product ABI) and nfs_dev.cu (measurement / debugging ABI, dev build only) ----------------
+}  // namespace nfs
+
+struct nfs_ctx {
+  nfs::Ctx c;
+};
+
+namespace nfs {
+
+// guard zones of NFS_FLAG_GUARD (nfs_dev.h): bytes on either side of every device buffer, and their canary value
+constexpr size_t kGuardBytes = 64 << 10;
+constexpr int kGuardByte = 0xA5;
+
+// every entry point that touches the device runs on the context's device
+inline bool enter(Ctx& c) {
+  if (c.status != NFS_OK) return false;
+  int dev = -1;
+  if (!NFS_CUDA(c, cudaGetDevice(&dev))) return false;
+  if (dev != c.device && !NFS_CUDA(c, cudaSetDevice(c.device))) return false;
+  return true;
+}
+
+inline bool lags_ok(const int32_t* lags, int n_lags) {
+  if (!lags || n_lags < 1) return false;
+  for (int l = 0; l < n_lags; ++l)
+    if (lags[l] < 1 || (l > 0 && lags[l] <= lags[l - 1])) return false;
+  return true;
+}
+
+
+// ---- out-of-core band schedule (Fig. 2(b) L37) ----------------------------------------------------
+// Memory plan for a device that holds only `cap` Fourier frames: batch b, band width N* = cap - 2 b (a window of
+// N* + b OLD frames and b NEW frames).  Returns false if no band fits.
+inline bool band_memory_plan(int cap, int batch_frames, int* b_out, int* nstar_out) {
+  int b = batch_frames > 0 ? batch_frames : std::min(1024, cap / 4);
+  b = std::max(1, std::min(b, 8192));
+  const int nstar = cap - 2 * b;
+  if (nstar < 1) return false;
+  *b_out = b;
+  *nstar_out = nstar;
+  return true;
+}
+
+// The sweeps of bands 1 .. n_bands-1 over a stack of N frames, as a sequence of uploads and launches.  Band k holds
+// the requested lags in (k N*, (k+1) N*], smallest tmin, largest tmax.  Its sweep walks the frames s = tmin .. N-1 in
+// batches of b: the batch goes into the NEW ring, the OLD frames s - tmax .. s - tmin it pairs with are kept in the
+// OLD ring, every frame of the window being uploaded once per band (the paper's FIFO: "one diagonal is filled by
+// subsequently replacing one FIFO image and uploading one 'current image'").  The same walk serves the device (uploads
+// and kernel launches) and the host-only transfer count of nfs_band_plan.
+template <typename UploadOld, typename UploadNew, typename Launch>
+bool band_sweeps(int64_t N, int b, int n_bands, const std::vector<int>& band_l0, const std::vector<int32_t>& lags,
+                 UploadOld&& upload_old, UploadNew&& upload_new, Launch&& launch) {
+  for (int k = 1; k < n_bands; ++k) {
+    const int l0 = band_l0[(size_t)k], l1 = band_l0[(size_t)k + 1];
+    if (l1 <= l0) continue;  // no requested lag in this band
+    const int64_t tmin = lags[(size_t)l0], tmax = lags[(size_t)l1 - 1];
+    int64_t old_next = -1;  // first OLD frame not yet in the OLD ring
+    for (int64_t t0 = tmin; t0 < N; t0 += b) {
+      const int bb = (int)std::min<int64_t>(b, N - t0);
+      const int64_t lo = std::max<int64_t>(0, t0 - tmax), hi = t0 + bb - 1 - tmin;  // OLD frames lo .. hi
+      const int64_t from = std::max(lo, old_next);
+      if (hi >= from && !upload_old(from, hi + 1)) return false;
+      old_next = std::max(old_next, hi + 1);
+      if (!upload_new(t0, t0 + bb)) return false;
+      if (!launch(t0, bb, k)) return false;
+    }
+  }
+  return true;
+}
+
+// Nothing may throw across the C boundary: allocation failures of the host-side containers become NFS_ERR_OOM.
+#define NFS_GUARDED(expr)            \
+  try {                              \
+    return (expr);                   \
+  } catch (const std::bad_alloc&) {  \
+    return NFS_ERR_OOM;              \
+  } catch (...) {                    \
+    return NFS_ERR_STATE;            \
+  }
+
 
 }  // namespace nfs

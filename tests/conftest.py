@@ -8,6 +8,13 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+# the tests exercise the measurement / debugging aids of include/nfs_dev.h as well: they run against the dev build
+# (same object files as the product library plus nfs_dev.cu and the probe); tests/test_abi.py checks what each exports
+from paper_1209_3362_b200 import binding as _binding  # noqa: E402
+
+_binding.use_dev_library()
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 

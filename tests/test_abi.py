@@ -20,10 +20,21 @@ def lib():
     return binding.load_library()
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "nfs.h")).read()
+def _declared_symbols(header="nfs.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"NFS_API\s+[\w\s\*]+?\b(nfs_\w+)\s*\(", src)))
+
+
+def _exported(path):
+    """nfs_* functions in the dynamic symbol table of a shared library (binutils nm), or None without nm."""
+    import shutil
+    import subprocess
+
+    if not shutil.which("nm"):
+        return None
+    out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True, check=True).stdout
+    return sorted(ln.split()[-1] for ln in out.splitlines() if ln.split()[-2:-1] == ["T"] and ln.split()[-1].startswith("nfs_"))
 
 
 def test_header_declares_the_north_star_calls():
@@ -33,7 +44,9 @@ def test_header_declares_the_north_star_calls():
         assert required in names, names
 
 
-def test_library_exports_every_declared_symbol(lib):
+def test_product_library_exports_exactly_the_public_header(lib):
+    """libnfs_b200.so = include/nfs.h, no more (measurement and debug aids do not belong in the product ABI)
+    and no less; the binding's product table names the same symbols."""
     from paper_1209_3362_b200 import binding
 
     raw = C.CDLL(binding.LIB_PATH)
@@ -41,17 +54,38 @@ def test_library_exports_every_declared_symbol(lib):
     assert len(declared) >= 15
     for name in declared:
         assert hasattr(raw, name), "libnfs_b200.so does not export %s" % name
-    bound = {s[0] for s in binding.SYMBOLS}
-    assert bound == set(declared), (sorted(bound ^ set(declared)))
+    for name in _declared_symbols("nfs_dev.h"):
+        assert not hasattr(raw, name), "libnfs_b200.so exports the dev-only %s" % name
+    exported = _exported(binding.LIB_PATH)
+    if exported is not None:
+        assert exported == declared, sorted(set(exported) ^ set(declared))
+    assert {s[0] for s in binding.SYMBOLS} == set(declared)
+
+
+def test_dev_library_exports_both_headers(lib):
+    """libnfs_b200_dev.so (what the tests and bench.py load) = include/nfs.h + include/nfs_dev.h."""
+    from paper_1209_3362_b200 import binding
+
+    raw = C.CDLL(binding.DEV_LIB_PATH)
+    dev = _declared_symbols("nfs_dev.h")
+    both = sorted(set(_declared_symbols()) | set(dev))
+    assert len(dev) == 8 and not set(dev) & set(_declared_symbols())
+    for name in both:
+        assert hasattr(raw, name), "libnfs_b200_dev.so does not export %s" % name
+    exported = _exported(binding.DEV_LIB_PATH)
+    if exported is not None:
+        assert exported == both, sorted(set(exported) ^ set(both))
+    assert {s[0] for s in binding.DEV_SYMBOLS} == set(dev)
 
 
 def test_no_torch_or_python_symbols_in_the_abi():
     """The boundary is plain C: the header includes only stdint.h and uses no C++/torch types."""
-    src = open(os.path.join(ROOT, "include", "nfs.h")).read()
-    assert re.findall(r"#include\s+[<\"]([^>\"]+)[>\"]", src) == ["stdint.h"]
-    assert 'extern "C"' in src
-    for bad in ("torch", "at::", "std::", "Tensor"):
-        assert bad not in src
+    for header, includes in (("nfs.h", ["stdint.h"]), ("nfs_dev.h", ["nfs.h"])):
+        src = open(os.path.join(ROOT, "include", header)).read()
+        assert re.findall(r"#include\s+[<\"]([^>\"]+)[>\"]", src) == includes
+        assert 'extern "C"' in src
+        for bad in ("torch", "at::", "std::", "Tensor"):
+            assert bad not in src
 
 
 def test_strerror(lib):
