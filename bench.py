@@ -257,6 +257,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-hbm-regime", action="store_true", help="skip the small-batch run of the lag kernel")
+    ap.add_argument("--mode", default="path", choices=["path", "bin-only", "banded", "fit"],
+                    help="path: the headline line (default).  Secondary measurements of the SURVEY 8(f) rows, one JSON line each, "
+                         "single GPU: bin-only (NFS_FLAG_BIN_ONLY against the 2-D mode), banded (out-of-core band schedule "
+                         "against the in-memory one; --bands sets alpha), fit (k_fit_eq1 device time)")
+    ap.add_argument("--bands", type=int, default=3, help="--mode banded: number of lag bands alpha the ring cap forces")
     ap.add_argument("--sharding", default="replicas", choices=["replicas", "time"],
                     help="N > 1: 'replicas' = every rank analyses its own stack (weak scaling, the default); 'time' = ONE "
                          "stack cut into time chunks with halos, one NCCL all-reduce of the partial sums (strong scaling, "
@@ -271,7 +276,106 @@ def main():
         cfg.N = args.frames
     if args.impl == "reference":
         return run_reference(args, cfg)
+    if args.mode != "path":
+        return run_mode(args, cfg)
     run_ours(args, cfg)
+
+
+def run_mode(args, cfg):
+    """Secondary measurements: one GPU, stack resident in HBM, CUDA events on the library's
+    stream, W warm-up and K timed steps; one JSON line (not the headline line: `metric` names what is measured)."""
+    import numpy as np
+    import torch
+    import synth
+    from paper_1209_3362_b200 import binding
+
+    binding.use_dev_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = "cuda:0"
+    stack = synth.make_stack(cfg, dev)
+    stream = torch.cuda.Stream(device=dev)
+    chunk = cfg.chunk or cfg.N
+
+    def timed(nfs, after=None):
+        def step():
+            nfs.reset()
+            for i in range(0, cfg.N, chunk):
+                nfs.push(stack[i:i + chunk])
+            return nfs.finalize()
+        for _ in range(max(args.warmup, 1)):
+            out = step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            out = step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps, out
+
+    base = dict(n_gpus=1, steps=args.steps, warmup=args.warmup, dtype="f32", data="synthetic",
+                config=dict(workload=cfg.name, W=cfg.W, H=cfg.H, frames=cfg.N, n_lags=len(cfg.lags), lag_max=cfg.lags[-1],
+                            n_qbins=cfg.n_qbins, inputs="stack resident in HBM, larger than L2"))
+    if args.mode == "bin-only":
+        full = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch)
+        ms_full, (D_full, I_full, _) = timed(full)
+        bytes_full = full.device_bytes
+        full.close()
+        bo = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch, bin_only=True)
+        ms_bo, (D_bo, I_bo, cnt) = timed(bo)
+        bytes_bo = bo.device_bytes
+        bo.close()
+        nz = cnt > 0
+        out = dict(base, metric="ms per stack, NFS_FLAG_BIN_ONLY (PAPER.md:L41)", value=ms_bo, unit="ms", higher_is_better=False,
+                   two_d_mode_ms=ms_full, slowdown_vs_2d=ms_bo / ms_full, device_bytes=bytes_bo, device_bytes_2d=bytes_full,
+                   max_rel_diff_binned_D_vs_2d=float(np.max(np.abs(D_bo[:, nz] - D_full[:, nz]) / D_full[:, nz])))
+    elif args.mode == "banded":
+        alpha = max(2, args.bands)
+        b = args.batch or 128
+        nstar = (cfg.lags[-1] + alpha - 1) // alpha
+        cap = nstar + 2 * b
+        mem = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=b)
+        ms_mem, (D_mem, _, cnt) = timed(mem)
+        mem.close()
+        bd = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=b, ring_frames_cap=cap, max_frames=cfg.N)
+        ms_bd, (D_bd, _, _) = timed(bd)
+        tc = bd.transfer_counts()   # of the last step (reset clears them)
+        ring = bd.ring_capacity
+        bd.close()
+        plan = binding.nfs_band_plan(cfg.N, cfg.lags, cap, b)
+        a = tc["bands"]
+        nz = cnt > 0
+        out = dict(base, metric="ms per stack, out-of-core band schedule (PAPER.md:L33, Fig. 2(b))", value=ms_bd, unit="ms",
+                   higher_is_better=False, in_memory_ms=ms_mem, slowdown_vs_in_memory=ms_bd / ms_mem, bands=a,
+                   band_width=tc["band_width"], batch=b, ring_frames_cap=cap, ring_frames=ring,
+                   fourier_frames_uploaded=tc["h2d_frames"], fourier_frames_downloaded=tc["d2h_frames"],
+                   band_plan_uploads=plan["old_uploads"] + plan["new_uploads"],
+                   paper_N_FFT=cfg.N * (2 * a - 3 + 2.0 / a),
+                   max_rel_diff_binned_D_vs_in_memory=float(np.max(np.abs(D_bd[:, nz] - D_mem[:, nz]) / D_mem[:, nz])))
+    else:  # fit
+        nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, stream=stream, batch_frames=args.batch)
+        for i in range(0, cfg.N, chunk):
+            nfs.push(stack[i:i + chunk])
+        nfs.finalize()
+        nfs.set_profiling(True)
+        for _ in range(max(args.warmup, 1)):
+            nfs.fit_eq1(), nfs.variance()
+        nfs.kernel_times()
+        for _ in range(args.steps):
+            nfs.variance()               # k_bin alone
+        ms_bin = nfs.kernel_times()["bin"][0] / args.steps
+        t0 = time.time()
+        for _ in range(args.steps):
+            A, Cq, G, chi2 = nfs.fit_eq1()  # k_bin + k_fit_eq1
+        call_ms = (time.time() - t0) / args.steps * 1e3
+        ms_both = nfs.kernel_times()["bin"][0] / args.steps
+        nfs.close()
+        out = dict(base, metric="k_fit_eq1 device time (PAPER.md:L23-25, Eq. 1; per-|q| fit of A, C, Gamma)", value=(ms_both - ms_bin) * 1e3,
+                   unit="us", higher_is_better=False, k_bin_us=ms_bin * 1e3, nfs_fit_eq1_call_ms=call_ms,
+                   bins_fitted=int((G > 0).sum()))
+    print(json.dumps(out), flush=True)
 
 
 def run_ours(args, cfg):

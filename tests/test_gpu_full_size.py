@@ -95,6 +95,23 @@ def test_full_size_binned_and_per_pixel(binding, oracle, idx):
     _compare_pixels(g_I2d, ref.I2d, "I2d")
 
 
+def test_config1_bin_only_full_size(binding, oracle):
+    """BASELINE.json configs[1] at full size through NFS_FLAG_BIN_ONLY: binned D of all 100 lags, I,
+    counts and pair counts against the live half-plane oracle; run-to-run bit-identical (fixed summation order)."""
+    cfg = synth.config(1)
+    st = synth.make_stack(cfg, "cuda")
+    outs = []
+    for _ in range(2):
+        nfs = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, bin_only=True)
+        nfs.push(st)
+        outs.append(nfs.finalize() + (nfs.pair_counts(),))
+        nfs.close()
+    ref = oracle.structure_function_half(st.cpu().numpy(), cfg.lags, cfg.n_qbins)
+    D, I_q, cnt, npairs = outs[0]
+    _compare_binned(D, I_q, cnt, npairs, ref.D, ref.I_q, ref.counts, ref.n_pairs)
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
 def test_config4_full_length_streamed(binding, oracle):
     """BASELINE.json configs[4]: 1024^2 x 10 000 frames pushed in chunks of 256, all lags 1..1000, 256 bins: ten lag
     groups, the Fourier ring (1000 + 1024 slots) wraps four times.  Binned D of ALL 1000 lags, I, counts, pair counts,
@@ -125,12 +142,26 @@ def test_config4_full_length_streamed(binding, oracle):
         ref = None
     g_pix = np.stack([nfs.D2d(l)[ky, kx] for l in lag_idx])
     g_Ipix = nfs.I2d()[ky, kx]
+    bytes_2d = nfs.device_bytes
     nfs.close()
+    # the same stack through NFS_FLAG_BIN_ONLY (the workload that mode exists for: 4.2 GB of 2-D totals
+    # shrink to a scratch of one lag group); compared below with the same oracle values, every lag
+    bo = binding.NFS(cfg.W, cfg.H, cfg.lags, cfg.n_qbins, bin_only=True)
+    for i in range(0, cfg.N, cfg.chunk):
+        bo.push(st[i:i + cfg.chunk])
+    D_bo, I_bo, cnt_bo = bo.finalize()
+    npairs_bo = bo.pair_counts()
+    bytes_bo = bo.device_bytes
+    with pytest.raises(binding.NFSError):
+        bo.D2d(0)
+    bo.close()
+    assert bytes_2d - bytes_bo > 3.5e9, (bytes_2d, bytes_bo)
     if ref is None:
         ref = g4.oracle_values(st.cpu().numpy(), cfg, oracle, lag_idx)
     del st
     sel_lags = [cfg.lags[l] for l in lag_idx]
     _compare_binned(D[lag_idx], I_q, cnt, npairs[lag_idx], ref["D"], ref["I_q"], ref["counts"], ref["n_pairs"])
+    _compare_binned(D_bo[lag_idx], I_bo, cnt_bo, npairs_bo[lag_idx], ref["D"], ref["I_q"], ref["counts"], ref["n_pairs"])
     assert int(cnt.sum()) == 823468
     assert ref["n_pairs"].tolist() == [cfg.N - t for t in sel_lags]
     # sampled pixels of every compared lag; threshold on the maximum of the whole stored [lags][pixels] array (R15),
