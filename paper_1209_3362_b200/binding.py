@@ -73,6 +73,7 @@ DEV_SYMBOLS = [
 KERNEL_CLASSES = ["ref_setup", "fft", "unused", "lag_accum", "bin"]
 NFS_FLAG_BIN_ONLY = 1
 NFS_FLAG_GUARD = 2
+NFS_FLAG_DIRECT = 4
 SHAPE_AUTO, SHAPE_ONE_TILE, SHAPE_PERSISTENT = 0, 1, 2
 
 _lib = None
@@ -225,7 +226,7 @@ class NFS:
     the caller of nfs_push_frames."""
 
     def __init__(self, W, H, lags, n_qbins, stream=None, batch_frames=0, bin_only=False, ring_frames_cap=0, max_frames=0,
-                 guard=False):
+                 guard=False, direct=False):
         import torch
 
         self.lib = load_library()
@@ -236,7 +237,8 @@ class NFS:
             stream = torch.cuda.Stream()
         self._stream = stream  # without a device nfs_create itself reports NFS_ERR_CUDA: no fallback
         self.handle = nfs_create(W, H, self.lags, n_qbins, stream.cuda_stream if stream is not None else None, batch_frames,
-                                 (NFS_FLAG_BIN_ONLY if bin_only else 0) | (NFS_FLAG_GUARD if guard else 0), ring_frames_cap,
+                                 (NFS_FLAG_BIN_ONLY if bin_only else 0) | (NFS_FLAG_GUARD if guard else 0) |
+                                 (NFS_FLAG_DIRECT if direct else 0), ring_frames_cap,
                                  max_frames)
 
     def transfer_counts(self):

@@ -252,7 +252,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   *out = nullptr;
   if (!lags_ok(lags, n_lags) || n_qbins < 1 || n_qbins > (1 << 20) || batch_frames < 0 || batch_frames > 8192)
     return NFS_ERR_INVALID_ARG;
-  if ((flags & ~(unsigned)(NFS_FLAG_BIN_ONLY | NFS_FLAG_GUARD)) != 0) return NFS_ERR_INVALID_ARG;
+  if ((flags & ~(unsigned)(NFS_FLAG_BIN_ONLY | NFS_FLAG_GUARD | NFS_FLAG_DIRECT)) != 0) return NFS_ERR_INVALID_ARG;
   if (!is_pow2(W) || !is_pow2(H) || W < 32 || H < 32 || W > 4096 || H > 4096) return NFS_ERR_INVALID_ARG;
   if (W != H) return NFS_ERR_UNSUPPORTED;
   if (n_lags > 65533) return NFS_ERR_INVALID_ARG;  // one grid row of the binning kernel per lag (+ I and V)
@@ -281,6 +281,7 @@ int create_impl(nfs_ctx** out, int W, int H, const int32_t* lags, int n_lags, in
   c.R = c.Lmax + c.B;
   c.bin_only = (flags & NFS_FLAG_BIN_ONLY) != 0;
   c.guard = (flags & NFS_FLAG_GUARD) != 0;
+  c.direct_only = (flags & NFS_FLAG_DIRECT) != 0;
   // band schedule: asked for by a ring capacity that cannot hold the whole lag window plus a batch
   if (ring_frames_cap < 0 || max_frames < 0) return NFS_ERR_INVALID_ARG;
   if (ring_frames_cap > 0 && ring_frames_cap < c.Lmax + (batch_frames > 0 ? batch_frames : 1)) {

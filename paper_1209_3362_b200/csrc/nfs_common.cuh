@@ -61,6 +61,7 @@ struct Ctx {
   int device = 0;
   int n_sm = 0;
   bool bin_only = false;  // accumulate |q|-binned totals only (no 2-D spectra kept)
+  bool direct_only = false;  // NFS_FLAG_DIRECT: no neighbouring-lag recurrence, every lag accumulated as |z_s - z_o|^2
   bool guard = false;     // NFS_FLAG_GUARD: canary zones around every device buffer (nfs_check_guards)
   struct Alloc {
     void* base;         // what cudaMalloc returned

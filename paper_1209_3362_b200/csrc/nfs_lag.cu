@@ -859,7 +859,7 @@ static bool plan_with(Ctx& c, int slots, int smem_sm, int n_sm, int64_t P, int d
     int j = i;
     while (j + 1 < c.n_lags && L[j + 1] == L[j] + 1 && band_of(L[j + 1]) == band_of(L[i])) ++j;
     const int len = j - i + 1;
-    if (len >= kDenseMin) {
+    if (len >= kDenseMin && !c.direct_only) {  // NFS_FLAG_DIRECT: every lag is summed by the plain difference form
       const int nt = (len + dense_max - 1) / dense_max;
       int l = i;
       for (int k = 0; k < nt; ++k) {

@@ -20,10 +20,10 @@ def binding():
     return b
 
 
-def run(binding, stack_np, lags, n_b, batch=0):
+def run(binding, stack_np, lags, n_b, batch=0, direct=False):
     st = torch.from_numpy(np.ascontiguousarray(stack_np)).cuda()
     N, H, W = st.shape
-    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch)
+    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch, direct=direct)
     nfs.push(st)
     D, I_q, cnt = nfs.finalize()
     D2d = np.stack([nfs.D2d(l) for l in range(len(lags))])
@@ -77,6 +77,14 @@ def test_telegraph_stack(binding):
         else:
             m = ref > 1e-6 * ref.max()
             assert (np.abs(D2d[l] - ref)[m] / ref[m]).max() < 1e-4
+    # NFS_FLAG_DIRECT: no recurrence anywhere, so every even lag is an exact zero again
+    Dd, _, _, D2d_direct, _ = run(binding, st, lags, 16, batch=8, direct=True)
+    for l, tau in enumerate(lags):
+        if tau % 2 == 0:
+            assert np.all(D2d_direct[l] == 0.0) and np.all(Dd[l] == 0.0)
+        else:
+            m = ref > 1e-6 * ref.max()
+            assert (np.abs(D2d_direct[l] - ref)[m] / ref[m]).max() < 1e-4
 
 
 def test_slowly_drifting_fringe_keeps_small_lags_accurate(binding):
@@ -109,6 +117,11 @@ def test_slowly_drifting_fringe_keeps_small_lags_accurate(binding):
     m = R > 1e-6 * R.max()
     assert (np.abs(D2d - R)[m] / R[m]).max() < TOL_PIXEL
     assert np.abs(D2d - R)[~m].max() <= recurrence_floor(R, lags)
+    # NFS_FLAG_DIRECT: the error no longer knows about the excursion Z: a few fp32 roundings of D itself
+    _, _, _, D2d_direct, _ = run(binding, st, lags, 16, direct=True)
+    err_d = np.abs(D2d_direct[:, k0y, k0x] - r)
+    assert (err_d / r).max() < 5e-6, (err_d / r).max()
+    assert (np.abs(D2d_direct - R)[m] / R[m]).max() < TOL_PIXEL
 
 
 def test_travelling_fringe_closed_form(binding):

@@ -25,9 +25,9 @@ def binding():
     return b
 
 
-def gpu_run(binding, stack, lags, n_b, batch=0, shape=0, split=None, want_2d=True):
+def gpu_run(binding, stack, lags, n_b, batch=0, shape=0, split=None, want_2d=True, direct=False):
     N, H, W = stack.shape
-    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch)
+    nfs = binding.NFS(W, H, lags, n_b, batch_frames=batch, direct=direct)
     nfs.set_launch_shape(shape)
     if split:
         i = 0
@@ -90,6 +90,25 @@ def cfg0():
 
     ref = o.structure_function(st.cpu().numpy(), cfg.lags, cfg.n_qbins, want_2d=True)
     return cfg, st, ref
+
+
+def test_direct_form_option(binding, cfg0):
+    """NFS_FLAG_DIRECT (include/nfs.h): the same results without the neighbouring-lag recurrence — config 0 in both launch
+    shapes, and a 128^2 x 300 stack with lags 1..60 (several lag groups of lag-list tasks only)."""
+    cfg, st, ref = cfg0
+    for shape in (1, 2):
+        check_against_oracle(gpu_run(binding, st, cfg.lags, cfg.n_qbins, shape=shape, direct=True), ref, cfg.W)
+    from oracle import nfs_oracle as o
+
+    lags = list(range(1, 61))
+    c1 = synth.config(1, W=128, N=300, lags=lags, n_qbins=32)
+    s1 = synth.make_stack(c1, "cuda")
+    r1 = o.structure_function(s1.cpu().numpy(), lags, c1.n_qbins, want_2d=True)
+    g1 = gpu_run(binding, s1, lags, c1.n_qbins, direct=True)
+    check_against_oracle(g1, r1, c1.W)
+    g0 = gpu_run(binding, s1, lags, c1.n_qbins)
+    nz = r1.counts > 0
+    assert relerr(g1["D"][:, nz], g0["D"][:, nz]).max() < 1e-5          # the two forms agree far inside the tolerance
 
 
 @pytest.mark.parametrize("shape,batch,split", [(0, 0, None), (1, 0, None), (0, 5, None), (0, 0, 3), (0, 7, 5),
